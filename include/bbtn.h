@@ -1,0 +1,201 @@
+/*
+ * bbtn.h -- C ABI of the B200-native BBTN hot path.
+ *
+ * Exact contraction of counting-tropical tensor networks, batched over
+ * branch-and-bound leaves (arxiv/paper_2602_05470; citations are PAPER.md:<line>).
+ *
+ *   element  = (energy, count)                       PAPER.md:53 (counting), :55 (zero = (inf,0))
+ *   a (.) b  = (ea + eb, ca * cb)                    PAPER.md:49 (x (.) y = x + y)
+ *   a (+) b  = the better energy; counts add on ties PAPER.md:49 (x (+) y = min(x,y)), :53
+ *
+ * The engine works in MAX-plus on negated Ising energies (the paper's min-sum
+ * mirrored, reading A1); MIS is natively a maximisation.
+ * Results are reported in the paper's units: Ising min H (Eq. 1),
+ * MIS max set weight.
+ *
+ * Conventions that hold for EVERY entry point
+ *   - plain C, no C++/torch types; all integers are fixed-width.
+ *   - pointers are HOST pointers unless the parameter is documented "device" or the
+ *     handle was built with BBTN_IO_DEVICE (then assign/energy/count/count_mod/bound
+ *     of the batched calls are device pointers and the call is asynchronous on
+ *     `cuda_stream`; with host pointers the call returns after the results landed).
+ *   - the caller owns every array it passes; the library copies what it keeps.
+ *     The handle owns all device memory, plans and CUDA graphs it creates.
+ *   - every function returns a bbtn_status; on error no output is written and the
+ *     message is available from bbtn_last_error(handle) (handle may be NULL for
+ *     errors of handle-less calls: thread-local).
+ *   - a handle is used by one host thread at a time.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - integer arithmetic only: results are bit-identical across runs, trees,
+ *     tilings and batch sizes.
+ *   - there is NO CPU fallback: without a CUDA device every compute call returns
+ *     BBTN_ECUDA.
+ */
+#ifndef BBTN_H_
+#define BBTN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bbtn_handle bbtn_handle;            /* opaque, library-owned */
+
+typedef enum { BBTN_ISING = 0, BBTN_MIS = 1 } bbtn_kind;
+
+typedef enum {
+  BBTN_OK = 0,
+  BBTN_EINVAL = 1,     /* malformed argument (bad vertex id, duplicate fixed vertex, bad tree ...) */
+  BBTN_ENOMEM = 2,     /* host or device allocation failed                                        */
+  BBTN_ECUDA = 3,      /* CUDA runtime error or no device                                         */
+  BBTN_ESHAPE = 4,     /* an intermediate would exceed max_elements_per_leaf (T_target)           */
+  BBTN_ERANGE = 5      /* sum of |couplings| + |fields/weights| exceeds BBTN_ENERGY_LIMIT         */
+} bbtn_status;
+
+/* Energy of the semiring zero element ("(inf, 0)"); its count is 0.
+ * Finite energies obey |e| <= BBTN_ENERGY_LIMIT, so NEG_INF + NEG_INF still fits an int32 and any
+ * energy below -2^29 is canonicalised back to (BBTN_NEG_INF, 0) (reading A8).
+ * Zero-ness is decided by the ENERGY, never by count == 0. */
+#define BBTN_NEG_INF (-(1 << 30))
+#define BBTN_ENERGY_LIMIT (1 << 28)
+
+/* flags of bbtn_problem_desc.flags */
+#define BBTN_COUNT_CRT 0x1u   /* also keep counts mod P1 and mod P2 (three passes over the tree)   */
+#define BBTN_IO_DEVICE 0x2u   /* batched calls take/return DEVICE pointers, asynchronous           */
+#define BBTN_NO_GRAPH  0x4u   /* launch kernels one by one instead of replaying a CUDA graph       */
+#define BBTN_FORCE_STREAMING 0x10u /* tuning/testing: never use the tiled GEMM + permute path          */
+#define BBTN_FORCE_TILED     0x20u /* tuning/testing: permute + tiled GEMM wherever an index is summed */
+
+#define BBTN_P1 2147483647u   /* 2^31 - 1  */
+#define BBTN_P2 2147483629u   /* 2^31 - 19 */
+
+/* The problem: a graph G=(V,E) with couplings/fields (Eq. 1) or vertex weights
+ * (MWIS), plus a contraction tree.  Input tensors are numbered
+ *   0 .. n_edges-1                      the bond tensor of edge e on indices (s_u, s_v)
+ *   n_edges .. n_edges+n_vertices-1     the vertex tensor of vertex i on index (s_i)
+ * and step t of the SSA tree contracts ids tree_l[t], tree_r[t] into id n_inputs + t; a complete
+ * tree has n_inputs - 1 steps.  tree_l == NULL: the library derives an elimination-order tree
+ * itself, per fixed set (results do not depend on the tree, only speed and width do). */
+typedef struct {
+  int32_t kind;                    /* bbtn_kind                                                  */
+  int32_t n_vertices, n_edges;
+  const int32_t *edge_u, *edge_v;  /* [n_edges], 0 <= u != v < n_vertices, no duplicate edges    */
+  const int32_t *edge_w;           /* Ising: integer J_ij per edge (NULL = all +1). MIS: ignored */
+  const int32_t *vertex_w;         /* Ising: integer h_i (NULL = no field). MIS: w_i (NULL = 1)  */
+  int32_t n_steps;                 /* 0 with tree_l == NULL, else n_edges + n_vertices - 1       */
+  const int32_t *tree_l, *tree_r;  /* [n_steps] or NULL                                          */
+  int64_t max_elements_per_leaf;   /* T_target of Eq. 4, in ELEMENTS; 0 = 2^28     */
+  uint32_t flags;
+} bbtn_problem_desc;
+
+/* What the planner derived for one fixed-set signature and batch size. */
+typedef struct {
+  int32_t n_nodes;            /* pairwise contraction steps that launch work                       */
+  int32_t n_variant_nodes;    /* of which depend on the leaf assignment (the rest run once)        */
+  int32_t max_rank;           /* log2 of the largest tensor of one leaf (contraction width)        */
+  int32_t n_gemm_tiled, n_absorb, n_permute, n_trace;   /* kernel launches per count ring, by kind */
+  int64_t rho;                /* Eq. 4 with T_target = max_elements_per_leaf                       */
+  double  fma_variant;        /* tropical FMAs per leaf in leaf-variant nodes                      */
+  double  fma_invariant;      /* tropical FMAs in leaf-invariant nodes (once per call)             */
+  double  bytes_per_call;     /* algorithmic bytes read+written by all kernels for this B          */
+  int64_t workspace_bytes;    /* device memory the plan holds for this B                           */
+} bbtn_plan_info;
+
+/* Build a handle: validates and copies the problem (graph, weights, tree).  Host only: device
+ * tables and arenas are created by the first batched call.  Errors: EINVAL, ERANGE, ENOMEM. */
+int bbtn_build(const bbtn_problem_desc *desc, bbtn_handle **out);
+
+/* Contract one batch of B leaves that share the fixed set F (Eq. 3: the reduced TN
+ * with s_{V_f} = x; "same topology but different contents").
+ *   fixed_vertices [n_fixed]   distinct vertex ids (host, always)
+ *   assign         [B][n_fixed] 0/1; 1 <=> sigma = +1 (Ising) / vertex in the set (MIS)
+ *   energy         [B] int32   Ising: min over the free spins of H (fixed-fixed terms included),
+ *                              so min_b energy[b] = E0;  MIS: max set weight given the assignment
+ *   count          [B] uint64  number of optimal completions, mod 2^64
+ *   count_mod      [B][2] uint32 residues mod BBTN_P1, BBTN_P2 (needs BBTN_COUNT_CRT), or NULL
+ * An infeasible leaf (MIS: two adjacent vertices fixed to 1) returns energy BBTN_NEG_INF, count 0.
+ * n_fixed = 0 with B = 1 is the unbranched contraction (assign may be NULL).
+ * Steps run on the device: K1 construct, K2 permute, K3 counting-tropical GEMM, K4 trace.
+ * Errors: EINVAL, ESHAPE, ENOMEM, ECUDA. */
+int bbtn_contract_batch(bbtn_handle *h,
+                        const int32_t *fixed_vertices, int32_t n_fixed,
+                        const uint8_t *assign, int64_t B,
+                        int32_t *energy, uint64_t *count, uint32_t *count_mod,
+                        void *cuda_stream);
+
+/* Plan (or look up) the signature without running it. */
+int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed_vertices, int32_t n_fixed, int64_t B,
+                    bbtn_plan_info *info);
+
+/* Local bounds for pruning ("evaluating local energy contributions over a subset
+ * of variables R"; reading A15).  Regions are disjoint vertex sets in CSR form
+ * (region_offsets [n_regions+1], region_vertices); fixed vertices listed in a region are ignored;
+ * a region may hold at most 20 free vertices.
+ *   bound[b] = exact value of every term whose endpoints are all fixed
+ *            + sum_j max over the free vertices of R_j of the terms inside R_j u F touching R_j
+ *            + for every other term its largest entry compatible with the fixed endpoints
+ * in the units of energy[]: Ising bound[b] <= energy[b] (a LOWER bound on min H), MIS
+ * bound[b] >= energy[b].  Infeasible leaf: BBTN_NEG_INF (MIS).  One warp per (leaf, region) (K5). */
+int bbtn_region_bound(bbtn_handle *h,
+                      const int32_t *region_offsets, const int32_t *region_vertices, int32_t n_regions,
+                      const int32_t *fixed_vertices, int32_t n_fixed,
+                      const uint8_t *assign, int64_t B,
+                      int32_t *bound, void *cuda_stream);
+
+/* Host branch-and-bound driver (global pruning :67; S6): depth-first
+ * over `branch_vertices` in the given order, `chunk` levels at a time; every partial assignment is
+ * bounded with bbtn_region_bound and discarded iff its bound is strictly worse than the incumbent
+ * (ties kept, reading A14); surviving full assignments are contracted in batches of <= max_batch
+ * with bbtn_contract_batch and (+)-accumulated.
+ *   incumbent_hint: energy (reported units) of some feasible configuration known to the caller,
+ *   used only to prune earlier; BBTN_NEG_INF = none.  A hint better than the true optimum
+ *   makes the search return (BBTN_NEG_INF, 0).
+ *   energy/count/count_mod: the exact optimum over ALL configurations; stats[0..3] = nodes
+ *   generated, pruned, leaves contracted, contract calls.  Host pointers only. */
+int bbtn_solve_bb(bbtn_handle *h,
+                  const int32_t *branch_vertices, int32_t n_branch, int32_t chunk,
+                  const int32_t *region_offsets, const int32_t *region_vertices, int32_t n_regions,
+                  int64_t max_batch, int32_t incumbent_hint, int32_t use_pruning,
+                  int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats,
+                  void *cuda_stream);
+
+/* Raw batched counting-tropical GEMM (K3 alone; the config-4 sweep):
+ *   C[b,m,n] = (+)_k A[b,m,k] (.) B[b,k,n]
+ * ALL pointers are DEVICE pointers.  Row-major: A [batch][M][K], B [batch][K][N], C [batch][M][N];
+ * stride* are the ELEMENT distances between consecutive batch entries (0 = operand shared by the
+ * whole batch).  Energies int32 (<= -2^29 means the zero element; outputs are canonical),
+ * counts uint64 mod 2^64.  M, N, K >= 1, any size (ragged tiles are handled).
+ * count_bits: upper bound on log2(count+1) of BOTH operands that the caller guarantees
+ * (64 = no promise; <= 32 selects the 32x32->64 multiply fast path).  Asynchronous on cuda_stream. */
+int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,
+                               const int32_t *Ae, const uint64_t *Ac,
+                               const int32_t *Be, const uint64_t *Bc,
+                               int32_t *Ce, uint64_t *Cc,
+                               int64_t strideA, int64_t strideB, int64_t strideC,
+                               int32_t count_bits, void *cuda_stream);
+
+/* Raw batched bit permutation (K2 alone): dst[b][pi(i)] = src[b][i] for i in [0, 2^rank), where
+ * bit j of pi(i) is bit perm[j] of i (perm is a HOST array, a permutation of 0..rank-1).
+ * Both planes (int32 energies, uint64 counts) move; DEVICE pointers; asynchronous. */
+int bbtn_permute_batched(int32_t rank, const int32_t *perm, int64_t batch,
+                         const int32_t *src_e, const uint64_t *src_c,
+                         int32_t *dst_e, uint64_t *dst_c, void *cuda_stream);
+
+/* Integer-pipe microbenchmarks (register-only, no memory traffic) that define the ALU roofline of
+ * K3.  which: 0 = IADD3 chain, 1 = IMNMX chain, 2 = fused add-max
+ * (VIADDMNMX), 3 = IMAD chain, 4 = mixed IADD3+IMAD (both pipes), 5 = the per-FMA op mix of the
+ * counting GEMM (energy pass + count pass, u64 counts), 6 = same with 32-bit-operand counts.
+ * Runs `iters` unrolled rounds on every SM; returns elapsed milliseconds (CUDA events) and the
+ * number of lane-operations (which <= 4) or tropical FMAs (which >= 5) executed. */
+int bbtn_int32_microbench(int32_t which, int32_t iters, double *milliseconds, double *operations,
+                          void *cuda_stream);
+
+void bbtn_destroy(bbtn_handle *h);                    /* NULL is a no-op */
+const char *bbtn_last_error(const bbtn_handle *h);    /* valid until the next call on h / this thread */
+const char *bbtn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BBTN_H_ */

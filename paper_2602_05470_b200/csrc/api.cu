@@ -1,0 +1,309 @@
+// api.cu -- the C ABI of include/bbtn.h: handle, plan cache, device arena, launch sequencing.
+// Host logic only; every arithmetic step of the path runs in the kernels (kernels.h).
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+#include <map>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "handle.h"
+
+using namespace bbtn;
+
+namespace bbtn {
+thread_local std::string g_err;
+int fail(bbtn_handle *h, int code, const std::string &msg) {
+  if (h) h->err = msg;
+  g_err = msg;
+  return code;
+}
+bool have_device() {
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return false; }
+  return true;
+}
+}  // namespace bbtn
+
+namespace {
+
+int get_plan(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, bool enforce, DevPlan **out) {
+  if (n_fixed < 0 || (n_fixed > 0 && !fixed)) return fail(h, BBTN_EINVAL, "bad fixed set");
+  std::vector<int32_t> key(fixed, fixed + n_fixed);
+  auto it = h->plans.find(key);
+  if (it == h->plans.end()) {
+    auto dp = std::make_unique<DevPlan>();
+    std::string err;
+    int rc = make_plan(h->P, key, h->force_mode, false, dp->plan, err);
+    if (rc) return fail(h, rc, err);
+    it = h->plans.emplace(key, std::move(dp)).first;
+  }
+  DevPlan *dp = it->second.get();
+  if (enforce && dp->plan.rho > 0)
+    return fail(h, BBTN_ESHAPE, "an intermediate of rank " + std::to_string(dp->plan.max_rank) +
+                                    " exceeds max_elements_per_leaf (Eq. 4 rho = " + std::to_string(dp->plan.rho) + ")");
+  *out = dp;
+  return BBTN_OK;
+}
+
+int upload_tables(bbtn_handle *h, DevPlan *dp) {
+  if (dp->tables_ready) return BBTN_OK;
+  const Plan &pl = dp->plan;
+  std::vector<int32_t> lv, li;
+  for (size_t t = 0; t < pl.inputs.size(); t++) {
+    if (pl.inputs[t].rank == 0) continue;
+    (pl.inputs[t].variant ? lv : li).push_back((int32_t)t);
+  }
+  dp->n_var = (int)lv.size(); dp->n_inv = (int)li.size(); dp->n_scalar = (int)pl.scalar_inputs.size();
+  CUDA_TRY(h, dp->inputs.ensure(pl.inputs.size() * sizeof(InputRec)));
+  CUDA_TRY(h, cudaMemcpy(dp->inputs.p, pl.inputs.data(), pl.inputs.size() * sizeof(InputRec), cudaMemcpyHostToDevice));
+  CUDA_TRY(h, dp->list_var.ensure(lv.size() * 4));
+  CUDA_TRY(h, dp->list_inv.ensure(li.size() * 4));
+  CUDA_TRY(h, dp->list_scalar.ensure(pl.scalar_inputs.size() * 4));
+  if (!lv.empty()) CUDA_TRY(h, cudaMemcpy(dp->list_var.p, lv.data(), lv.size() * 4, cudaMemcpyHostToDevice));
+  if (!li.empty()) CUDA_TRY(h, cudaMemcpy(dp->list_inv.p, li.data(), li.size() * 4, cudaMemcpyHostToDevice));
+  if (!pl.scalar_inputs.empty())
+    CUDA_TRY(h, cudaMemcpy(dp->list_scalar.p, pl.scalar_inputs.data(), pl.scalar_inputs.size() * 4, cudaMemcpyHostToDevice));
+  CUDA_TRY(h, dp->inv_e.ensure((size_t)pl.arena_invariant_elems * 4));
+  CUDA_TRY(h, dp->inv_c.ensure((size_t)pl.arena_invariant_elems * 8));
+  dp->tables_ready = true;
+  return BBTN_OK;
+}
+
+int ensure_batch(bbtn_handle *h, DevPlan *dp, int64_t B, bool host_io) {
+  const Plan &pl = dp->plan;
+  if (B > dp->B_cap) {
+    size_t need = (size_t)pl.arena_variant_elems * (size_t)B;
+    size_t free_b = 0, total_b = 0;
+    CUDA_TRY(h, cudaMemGetInfo(&free_b, &total_b));
+    if (need * 12 > free_b + dp->var_e.bytes + dp->var_c.bytes)
+      return fail(h, BBTN_ENOMEM, "batch needs " + std::to_string(need * 12) + " bytes of device memory");
+    CUDA_TRY(h, dp->var_e.ensure(need * 4));
+    CUDA_TRY(h, dp->var_c.ensure(need * 8));
+    CUDA_TRY(h, dp->off_e.ensure((size_t)B * 4));
+    CUDA_TRY(h, dp->off_c.ensure((size_t)B * 8));
+    dp->B_cap = B;
+  }
+  if (host_io) {
+    CUDA_TRY(h, dp->assign.ensure((size_t)B * std::max<size_t>(pl.fixed.size(), 1)));
+    CUDA_TRY(h, dp->energy.ensure((size_t)B * 4));
+    CUDA_TRY(h, dp->count.ensure((size_t)B * 8));
+    CUDA_TRY(h, dp->count_mod.ensure((size_t)B * 8));
+  }
+  return BBTN_OK;
+}
+
+// enqueue the whole contraction for one count ring
+void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d_assign, int32_t *d_energy,
+                  uint64_t *d_count, uint32_t *d_count_mod, int ring, cudaStream_t st) {
+  const Plan &pl = dp->plan;
+  int32_t *ve = (int32_t *)dp->var_e.p, *ie = (int32_t *)dp->inv_e.p;
+  char *vc = (char *)dp->var_c.p, *ic = (char *)dp->inv_c.p;
+  const size_t csz = ring == 0 ? 8 : 4;
+  launch_construct(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_var.p, dp->n_var,
+                   (const int32_t *)dp->list_inv.p, dp->n_inv, (const int32_t *)dp->list_scalar.p, dp->n_scalar,
+                   d_assign, (int)pl.fixed.size(), B, ve, vc, ie, ic, (int32_t *)dp->off_e.p, dp->off_c.p, ring, st);
+  auto pe = [&](int v, int64_t off) { return v ? ve + off * B : ie + off; };
+  auto pc = [&](int v, int64_t off) { return (void *)(v ? vc + (size_t)off * B * csz : ic + (size_t)off * csz); };
+  for (const Step &s : pl.steps) {
+    const int64_t nb = s.variant ? B : 1;
+    switch (s.kind) {
+      case STEP_ABSORB:
+        launch_absorb(s, nb, pe(s.vA, s.offA), pc(s.vA, s.offA), pe(s.vB, s.offB), pc(s.vB, s.offB),
+                      pe(s.vC, s.offC), pc(s.vC, s.offC), ring, st);
+        break;
+      case STEP_REDUCE:
+        launch_reduce(s, nb, pe(s.vA, s.offA), pc(s.vA, s.offA), pe(s.vB, s.offB), pc(s.vB, s.offB),
+                      pe(s.vC, s.offC), pc(s.vC, s.offC), ring, st);
+        break;
+      case STEP_PERMUTE:
+        launch_permute(s.rO, s.perm, nb, pe(s.vA, s.offA), pc(s.vA, s.offA), pe(s.vC, s.offC), pc(s.vC, s.offC), ring, st);
+        break;
+      case STEP_GEMM:
+        launch_gemm_tiled(nb, (int64_t)1 << s.lg, 1 << s.lm, 1 << s.ln, 1 << s.lk, 1,
+                          pe(s.vA, s.offA), pc(s.vA, s.offA), pe(s.vB, s.offB), pc(s.vB, s.offB),
+                          pe(s.vC, s.offC), pc(s.vC, s.offC),
+                          s.vA ? ((int64_t)1 << s.rA) : 0, s.vB ? ((int64_t)1 << s.rB) : 0, (int64_t)1 << s.rO,
+                          ring, 64, st);
+        break;
+    }
+  }
+  const bool has_root = pl.result_offset >= 0;
+  launch_finalize(h->P.kind, B, has_root ? pe(pl.result_variant, pl.result_offset) : nullptr,
+                  has_root ? pc(pl.result_variant, pl.result_offset) : nullptr, pl.result_variant ? 1 : 0,
+                  (const int32_t *)dp->off_e.p, dp->off_c.p, d_energy, d_count, d_count_mod, ring, st);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *bbtn_version(void) { return "bbtn-b200 0.1 (sm_100a)"; }
+
+const char *bbtn_last_error(const bbtn_handle *h) { return h ? h->err.c_str() : bbtn::g_err.c_str(); }
+
+int bbtn_build(const bbtn_problem_desc *d, bbtn_handle **out) {
+  if (!d || !out) return fail(nullptr, BBTN_EINVAL, "null argument");
+  *out = nullptr;
+  if (d->kind != BBTN_ISING && d->kind != BBTN_MIS) return fail(nullptr, BBTN_EINVAL, "unknown kind");
+  if (d->n_vertices < 0 || d->n_edges < 0 || (d->n_edges > 0 && (!d->edge_u || !d->edge_v)))
+    return fail(nullptr, BBTN_EINVAL, "bad graph");
+  auto h = std::make_unique<bbtn_handle>();
+  Problem &P = h->P;
+  P.kind = d->kind; P.n = d->n_vertices; P.m = d->n_edges; P.flags = d->flags;
+  P.eu.assign(d->edge_u, d->edge_u + P.m); P.ev.assign(d->edge_v, d->edge_v + P.m);
+  std::vector<std::pair<int, int>> seen;
+  int64_t range = 0;
+  for (int e = 0; e < P.m; e++) {
+    int u = P.eu[e], v = P.ev[e];
+    if (u < 0 || v < 0 || u >= P.n || v >= P.n || u == v) return fail(nullptr, BBTN_EINVAL, "edge " + std::to_string(e) + " is malformed");
+    seen.push_back({std::min(u, v), std::max(u, v)});
+  }
+  std::sort(seen.begin(), seen.end());
+  for (size_t i = 1; i < seen.size(); i++) if (seen[i] == seen[i - 1]) return fail(nullptr, BBTN_EINVAL, "duplicate edge");
+  P.ew.resize(P.m); P.vw.resize(P.n);
+  for (int e = 0; e < P.m; e++) { P.ew[e] = (P.kind == BBTN_ISING && d->edge_w) ? d->edge_w[e] : 1; if (P.kind == BBTN_ISING) range += std::abs((int64_t)P.ew[e]); }
+  for (int i = 0; i < P.n; i++) {
+    P.vw[i] = d->vertex_w ? d->vertex_w[i] : (P.kind == BBTN_ISING ? 0 : 1);
+    range += std::abs((int64_t)P.vw[i]);
+  }
+  if (range > BBTN_ENERGY_LIMIT) return fail(nullptr, BBTN_ERANGE, "sum of |couplings| + |weights| exceeds 2^28");
+  if (d->tree_l || d->n_steps > 0) {
+    if (!d->tree_l || !d->tree_r || d->n_steps != P.n + P.m - 1)
+      return fail(nullptr, BBTN_EINVAL, "tree must have n_edges + n_vertices - 1 steps");
+    P.tree_l.assign(d->tree_l, d->tree_l + d->n_steps); P.tree_r.assign(d->tree_r, d->tree_r + d->n_steps);
+  }
+  P.max_elements = d->max_elements_per_leaf > 0 ? d->max_elements_per_leaf : ((int64_t)1 << 28);
+  h->force_mode = (d->flags & BBTN_FORCE_STREAMING) ? 1 : ((d->flags & BBTN_FORCE_TILED) ? 2 : 0);
+  // validate the tree once on the unsliced network
+  if (!P.tree_l.empty()) {
+    Plan tmp; std::string err;
+    int rc = make_plan(P, {}, h->force_mode, false, tmp, err);
+    if (rc) return fail(nullptr, rc, err);
+  }
+  *out = h.release();
+  return BBTN_OK;
+}
+
+void bbtn_destroy(bbtn_handle *h) { delete h; }
+
+int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, int64_t B, bbtn_plan_info *info) {
+  if (!h || !info || B < 1) return fail(h, BBTN_EINVAL, "null argument");
+  DevPlan *dp = nullptr;
+  int rc = get_plan(h, fixed, n_fixed, false, &dp);
+  if (rc) return rc;
+  const Plan &pl = dp->plan;
+  std::memset(info, 0, sizeof(*info));
+  info->n_nodes = pl.n_nodes; info->n_variant_nodes = pl.n_variant_nodes; info->max_rank = pl.max_rank;
+  for (const Step &s : pl.steps) {
+    if (s.kind == STEP_GEMM) info->n_gemm_tiled++;
+    else if (s.kind == STEP_ABSORB) info->n_absorb++;
+    else if (s.kind == STEP_PERMUTE) info->n_permute++;
+    else info->n_trace++;
+  }
+  info->rho = pl.rho;
+  info->fma_variant = pl.fma_variant; info->fma_invariant = pl.fma_invariant;
+  info->bytes_per_call = pl.bytes_variant * (double)B + pl.bytes_invariant;
+  info->workspace_bytes = (pl.arena_variant_elems * B + pl.arena_invariant_elems) * 12;
+  return BBTN_OK;
+}
+
+int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, const uint8_t *assign, int64_t B,
+                        int32_t *energy, uint64_t *count, uint32_t *count_mod, void *stream) {
+  if (!h) return fail(nullptr, BBTN_EINVAL, "null handle");
+  if (B < 1 || !energy || !count || (n_fixed > 0 && !assign)) return fail(h, BBTN_EINVAL, "bad batch arguments");
+  const bool crt = (h->P.flags & BBTN_COUNT_CRT) != 0;
+  if (count_mod && !crt) return fail(h, BBTN_EINVAL, "count_mod needs a handle built with BBTN_COUNT_CRT");
+  if (!have_device()) return fail(h, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  DevPlan *dp = nullptr;
+  int rc = get_plan(h, fixed, n_fixed, true, &dp);
+  if (rc) return rc;
+  if ((rc = upload_tables(h, dp))) return rc;
+  const bool dev_io = (h->P.flags & BBTN_IO_DEVICE) != 0;
+  if ((rc = ensure_batch(h, dp, B, !dev_io))) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint8_t *d_assign = assign; int32_t *d_energy = energy; uint64_t *d_count = count; uint32_t *d_mod = count_mod;
+  if (!dev_io) {
+    d_assign = (const uint8_t *)dp->assign.p; d_energy = (int32_t *)dp->energy.p; d_count = (uint64_t *)dp->count.p;
+    d_mod = count_mod ? (uint32_t *)dp->count_mod.p : nullptr;
+    if (n_fixed > 0) CUDA_TRY(h, cudaMemcpyAsync(dp->assign.p, assign, (size_t)B * n_fixed, cudaMemcpyHostToDevice, st));
+  }
+  const int n_rings = (crt && d_mod) ? 3 : 1;
+  const bool use_graph = !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
+  if (!use_graph) {
+    for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring, st);
+  } else {
+    const void *io[4] = {d_assign, d_energy, d_count, d_mod};
+    const bool stale = dp->graph_B != B || (int)dp->graphs.size() != n_rings || std::memcmp(io, dp->graph_io, sizeof(io)) != 0;
+    if (stale) {
+      for (auto g : dp->graphs) if (g) cudaGraphExecDestroy(g);
+      dp->graphs.clear();
+      cudaStream_t cs;
+      CUDA_TRY(h, cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+      for (int ring = 0; ring < n_rings; ring++) {
+        cudaGraph_t g = nullptr; cudaGraphExec_t ge = nullptr;
+        CUDA_TRY(h, cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+        enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring, cs);
+        CUDA_TRY(h, cudaStreamEndCapture(cs, &g));
+        CUDA_TRY(h, cudaGraphInstantiate(&ge, g, 0));
+        cudaGraphDestroy(g);
+        dp->graphs.push_back(ge);
+      }
+      cudaStreamDestroy(cs);
+      dp->graph_B = B; std::memcpy(dp->graph_io, io, sizeof(io));
+    }
+    for (auto ge : dp->graphs) CUDA_TRY(h, cudaGraphLaunch(ge, st));
+  }
+  CUDA_TRY(h, cudaGetLastError());
+  if (!dev_io) {
+    // stage into temporaries so that outputs stay untouched on error
+    std::vector<int32_t> te((size_t)B); std::vector<uint64_t> tc((size_t)B); std::vector<uint32_t> tm(count_mod ? (size_t)B * 2 : 0);
+    CUDA_TRY(h, cudaMemcpyAsync(te.data(), d_energy, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(h, cudaMemcpyAsync(tc.data(), d_count, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    if (count_mod) CUDA_TRY(h, cudaMemcpyAsync(tm.data(), d_mod, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    std::memcpy(energy, te.data(), (size_t)B * 4); std::memcpy(count, tc.data(), (size_t)B * 8);
+    if (count_mod) std::memcpy(count_mod, tm.data(), (size_t)B * 8);
+  }
+  return BBTN_OK;
+}
+
+int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac,
+                               const int32_t *Be, const uint64_t *Bc, int32_t *Ce, uint64_t *Cc,
+                               int64_t strideA, int64_t strideB, int64_t strideC, int32_t count_bits, void *stream) {
+  if (batch < 1 || M < 1 || N < 1 || K < 1 || !Ae || !Ac || !Be || !Bc || !Ce || !Cc || strideA < 0 || strideB < 0 || strideC < 0)
+    return fail(nullptr, BBTN_EINVAL, "bad GEMM arguments");
+  if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
+  if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  launch_gemm_tiled(batch, 1, M, N, K, 0, Ae, Ac, Be, Bc, Ce, Cc, strideA, strideB, strideC, RING_U64, count_bits,
+                    (cudaStream_t)stream);
+  CUDA_TRY(nullptr, cudaGetLastError());
+  return BBTN_OK;
+}
+
+int bbtn_permute_batched(int32_t rank, const int32_t *perm, int64_t batch, const int32_t *src_e, const uint64_t *src_c,
+                         int32_t *dst_e, uint64_t *dst_c, void *stream) {
+  if (rank < 0 || rank > 30 || batch < 1 || (rank > 0 && !perm) || !src_e || !src_c || !dst_e || !dst_c)
+    return fail(nullptr, BBTN_EINVAL, "bad permute arguments");
+  uint32_t seen = 0;
+  for (int j = 0; j < rank; j++) {
+    if (perm[j] < 0 || perm[j] >= rank || (seen >> perm[j]) & 1u) return fail(nullptr, BBTN_EINVAL, "perm is not a permutation");
+    seen |= 1u << perm[j];
+  }
+  if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  launch_permute(rank, perm, batch, src_e, src_c, dst_e, dst_c, RING_U64, (cudaStream_t)stream);
+  CUDA_TRY(nullptr, cudaGetLastError());
+  return BBTN_OK;
+}
+
+int bbtn_int32_microbench(int32_t which, int32_t iters, double *ms, double *ops, void *stream) {
+  if (which < 0 || which > 6 || iters < 1 || !ms || !ops) return fail(nullptr, BBTN_EINVAL, "bad microbench arguments");
+  if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device");
+  int rc = run_microbench(which, iters, ms, ops, (cudaStream_t)stream);
+  if (rc) return fail(nullptr, BBTN_ECUDA, "microbenchmark failed");
+  return BBTN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,109 @@
+// gemm.cu -- K3: register- and shared-memory-tiled batched counting-tropical GEMM (sm_100a).
+//
+//   C[b,g,m,n] = (+)_k A[b,g,m,k] (.) B[b,g,k,n]        (PAPER.md:51 Eq. 2 evaluated pairwise, :57)
+//   (ea,ca) (.) (eb,cb) = (ea+eb, ca*cb);  (+) keeps the max energy, adds counts on ties.
+//
+// Tensor cores cannot evaluate max-plus, so this runs on the integer CUDA cores (north_star).
+// v1: single pass, 64x64 CTA tile, BK = 16, 256 threads, 4x4 outputs per thread.
+#include "kernels.h"
+#include "ring.cuh"
+
+namespace bbtn {
+namespace {
+
+constexpr int BM = 64, BN = 64, BK = 16, TM = 4, TN = 4, NT = 256;
+
+template <class R, bool A_KMAJOR>
+__global__ void __launch_bounds__(NT) gemm_tiled_kernel(int64_t G, int M, int N, int K,
+                                                        const int32_t *__restrict__ Ae, const typename R::T *__restrict__ Ac,
+                                                        const int32_t *__restrict__ Be, const typename R::T *__restrict__ Bc,
+                                                        int32_t *__restrict__ Ce, typename R::T *__restrict__ Cc,
+                                                        int64_t sA, int64_t sB, int64_t sC) {
+  using CT = typename R::T;
+  __shared__ int32_t As_e[BK][BM + 4];
+  __shared__ CT As_c[BK][BM + 2];
+  __shared__ int32_t Bs_e[BK][BN + 4];
+  __shared__ CT Bs_c[BK][BN + 2];
+
+  const int tiles_n = (N + BN - 1) / BN, tiles_m = (M + BM - 1) / BM;
+  const int64_t bg = blockIdx.x / (tiles_n * tiles_m);
+  const int tile = (int)(blockIdx.x - bg * (tiles_n * tiles_m));
+  const int64_t b = bg / G, g = bg - b * G;
+  const int m0 = (tile / tiles_n) * BM, n0 = (tile % tiles_n) * BN;
+  const int32_t *ae = Ae + b * sA + g * (int64_t)M * K; const CT *ac = Ac + b * sA + g * (int64_t)M * K;
+  const int32_t *be = Be + b * sB + g * (int64_t)K * N; const CT *bc = Bc + b * sB + g * (int64_t)K * N;
+  int32_t *ce = Ce + b * sC + g * (int64_t)M * N; CT *cc = Cc + b * sC + g * (int64_t)M * N;
+
+  const int tx = threadIdx.x % (BN / TN), ty = threadIdx.x / (BN / TN);   // 16 x 16 threads
+  int32_t acc_e[TM][TN]; CT acc_c[TM][TN];
+#pragma unroll
+  for (int i = 0; i < TM; i++)
+#pragma unroll
+    for (int j = 0; j < TN; j++) { acc_e[i][j] = NEG_INF; acc_c[i][j] = 0; }
+
+  for (int k0 = 0; k0 < K; k0 += BK) {
+    // stage A tile as [k][m] and B tile as [k][n]; out-of-range entries are the zero element
+    for (int i = threadIdx.x; i < BM * BK; i += NT) {
+      int kk, mm;
+      if (A_KMAJOR) { kk = i / BM; mm = i % BM; } else { mm = i / BK; kk = i % BK; }
+      const int gm = m0 + mm, gk = k0 + kk;
+      int32_t e = NEG_INF; CT c = 0;
+      if (gm < M && gk < K) {
+        const int64_t idx = A_KMAJOR ? (int64_t)gk * M + gm : (int64_t)gm * K + gk;
+        e = ae[idx]; c = ac[idx];
+      }
+      As_e[kk][mm] = e; As_c[kk][mm] = c;
+    }
+    for (int i = threadIdx.x; i < BN * BK; i += NT) {
+      const int kk = i / BN, nn = i % BN;
+      const int gn = n0 + nn, gk = k0 + kk;
+      int32_t e = NEG_INF; CT c = 0;
+      if (gn < N && gk < K) { e = be[(int64_t)gk * N + gn]; c = bc[(int64_t)gk * N + gn]; }
+      Bs_e[kk][nn] = e; Bs_c[kk][nn] = c;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < BK; kk++) {
+      int32_t a_e[TM], b_e[TN]; CT a_c[TM], b_c[TN];
+#pragma unroll
+      for (int i = 0; i < TM; i++) { a_e[i] = As_e[kk][ty * TM + i]; a_c[i] = As_c[kk][ty * TM + i]; }
+#pragma unroll
+      for (int j = 0; j < TN; j++) { b_e[j] = Bs_e[kk][tx * TN + j]; b_c[j] = Bs_c[kk][tx * TN + j]; }
+#pragma unroll
+      for (int i = 0; i < TM; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) oplus<R>(acc_e[i][j], acc_c[i][j], a_e[i] + b_e[j], R::mul(a_c[i], b_c[j]));
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < TM; i++)
+#pragma unroll
+    for (int j = 0; j < TN; j++) {
+      const int gm = m0 + ty * TM + i, gn = n0 + tx * TN + j;
+      if (gm < M && gn < N) {
+        int32_t e = acc_e[i][j]; CT c = acc_c[i][j];
+        canonicalise<R>(e, c);
+        ce[(int64_t)gm * N + gn] = e; cc[(int64_t)gm * N + gn] = c;
+      }
+    }
+}
+
+}  // namespace
+
+void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
+                       const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc, int32_t *Ce, void *Cc,
+                       int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, cudaStream_t st) {
+  (void)count_bits;
+  const int64_t n_cta = (int64_t)((N + BN - 1) / BN) * ((M + BM - 1) / BM) * batch * G;
+  dim3 grid((unsigned)n_cta);
+  BBTN_RING_DISPATCH(ring, {
+    using CT = typename R::T;
+    if (a_kmajor)
+      gemm_tiled_kernel<R, true><<<grid, NT, 0, st>>>(G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
+    else
+      gemm_tiled_kernel<R, false><<<grid, NT, 0, st>>>(G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
+  });
+}
+
+}  // namespace bbtn

@@ -1,0 +1,75 @@
+// handle.h -- private definition of bbtn_handle and shared host helpers (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <map>
+#include <memory>
+#include <string>
+#include <vector>
+
+#include "../../include/bbtn.h"
+#include "kernels.h"
+#include "plan.h"
+
+namespace bbtn {
+
+struct DevBuf {
+  void *p = nullptr; size_t bytes = 0;
+  DevBuf() = default;
+  DevBuf(const DevBuf &) = delete;
+  DevBuf &operator=(const DevBuf &) = delete;
+  ~DevBuf() { if (p) cudaFree(p); }
+  cudaError_t ensure(size_t n) {
+    if (n <= bytes && p) return cudaSuccess;
+    if (p) { cudaFree(p); p = nullptr; bytes = 0; }
+    cudaError_t e = cudaMalloc(&p, n ? n : 1);
+    if (e == cudaSuccess) bytes = n;
+    return e;
+  }
+  template <class T> cudaError_t upload(const std::vector<T> &v) {
+    cudaError_t e = ensure(v.size() * sizeof(T));
+    if (e != cudaSuccess || v.empty()) return e;
+    return cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+  }
+};
+
+struct DevPlan {
+  Plan plan;
+  DevBuf inputs, list_var, list_inv, list_scalar;
+  int n_var = 0, n_inv = 0, n_scalar = 0;
+  DevBuf var_e, var_c, inv_e, inv_c, off_e, off_c;
+  DevBuf assign, energy, count, count_mod;      // staging for host-pointer calls
+  bool tables_ready = false;
+  int64_t B_cap = 0;
+  std::vector<cudaGraphExec_t> graphs;          // per ring, for graph_B
+  int64_t graph_B = -1;
+  const void *graph_io[4] = {nullptr, nullptr, nullptr, nullptr};
+  ~DevPlan() { for (auto g : graphs) if (g) cudaGraphExecDestroy(g); }
+};
+
+struct BoundPlan {
+  DevBuf tab[20];
+  BoundTables t;
+  DevBuf scratch, assign, bound;
+};
+
+int fail(bbtn_handle *h, int code, const std::string &msg);
+bool have_device();
+
+}  // namespace bbtn
+
+struct bbtn_handle {
+  bbtn::Problem P;
+  std::string err;
+  int force_mode = 0;
+  std::map<std::vector<int32_t>, std::unique_ptr<bbtn::DevPlan>> plans;
+  std::map<std::vector<int32_t>, std::unique_ptr<bbtn::BoundPlan>> bounds;
+};
+
+#define CUDA_TRY(h, expr)                                                                       \
+  do {                                                                                          \
+    cudaError_t _e = (expr);                                                                    \
+    if (_e != cudaSuccess)                                                                      \
+      return ::bbtn::fail(h, _e == cudaErrorMemoryAllocation ? BBTN_ENOMEM : BBTN_ECUDA,        \
+                          std::string(#expr) + ": " + cudaGetErrorString(_e));                  \
+  } while (0)

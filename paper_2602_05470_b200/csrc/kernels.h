@@ -1,0 +1,70 @@
+// kernels.h -- launchers of the sm_100a kernels (K1..K5).  All pointers are DEVICE pointers.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "plan.h"
+
+namespace bbtn {
+
+enum RingId : int { RING_U64 = 0, RING_P1 = 1, RING_P2 = 2 };   // counts mod 2^64 / mod 2^31-1 / mod 2^31-19
+
+constexpr int32_t kNegInf = -(1 << 30);
+constexpr int32_t kZeroThreshold = -(1 << 29);   // e < threshold  <=>  zero element (reading A8)
+
+// K1: build the sliced input tensors of every leaf and the per-leaf scalar offset.
+//   d_inputs: InputRec table; d_list: ids to build (rank > 0); variant inputs are written for
+//   b = 0..B-1 at arena offset off*B + b*2^rank, invariant ones once.
+void launch_construct(int kind, const InputRec *d_inputs, const int32_t *d_list_var, int n_var,
+                      const int32_t *d_list_inv, int n_inv, const int32_t *d_list_scalar, int n_scalar,
+                      const uint8_t *d_assign, int n_fixed, int64_t B,
+                      int32_t *var_e, void *var_c, int32_t *inv_e, void *inv_c,
+                      int32_t *off_e, void *off_c, int ring, cudaStream_t st);
+
+// K2: dst[b][pi(i)] = src[b][i], bit j of pi(i) = bit perm[j] of i.
+void launch_permute(int rank, const int32_t *perm, int64_t batch, const int32_t *src_e, const void *src_c,
+                    int32_t *dst_e, void *dst_c, int ring, cudaStream_t st);
+
+// K3 (streaming form, permutation fused into the operand addressing) and its long-reduction form.
+void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
+                   int32_t *Ce, void *Cc, int ring, cudaStream_t st);
+void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
+                   int32_t *Ce, void *Cc, int ring, cudaStream_t st);
+
+// K3 (register/shared-memory tiled form).  C[b,g,m,n] = (+)_k A (.) B.
+//   a_kmajor = 1: A is [g][k][m] (m fastest, the engine's canonical order); 0: A is row-major [m][k].
+//   B is [g][k][n], C is [g][m][n].  Batch strides in elements (0 = shared).  count_bits <= 32 selects the
+//   32-bit-operand multiply path (RING_U64 only).
+void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
+                       const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc, int32_t *Ce, void *Cc,
+                       int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, cudaStream_t st);
+
+// K4: (E[b], c[b]) = offset[b] (.) root[b]; canonicalise; convert to reported units.
+//   root_e == nullptr: the network is all scalars.  root_stride 0: root is leaf-invariant.
+void launch_finalize(int kind, int64_t B, const int32_t *root_e, const void *root_c, int64_t root_stride,
+                     const int32_t *off_e, const void *off_c, int32_t *energy, uint64_t *count,
+                     uint32_t *count_mod, int ring, cudaStream_t st);
+
+// K5: warp-level region bounds (reading A15).
+struct BoundTables {                 // device CSR tables built once per (regions, F)
+  int kind, n_regions, n_fixed;
+  const int32_t *reg_off;            // [n_regions+1] free vertices of each region
+  const int32_t *reg_vw;             // vertex weight of each free region vertex
+  const int32_t *reg_fix_off;        // [n_regions+1] per-region unary terms from fixed neighbours
+  const int32_t *reg_fix_bit, *reg_fix_col, *reg_fix_w;   // local bit, assign column, coupling
+  const int32_t *reg_pair_off;       // [n_regions+1] bonds inside the region
+  const int32_t *reg_pair_a, *reg_pair_b, *reg_pair_w;    // local bits, coupling
+  // terms outside every region
+  int n_ff; const int32_t *ff_cu, *ff_cv, *ff_w;          // fixed-fixed bonds: assign columns, coupling
+  int n_fv; const int32_t *fv_c, *fv_w;                   // fixed vertices: column, weight
+  int n_uf; const int32_t *uf_c, *uf_w;                   // uncovered bonds with one fixed endpoint: column, coupling
+  int n_uv; const int32_t *uv_off, *uv_cols, *uv_w;       // MIS: uncovered free vertices: CSR of fixed-neighbour columns, weight
+  int32_t const_term;                                     // assignment-independent part
+};
+void launch_region_bound(const BoundTables &t, const uint8_t *d_assign, int64_t B, int32_t *region_scratch,
+                         int32_t *bound, cudaStream_t st);
+
+// register-only integer microbenchmarks (include/bbtn.h: bbtn_int32_microbench)
+int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t st);
+
+}  // namespace bbtn

@@ -1,0 +1,121 @@
+// microbench.cu -- register-only integer-pipe microbenchmarks: the measured CUDA-core int32 roof
+// that K3 is reported against (include/bbtn.h: bbtn_int32_microbench).
+// Many resident warps, 8 independent dependency chains per thread, unrolled, no memory traffic,
+// result consumed.  Chains are cross-coupled (Fibonacci-like) so nothing folds to a closed form.
+#include "kernels.h"
+#include "ring.cuh"
+
+namespace bbtn {
+namespace {
+
+constexpr int CH = 8;          // independent chains per thread
+constexpr int UNROLL = 16;     // rounds per loop iteration
+
+template <int WHICH>
+__global__ void __launch_bounds__(256) pipe_kernel(int iters, int32_t seed, int32_t *sink) {
+  int32_t r[CH];
+#pragma unroll
+  for (int i = 0; i < CH; i++) r[i] = seed * (i + 1) + threadIdx.x;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int u = 0; u < UNROLL; u++) {
+#pragma unroll
+      for (int i = 0; i < CH; i++) {
+        const int32_t x = r[(i + 1) % CH], y = r[(i + 3) % CH];
+        if (WHICH == 0) asm volatile("add.s32 %0, %0, %1;\n\tadd.s32 %0, %0, %2;" : "+r"(r[i]) : "r"(x), "r"(y));   // -> IADD3
+        else if (WHICH == 1) { if (u & 1) asm volatile("max.s32 %0, %0, %1;" : "+r"(r[i]) : "r"(x)); else asm volatile("min.s32 %0, %0, %1;" : "+r"(r[i]) : "r"(y)); }
+        else if (WHICH == 2) r[i] = __viaddmax_s32(r[i], x, y);                                                      // max(r+x, y)
+        else if (WHICH == 3) asm volatile("mad.lo.s32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(x), "r"(y));              // IMAD
+        else if (WHICH == 4) {
+          if (i & 1) asm volatile("mad.lo.s32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(x), "r"(y));
+          else asm volatile("add.s32 %0, %0, %1;\n\tadd.s32 %0, %0, %2;" : "+r"(r[i]) : "r"(x), "r"(y));
+        }
+      }
+    }
+  }
+  int32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < CH; i++) s ^= r[i];
+  if (s == 0x7fffffff) sink[0] = s;       // consume
+}
+
+// per-FMA op mix of the counting GEMM on registers only: an 8x8 register tile, energy pass
+// (fused add-max) then count pass (tie test + predicated 64-bit multiply-add).
+template <bool WIDE>
+__global__ void __launch_bounds__(256) opmix_kernel(int iters, int32_t seed, uint64_t *sink) {
+  int32_t ae[8], be[8], acc_e[8][8];
+  uint64_t ac[8], bc[8], acc_c[8][8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) {
+    ae[i] = (seed + i * 7 + threadIdx.x) & 63; be[i] = (seed * 3 + i * 5 + threadIdx.x) & 63;
+    ac[i] = (uint64_t)(seed + i) | (WIDE ? ((uint64_t)(seed + 2 * i) << 32) : 0);
+    bc[i] = (uint64_t)(seed + 3 * i + 1) | (WIDE ? ((uint64_t)(seed + 5 * i) << 32) : 0);
+#pragma unroll
+    for (int j = 0; j < 8; j++) { acc_e[i][j] = NEG_INF; acc_c[i][j] = 0; }
+  }
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+#pragma unroll
+      for (int j = 0; j < 8; j++) acc_e[i][j] = __viaddmax_s32(ae[i], be[j], acc_e[i][j]);
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+#pragma unroll
+      for (int j = 0; j < 8; j++) {
+        if (ae[i] + be[j] == acc_e[i][j]) {
+          if (WIDE) acc_c[i][j] += ac[i] * bc[j];
+          else acc_c[i][j] += (uint64_t)(uint32_t)ac[i] * (uint32_t)bc[j];
+        }
+      }
+#pragma unroll
+    for (int i = 0; i < 8; i++) { ae[i] = (ae[i] + it) & 63; be[i] = (be[i] ^ it) & 63; }
+  }
+  uint64_t s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; i++)
+#pragma unroll
+    for (int j = 0; j < 8; j++) s += acc_c[i][j] + (uint64_t)acc_e[i][j];
+  if (s == 0x123456789abcdefull) sink[0] = s;
+}
+
+}  // namespace
+
+int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t st) {
+  void *sink = nullptr;
+  if (cudaMalloc(&sink, 64) != cudaSuccess) return 3;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int grid = 148 * 8, block = 256;
+  auto launch = [&](int n) {
+    switch (which) {
+      case 0: pipe_kernel<0><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 1: pipe_kernel<1><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 2: pipe_kernel<2><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 3: pipe_kernel<3><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 4: pipe_kernel<4><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 5: opmix_kernel<true><<<grid, block, 0, st>>>(n, 12345, (uint64_t *)sink); break;
+      default: opmix_kernel<false><<<grid, block, 0, st>>>(n, 12345, (uint64_t *)sink); break;
+    }
+  };
+  launch(iters / 8 + 1);                       // warm-up
+  cudaEventRecord(e0, st);
+  launch(iters);
+  cudaEventRecord(e1, st);
+  cudaError_t err = cudaEventSynchronize(e1);
+  float t = 0;
+  cudaEventElapsedTime(&t, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(sink);
+  if (err != cudaSuccess || cudaGetLastError() != cudaSuccess) return 3;
+  *ms = t;
+  const double threads = (double)grid * block;
+  if (which <= 4) {
+    double per_round = CH;                     // one instruction per chain per round
+    *ops = threads * (double)iters * UNROLL * per_round;
+  } else {
+    *ops = threads * (double)iters * 64.0;     // tropical FMAs
+  }
+  return 0;
+}
+
+}  // namespace bbtn

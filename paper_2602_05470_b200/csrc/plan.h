@@ -1,0 +1,90 @@
+// plan.h -- host-side planner of the BBTN contraction engine (plain C++, no CUDA).
+//
+// For one fixed-set signature F (Eq. 3) the planner turns
+// (graph, SSA tree) into a list of device steps: which input tensors K1 builds,
+// how every pairwise contraction (Eq. 2 evaluated pairwise) maps
+// onto index classes  g = I_L n I_R n I_O,  K = (I_L n I_R) \ I_O,
+// M = I_L \ I_R,  N = I_R \ I_L,  which bit permutations K2 must apply, which
+// K3 variant runs, and where every tensor lives in the device arena.
+// All tensor dimensions are 2, so a rank-r tensor is 2^r elements and a layout
+// is the list of index labels per bit of the linear element index.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace bbtn {
+
+struct Problem {
+  int kind = 0;                       // 0 Ising, 1 MIS
+  int n = 0, m = 0;
+  std::vector<int32_t> eu, ev, ew, vw;  // ew/vw always materialised (defaults applied)
+  std::vector<int32_t> tree_l, tree_r;  // empty = derive per signature
+  int64_t max_elements = (int64_t)1 << 28;
+  uint32_t flags = 0;
+};
+
+// One input tensor as K1 must build it.
+struct InputRec {
+  int32_t type;        // 0 bond, 1 vertex
+  int32_t u, v;        // vertex ids (v = -1 for vertex tensors)
+  int32_t w;           // J_ij or h_i / w_i
+  int32_t fu, fv;      // column of u / v inside `assign`, or -1 when free
+  int32_t su, sv;      // 1 if the free index u / v occurs in no other tensor: summed inside K1 (reading A7)
+  int32_t bu, bv;      // bit position of u / v in the emitted tensor, -1 if absent
+  int32_t rank;        // rank of the emitted tensor (0 => folded into offset[b])
+  int32_t variant;     // depends on the assignment
+  int64_t offset;      // element offset in the arena (rank > 0)
+};
+
+enum StepKind : int32_t { STEP_ABSORB = 0, STEP_REDUCE = 1, STEP_PERMUTE = 2, STEP_GEMM = 3 };
+
+// A device launch.  Offsets are element offsets into the arena; batch strides are 0 for
+// leaf-invariant tensors (contracted once, broadcast to every leaf).
+struct Step {
+  int32_t kind = 0;
+  int32_t variant = 0;          // 1: runs for every leaf, 0: once
+  // ABSORB / REDUCE: out[o] = (+)_k A[fa(o) + ka(k)] (.) B[fb(o) + kb(k)]
+  int32_t rO = 0, nK = 0;
+  uint32_t addA[32] = {0}, addB[32] = {0};   // per output bit
+  uint32_t kA[32] = {0}, kB[32] = {0};       // per contracted bit
+  // tensor locations: element offset inside the variant arena (per-leaf units; the real
+  // offset is off * B, the tensor is [B][2^rank]) or inside the invariant arena.
+  int64_t offA = 0, offB = 0, offC = 0;
+  int32_t vA = 0, vB = 0, vC = 0;            // 1 = lives in the variant arena
+  int32_t rA = 0, rB = 0;                    // operand ranks (batch stride = vX ? 2^rX : 0)
+  // PERMUTE: dst[pi(i)] = src[i], bit j of pi(i) = bit perm[j] of i   (offA -> offC, rank rO)
+  int32_t perm[32] = {0};
+  // GEMM: A [g][k][m], B [g][k][n] -> C [g][m][n]   (log2 sizes)
+  int32_t lg = 0, lm = 0, ln = 0, lk = 0;
+  double fma = 0;               // tropical FMAs of this launch per batch entry
+  double bytes = 0;             // algorithmic bytes per batch entry (12 B per element moved)
+};
+
+struct Plan {
+  std::vector<int32_t> fixed;
+  std::vector<InputRec> inputs;          // all n_in inputs in ABI order
+  std::vector<int32_t> scalar_inputs;    // ids of inputs folded into offset[b]
+  std::vector<Step> steps;
+  int64_t result_offset = -1;            // rank-0 result tensor, -1 if the network is all scalars
+  int32_t result_variant = 0;
+  int64_t arena_variant_elems = 0;       // per-leaf elements (multiply by B)
+  int64_t arena_invariant_elems = 0;
+  int32_t max_rank = 0;
+  int64_t rho = 0;
+  double fma_variant = 0, fma_invariant = 0;
+  double bytes_variant = 0, bytes_invariant = 0;
+  int32_t n_nodes = 0, n_variant_nodes = 0;
+};
+
+// Returns 0 or a bbtn_status value; err receives the message.
+// force_mode: 0 = automatic, 1 = never use the tiled GEMM path, 2 = use it wherever |K| >= 1.
+// enforce_cap: fail with ESHAPE when a tensor exceeds P.max_elements (otherwise only rho records it).
+int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mode, bool enforce_cap,
+              Plan &out, std::string &err);
+
+// Elimination-order tree for the network with `fixed` sliced out (used when the caller gave no tree).
+void derive_tree(const Problem &P, const std::vector<int32_t> &fixed,
+                 std::vector<int32_t> &tl, std::vector<int32_t> &tr);
+
+}  // namespace bbtn

@@ -1,0 +1,132 @@
+"""CPU-side checks of the boundary: the C-ABI library builds/loads, exports every symbol that
+include/bbtn.h declares, validates its arguments, plans on the host, and refuses to compute
+without a device (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2602_05470_b200 import binding as bb
+from paper_2602_05470_b200 import build as bbuild
+from paper_2602_05470_b200 import instances as I
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    bbuild.build()
+    return bb.load()
+
+
+def _has_gpu():
+    try:
+        import torch
+        return torch.cuda.is_available()
+    except Exception:
+        return False
+
+
+def test_every_declared_symbol_is_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "bbtn.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(bbtn_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(bb.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.bbtn_version()
+
+
+def test_build_validates_arguments(lib):
+    inst = I.ising_lattice_2d(3, 3, 1)
+    bb.Handle(inst).close()
+    bad = I.ising_lattice_2d(3, 3, 1); bad.edge_v = bad.edge_v.copy(); bad.edge_v[0] = 99
+    with pytest.raises(bb.BbtnError) as e:
+        bb.Handle(bad)
+    assert e.value.status == bb.BBTN_EINVAL
+    dup = I.ising_lattice_2d(3, 3, 1); dup.edge_u = np.append(dup.edge_u, dup.edge_v[0]).astype(np.int32)
+    dup.edge_v = np.append(dup.edge_v, dup.edge_u[0]).astype(np.int32); dup.edge_w = np.append(dup.edge_w, 1).astype(np.int32)
+    with pytest.raises(bb.BbtnError) as e:
+        bb.Handle(dup)
+    assert e.value.status == bb.BBTN_EINVAL
+    big = I.ising_lattice_2d(3, 3, 1); big.edge_w = (big.edge_w.astype(np.int64) * (1 << 27)).astype(np.int32)
+    with pytest.raises(bb.BbtnError) as e:
+        bb.Handle(big)
+    assert e.value.status == bb.BBTN_ERANGE
+    with pytest.raises(bb.BbtnError) as e:      # wrong number of tree steps
+        bb.Handle(inst, tree=(np.zeros(3, np.int32), np.ones(3, np.int32)))
+    assert e.value.status == bb.BBTN_EINVAL
+    tl, tr = I.elimination_tree(inst.input_index_sets(), I.natural_order(9))
+    tl2 = tl.copy(); tl2[5] = tl2[4]              # reuses a consumed tensor
+    with pytest.raises(bb.BbtnError) as e:
+        bb.Handle(inst, tree=(tl2, tr))
+    assert e.value.status == bb.BBTN_EINVAL
+
+
+def test_planner_widths_and_counts_on_host(lib):
+    # row-major sweep of an LxL lattice has width L+1 (frontier L plus the new site's bond index)
+    for L in (4, 6, 8):
+        inst = I.ising_lattice_2d(L, L, 1)
+        tl, tr = I.elimination_tree(inst.input_index_sets(), I.natural_order(L * L))
+        h = bb.Handle(inst, tree=(tl, tr))
+        info = h.plan_query()
+        assert L <= info["max_rank"] <= L + 2
+        assert info["n_variant_nodes"] == 0 and info["fma_variant"] == 0
+        assert info["n_nodes"] == inst.n_edges + inst.n_vertices - 1
+        assert info["rho"] == 0
+        # fixing the middle column splits the lattice: width drops, nodes next to F become leaf-variant
+        fixed = np.array([r * L + L // 2 for r in range(L)], np.int32)
+        tl2, tr2 = I.elimination_tree(inst.input_index_sets(fixed), I.natural_order(L * L, exclude=fixed))
+        h2 = bb.Handle(inst, tree=(tl2, tr2))
+        info2 = h2.plan_query(fixed, B=16)
+        assert info2["max_rank"] <= info["max_rank"]
+        assert info2["n_variant_nodes"] > 0 and info2["fma_variant"] > 0
+        # library-derived tree (tree = NULL) must also plan
+        h3 = bb.Handle(inst)
+        assert h3.plan_query(fixed, B=4)["max_rank"] >= 1
+
+
+def test_rho_eq4_reported_when_cap_exceeded(lib):
+    inst = I.ising_lattice_2d(8, 8, 1)
+    tl, tr = I.elimination_tree(inst.input_index_sets(), I.natural_order(64))
+    h = bb.Handle(inst, tree=(tl, tr), max_elements_per_leaf=1 << 6)
+    info = h.plan_query()
+    assert info["max_rank"] > 6 and info["rho"] > 0        # Eq. 4: cumulative overflow over T_target
+
+
+def test_slit_order_gives_narrow_leaves(lib):
+    # config 3 recipe: f contiguous spins of the middle column + angular order -> width ~ max(L/2, L-f)+1
+    L = 24
+    inst = I.ising_lattice_2d(L, L, 1)
+    for f, wmax in ((8, 19), (10, 17), (12, 15)):
+        fixed = I.slit_fixed_set_2d(L, L, f)
+        order = I.slit_angular_order_2d(L, L, f)
+        assert len(order) == L * L - f
+        tl, tr = I.elimination_tree(inst.input_index_sets(fixed), order)
+        h = bb.Handle(inst, tree=(tl, tr), max_elements_per_leaf=1 << 26)
+        info = h.plan_query(fixed, B=1 << f)
+        assert info["max_rank"] <= wmax, (f, info)
+        assert info["rho"] == 0
+
+
+@pytest.mark.skipif(_has_gpu(), reason="checks the no-device behaviour")
+def test_no_cpu_fallback(lib):
+    inst = I.ising_lattice_2d(3, 3, 1)
+    h = bb.Handle(inst)
+    with pytest.raises(bb.BbtnError) as e:
+        h.contract_batch()
+    assert e.value.status == bb.BBTN_ECUDA
+    with pytest.raises(bb.BbtnError) as e:
+        h.region_bound([0], [])
+    assert e.value.status == bb.BBTN_ECUDA
+    with pytest.raises(bb.BbtnError) as e:
+        bb.int32_microbench(0, 10)
+    assert e.value.status == bb.BBTN_ECUDA
+
+
+def test_crt_combine_host():
+    for x in (0, 1, 2 ** 64 - 1, 2 ** 64 + 12345, 3 ** 70, 2 ** 125 + 7):
+        got = bb.crt_combine(x % 2 ** 64, x % bb.BBTN_P1, x % bb.BBTN_P2)
+        assert got == x

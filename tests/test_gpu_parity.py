@@ -1,0 +1,357 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Integer work: the bar is BIT-EXACT for energies and counts."""
+import numpy as np
+import pytest
+
+from paper_2602_05470_b200 import instances as I
+
+pytestmark = pytest.mark.gpu
+
+NEG_INF = -(1 << 30)
+MASK64 = (1 << 64) - 1
+
+
+@pytest.fixture(scope="module")
+def bb():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2602_05470_b200 import binding
+    binding.load()          # fails loudly if the extension is missing
+    return binding
+
+
+def _to_dev(e, c):
+    import torch
+    return (torch.from_numpy(np.ascontiguousarray(e)).cuda(),
+            torch.from_numpy(np.ascontiguousarray(c).view(np.int64)).cuda())
+
+
+def _oracle_gemm(oracle, Ae, Ac, Be, Bc):
+    Az = (Ae <= -(1 << 29)).astype(np.uint8); Bz = (Be <= -(1 << 29)).astype(np.uint8)
+    Ce, Cz, Cc = oracle.gemm(Ae.astype(np.int64), Az, Ac, Be.astype(np.int64), Bz, Bc)
+    Ce = np.where(Cz == 1, NEG_INF, Ce).astype(np.int32)
+    Cc = np.where(Cz == 1, 0, Cc).astype(np.uint64)
+    return Ce, Cc
+
+
+# ---- K3 alone -------------------------------------------------------------------------
+@pytest.mark.parametrize("B,M,N,K,seed,frac,wide", [
+    (1, 64, 64, 64, 1, 0.0, False),
+    (3, 256, 256, 256, 2, 0.0, False),
+    (2, 100, 70, 37, 3, 0.1, False),       # ragged tiles in every dimension + zero elements
+    (5, 1, 1, 1, 4, 0.0, False),
+    (1, 129, 65, 513, 5, 0.0, True),       # full-range uint64 counts: wrap-around mod 2^64
+    (4, 17, 200, 3, 6, 0.5, True),
+    (1, 1, 300, 1000, 7, 0.0, False),
+    (2, 333, 1, 129, 8, 0.3, False),
+])
+def test_gemm_matches_oracle(bb, oracle, B, M, N, K, seed, frac, wide):
+    Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed, neg_inf_frac=frac, wide_counts=wide)
+    want_e, want_c = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    for bits in (64, 32) if not wide else (64,):
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+        got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
+        assert (got_e == want_e).all()
+        assert (got_c == want_c).all()
+
+
+def test_gemm_shared_operand_stride0(bb, oracle):
+    Ae, Ac, Be, Bc = I.gemm_operands(4, 96, 80, 72, seed=11)
+    want_e, want_c = _oracle_gemm(oracle, Ae, Ac, np.broadcast_to(Be[0], Be.shape).copy(), np.broadcast_to(Bc[0], Bc.shape).copy())
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be[0], Bc[0])
+    Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc)
+    assert (Ce.cpu().numpy() == want_e).all() and (Cc.cpu().numpy().view(np.uint64) == want_c).all()
+
+
+def test_gemm_large_sampled_rows(bb, oracle):
+    # BASELINE config 4a size n = 1024: full oracle is 1e9 FMAs; check 16 sampled rows of one batch entry
+    n, B = 1024, 2
+    Ae, Ac, Be, Bc = I.gemm_operands(B, n, n, n, seed=21)
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc)
+    got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
+    rows = (I.splitmix64(5, 16, 20) % np.uint64(n)).astype(np.int64)
+    for b in range(B):
+        we, wc = _oracle_gemm(oracle, Ae[b:b + 1, rows], Ac[b:b + 1, rows], Be[b:b + 1], Bc[b:b + 1])
+        assert (got_e[b, rows] == we[0]).all() and (got_c[b, rows] == wc[0]).all()
+
+
+# ---- K2 alone -------------------------------------------------------------------------
+@pytest.mark.parametrize("r,B,seed", [(0, 3, 0), (1, 2, 1), (3, 5, 2), (7, 3, 3), (12, 4, 4), (16, 2, 5), (20, 1, 6)])
+def test_permute_matches_oracle(bb, oracle, r, B, seed):
+    n = 1 << r
+    perm = I.random_bit_permutation(r, seed)
+    src_e = (I.splitmix64(seed, B * n, 8) % np.uint64(100000)).astype(np.int32).reshape(B, n)
+    src_c = I.splitmix64(seed, B * n, 9).reshape(B, n)
+    want_e, want_c = oracle.permute(perm, src_e, src_c)
+    de, dc = _to_dev(src_e, src_c)
+    oe, oc = bb.permute_batched(perm, de, dc)
+    assert (oe.cpu().numpy() == want_e).all() and (oc.cpu().numpy().view(np.uint64) == want_c).all()
+    # pi then pi^-1 is the identity
+    be_, bc_ = bb.permute_batched(np.argsort(perm).astype(np.int32), oe, oc)
+    assert (be_.cpu().numpy() == src_e).all() and (bc_.cpu().numpy().view(np.uint64) == src_c).all()
+
+
+def test_permute_structured(bb, oracle):
+    # identity, full reversal, a single high<->low swap and a rotation (typical "move k to the top")
+    r, B = 14, 2
+    n = 1 << r
+    src_e = (I.splitmix64(1, B * n, 8) % np.uint64(1000)).astype(np.int32).reshape(B, n)
+    src_c = I.splitmix64(1, B * n, 9).reshape(B, n)
+    de, dc = _to_dev(src_e, src_c)
+    ident = np.arange(r, dtype=np.int32)
+    swap = ident.copy(); swap[0], swap[r - 1] = swap[r - 1], swap[0]
+    for perm in (ident, ident[::-1].copy(), swap, np.roll(ident, 3), np.roll(ident, -1)):
+        want_e, want_c = oracle.permute(perm, src_e, src_c)
+        oe, oc = bb.permute_batched(perm, de, dc)
+        assert (oe.cpu().numpy() == want_e).all() and (oc.cpu().numpy().view(np.uint64) == want_c).all()
+
+
+# ---- whole path: K1 -> (K2) -> K3 -> K4 -----------------------------------------------
+MODES = {"auto": 0, "streaming": 0x10, "tiled": 0x20, "auto_nograph": 0x4}
+
+
+def _check_leaves(bb, oracle, inst, tree, fixed, assign, flags=0, sample=None):
+    h = bb.Handle(inst, tree=tree, flags=flags)
+    energy, count = h.contract_batch(fixed, assign)[:2]
+    idx = range(len(assign)) if sample is None else sample
+    for b in idx:
+        we, wc = oracle.contract_tree(inst, tree[0], tree[1], fixed, assign[b]) if tree is not None else \
+            oracle.frontier_dp(inst, None, fixed, assign[b])
+        if we is None:
+            assert energy[b] == NEG_INF and count[b] == 0
+        else:
+            assert int(energy[b]) == we, (b, energy[b], we)
+            assert int(count[b]) == wc & MASK64, (b, count[b], wc)
+    h.close()
+    return energy, count
+
+
+@pytest.mark.parametrize("seed", range(1, 11))
+def test_config1_ising_6x6_unbranched(bb, oracle, seed):
+    # BASELINE config 1: 6x6 open +-J, 36 spins / 60 bonds, no field, no branching
+    inst = I.ising_lattice_2d(6, 6, seed)
+    assert inst.n_vertices == 36 and inst.n_edges == 60
+    tree = I.elimination_tree(inst.input_index_sets(), I.natural_order(36))
+    want = oracle.contract_tree(inst, *tree)
+    assert want == oracle.frontier_dp(inst)
+    for mode, fl in MODES.items():
+        h = bb.Handle(inst, tree=tree, flags=fl)
+        e, c = h.contract_batch()
+        assert (int(e[0]), int(c[0])) == want, mode
+    h = bb.Handle(inst)                  # library-derived tree
+    e, c = h.contract_batch()
+    assert (int(e[0]), int(c[0])) == want
+
+
+@pytest.mark.parametrize("seed", range(1, 11))
+def test_config2_kings_12x12(bb, oracle, seed):
+    # BASELINE config 2: King's subgraph 12x12, filling 0.8, unit weights
+    k = I.kings_subgraph(12, 12, 0.8, seed)
+    tree = I.elimination_tree(k.input_index_sets(), I.natural_order(k.n_vertices))
+    want = oracle.contract_tree(k, *tree)
+    assert want == oracle.frontier_dp(k)
+    for mode, fl in MODES.items():
+        h = bb.Handle(k, tree=tree, flags=fl)
+        e, c = h.contract_batch()
+        assert (int(e[0]), int(c[0])) == want, mode
+
+
+@pytest.mark.parametrize("mode", list(MODES))
+@pytest.mark.parametrize("case", range(6))
+def test_sliced_batches_all_modes(bb, oracle, mode, case):
+    if case == 0:
+        inst = I.ising_lattice_2d(5, 6, 3, field_h=1)
+    elif case == 1:
+        inst = I.kings_subgraph(6, 6, 0.8, 4, weights="rand")
+    elif case == 2:
+        inst = I.ising_lattice_3d(3, 3, 3, 5)
+    elif case == 3:
+        inst = I.random_graph(18, 0.25, 6, "ising", field_h=True)
+    elif case == 4:
+        inst = I.random_graph(20, 0.2, 7, "mis")
+    else:
+        inst = I.kings_subgraph(7, 5, 0.6, 8)            # isolated vertices likely (reading A7)
+    n = inst.n_vertices
+    f = 4
+    fixed = I.random_order(n, 40 + case)[:f]
+    assign = I.all_assignments(f)
+    # one tree built on the sliced network, one on the unsliced network (rank-0 inputs stay in the tree)
+    t_sliced = I.elimination_tree(inst.input_index_sets(fixed), I.random_order(n, 60 + case, exclude=fixed))
+    t_full = I.elimination_tree(inst.input_index_sets(), I.natural_order(n))
+    for tree in (t_sliced, t_full):
+        e, c = _check_leaves(bb, oracle, inst, tree, fixed, assign, MODES[mode])
+    # Eq. 3: (+) over all leaves == unbranched
+    whole = oracle.contract_tree(inst, *t_full)
+    feas = e != NEG_INF
+    if inst.kind == "ising":
+        best = int(e[feas].min())
+    else:
+        best = int(e[feas].max())
+    tot = sum(int(x) for x in c[feas & (e == best)])
+    assert (best, tot & MASK64) == (whole[0], whole[1] & MASK64)
+
+
+def test_infeasible_leaves_and_empty_fixed(bb, oracle):
+    k = I.kings_subgraph(4, 4, 1.0, 1)
+    fixed = np.array([0, 1, 5], np.int32)
+    assign = I.all_assignments(3)
+    tree = I.elimination_tree(k.input_index_sets(), I.natural_order(16))
+    e, c = _check_leaves(bb, oracle, k, tree, fixed, assign)
+    assert (e == NEG_INF).sum() == 4 and (c[e == NEG_INF] == 0).all()   # any two of {0,1,5} both in: adjacent
+    # everything fixed: the network is all scalars
+    inst = I.ising_lattice_2d(2, 3, 2, field_h=1)
+    fixed = np.arange(6, dtype=np.int32)
+    assign = I.all_assignments(6)
+    h = bb.Handle(inst)
+    e, c = h.contract_batch(fixed, assign)
+    for b in range(64):
+        we, wc = oracle.exhaustive(inst, fixed, assign[b])
+        assert (int(e[b]), int(c[b])) == (we, wc)
+
+
+def test_counts_wrap_mod_2_64_and_crt(bb, oracle):
+    # 30 disjoint AF triangles: count 6^30 > 2^64; 70 isolated spins: 2^70
+    import itertools
+    edges = []
+    for t in range(30):
+        edges += [(3 * t, 3 * t + 1), (3 * t + 1, 3 * t + 2), (3 * t, 3 * t + 2)]
+    n = 90 + 70
+    inst = I.Instance("ising", n, np.array([a for a, _ in edges], np.int32), np.array([b for _, b in edges], np.int32),
+                      -np.ones(len(edges), np.int32), None)
+    true = 6 ** 30 * 2 ** 70
+    h = bb.Handle(inst, flags=bb.BBTN_COUNT_CRT)
+    e, c, cm = h.contract_batch()
+    assert int(e[0]) == -30
+    assert int(c[0]) == true % (1 << 64)
+    assert int(cm[0, 0]) == true % bb.BBTN_P1 and int(cm[0, 1]) == true % bb.BBTN_P2
+    # CRT recovers counts below 2^64 * P1 * P2 ~ 2^126
+    inst2 = I.Instance("ising", 90, inst.edge_u, inst.edge_v, inst.edge_w, None)
+    h2 = bb.Handle(inst2, flags=bb.BBTN_COUNT_CRT)
+    e, c, cm = h2.contract_batch()
+    assert bb.crt_combine(c[0], cm[0, 0], cm[0, 1]) == 6 ** 30
+    # CRT residues on a branched lattice batch agree with the oracle's big integers
+    lat = I.ising_lattice_2d(6, 6, 9)
+    fixed = np.array([14, 15, 20], np.int32); assign = I.all_assignments(3)
+    tree = I.elimination_tree(lat.input_index_sets(fixed), I.natural_order(36, exclude=fixed))
+    h3 = bb.Handle(lat, tree=tree, flags=bb.BBTN_COUNT_CRT)
+    e, c, cm = h3.contract_batch(fixed, assign)
+    for b in range(8):
+        we, wc = oracle.contract_tree(lat, tree[0], tree[1], fixed, assign[b])
+        assert int(e[b]) == we and int(c[b]) == wc % (1 << 64)
+        assert int(cm[b, 0]) == wc % bb.BBTN_P1 and int(cm[b, 1]) == wc % bb.BBTN_P2
+
+
+def test_closed_forms_on_gpu(bb):
+    # north_star closed forms, straight through the CUDA path
+    for L in (3, 8, 12):
+        inst = I.ising_lattice_2d(L, L, 1, ferro=True)
+        e, c = bb.Handle(inst, tree=I.elimination_tree(inst.input_index_sets(), I.natural_order(L * L))).contract_batch()
+        assert (int(e[0]), int(c[0])) == (-2 * L * (L - 1), 2)
+    for L in (3, 5, 7, 9):
+        k = I.kings_subgraph(L, L, 1.0, 1)
+        e, c = bb.Handle(k, tree=I.elimination_tree(k.input_index_sets(), I.natural_order(L * L))).contract_batch()
+        assert (int(e[0]), int(c[0])) == (((L + 1) // 2) ** 2, 1)
+
+
+def test_config3_shape_branched_lattice_sampled(bb, oracle):
+    # config 3 at reduced size (12x12, slit of 6 -> 64 leaves): every leaf vs oracle-2, leaf-sum vs oracle-3
+    L, f = 12, 6
+    inst = I.ising_lattice_2d(L, L, 5)
+    fixed = I.slit_fixed_set_2d(L, L, f)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(L, L, f))
+    assign = I.all_assignments(f)
+    e, c = _check_leaves(bb, oracle, inst, tree, fixed, assign, sample=range(0, 64, 7))
+    whole = oracle.frontier_dp(inst)
+    best = int(e.min())
+    assert (best, sum(int(x) for x in c[e == best]) & MASK64) == (whole[0], whole[1] & MASK64)
+
+
+def test_batch_size_and_order_independence(bb):
+    inst = I.ising_lattice_2d(8, 8, 3)
+    fixed = I.slit_fixed_set_2d(8, 8, 4)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(8, 8, 4))
+    assign = I.all_assignments(4)
+    h = bb.Handle(inst, tree=tree)
+    e_all, c_all = h.contract_batch(fixed, assign)
+    for b in (0, 5, 15):
+        e1, c1 = h.contract_batch(fixed, assign[b:b + 1])
+        assert e1[0] == e_all[b] and c1[0] == c_all[b]
+    perm = np.argsort(I.splitmix64(1, 16, 0))
+    e_p, c_p = h.contract_batch(fixed, assign[perm])
+    assert (e_p == e_all[perm]).all() and (c_p == c_all[perm]).all()
+
+
+# ---- K5 + host B&B ---------------------------------------------------------------------
+def _grid_regions(rows, cols, br, bc, ids=None):
+    offs, verts = [0], []
+    for r0 in range(0, rows, br):
+        for c0 in range(0, cols, bc):
+            for r in range(r0, min(r0 + br, rows)):
+                for c in range(c0, min(c0 + bc, cols)):
+                    v = r * cols + c if ids is None else ids[r][c]
+                    if v >= 0:
+                        verts.append(v)
+            offs.append(len(verts))
+    return np.array(offs, np.int32), np.array(verts, np.int32)
+
+
+@pytest.mark.parametrize("case", range(4))
+def test_region_bound_matches_oracle(bb, oracle, case):
+    rows, cols = 6, 7
+    if case % 2 == 0:
+        inst = I.ising_lattice_2d(rows, cols, case, field_h=case - 1)
+        ids = None
+    else:
+        inst = I.kings_subgraph(rows, cols, 0.8, case, weights="rand" if case == 3 else "unit")
+        ids = -np.ones((rows, cols), int); ids[inst.meta["keep"]] = np.arange(inst.n_vertices)
+    offs, verts = _grid_regions(rows, cols, 3, 3, ids)
+    f = 5
+    fixed = I.random_order(inst.n_vertices, 90 + case)[:f]
+    assign = I.all_assignments(f)
+    h = bb.Handle(inst)
+    got = h.region_bound(offs, verts, fixed, assign)
+    energy, _ = h.contract_batch(fixed, assign)
+    for b in range(len(assign)):
+        want = oracle.region_bound(inst, offs, verts, fixed, assign[b])
+        if want is None:
+            assert got[b] == NEG_INF
+            continue
+        assert int(got[b]) == (-want if inst.kind == "ising" else want)
+        # admissible: never cuts off the exact value of the leaf
+        if inst.kind == "ising":
+            assert got[b] <= energy[b]
+        else:
+            assert got[b] >= energy[b]
+    # no regions at all, and no fixed vertices
+    got0 = h.region_bound([0], [], fixed, assign)
+    for b in (0, 7, 31):
+        want = oracle.region_bound(inst, [0], [], fixed, assign[b])
+        assert (got0[b] == NEG_INF) if want is None else int(got0[b]) == (-want if inst.kind == "ising" else want)
+    w = oracle.region_bound(inst, offs, verts)
+    assert int(h.region_bound(offs, verts)[0]) == (-w if inst.kind == "ising" else w)
+
+
+@pytest.mark.parametrize("case", range(4))
+def test_solve_bb_matches_unbranched(bb, oracle, case):
+    if case % 2 == 0:
+        rows, cols = 8, 8
+        inst = I.ising_lattice_2d(rows, cols, 10 + case)
+        ids = None
+        branch = np.array([r * cols + cols // 2 for r in range(rows)], np.int32)
+    else:
+        rows, cols = 9, 9
+        inst = I.kings_subgraph(rows, cols, 0.8, 10 + case)
+        ids = -np.ones((rows, cols), int); ids[inst.meta["keep"]] = np.arange(inst.n_vertices)
+        branch = np.array([ids[r][cols // 2] for r in range(rows) if ids[r][cols // 2] >= 0], np.int32)
+    offs, verts = _grid_regions(rows, cols, 3, 3, ids)
+    whole = oracle.frontier_dp(inst)
+    h = bb.Handle(inst, flags=bb.BBTN_COUNT_CRT)
+    for pruning in (False, True):
+        out = h.solve_bb(branch, 3, offs, verts, max_batch=64, use_pruning=pruning)
+        assert (out["energy"], out["count"]) == (whole[0], whole[1] & MASK64)
+        assert out["count_mod"] == (whole[1] % bb.BBTN_P1, whole[1] % bb.BBTN_P2)
+        if not pruning and inst.kind == "ising":
+            assert out["contracted"] == 1 << len(branch)
+    assert out["contracted"] <= 1 << len(branch)
