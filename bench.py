@@ -1,0 +1,377 @@
+#!/usr/bin/env python
+"""bench.py -- measurement of the BBTN hot path on B200 (contract of the driver).
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+Workload = BASELINE.json configs[3], the configuration the metric ("counting-tropical GEMM Gop/s & %
+of int32 CUDA-core peak") is quoted on.  ONE STEP is one pass of the whole hot path over one batch:
+  (a) raw batched counting-tropical GEMM (K3 tiled): M=N=K=1024, batch 64 per GPU, energies uniform
+      in [-64,64], counts uniform in {1..4} (so the caller promises count_bits = 3);
+  (b) the 5x5x5 open +-J cube, 2^f leaves (f = 8 spins of the central layer, all assignments) per
+      GPU: K5 region bounds for every leaf, then K1 construct -> K2 permute / K3 GEMM (tiled and
+      streaming forms, chosen per tree node by the planner) -> K4 finalize.
+Units: 1 tropical FMA = one (batch, m, n, k) term ((.) then (+)); Gop/s = 2 x GFMA/s.
+`value` counts the planner's algorithmic FMAs (leaf-invariant nodes once), inputs resident in HBM;
+`e2e` is the same step through the host-pointer C-ABI calls (H2D of operands/assignments and D2H of
+results inside the timed region).  Weak scaling: every rank runs its own seeded batch; no collective
+on the data path (results are 12 bytes per leaf).  Inputs are larger than L2 (no flush needed).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2602_05470_b200 import instances as I  # noqa: E402  (seeded inputs only; no arithmetic of the method)
+
+GEMM_N, GEMM_BATCH = 1024, 64
+CUBE_L, CUBE_F = 5, 8
+METRIC = "counting-tropical GEMM Gop/s (2 x tropical FMA/s) over one pass of the hot path"
+# int32 lane-instructions a tropical FMA needs on this ISA:
+# fused add-max, tie test = add + compare, multiply-accumulate of the counts (1 IMAD.WIDE for <=32-bit
+# operand counts, 3 IMADs for full 64x64->64).
+INT_OPS_PER_FMA = {32: 4, 64: 6}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d.get("hbm_gbs", 6650.0), "measured", d.get("sm_max_mhz", 1965.0)
+    return 6650.0, "fallback", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for _, r in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cube_problem(seed: int):
+    inst = I.ising_lattice_3d(CUBE_L, CUBE_L, CUBE_L, seed)
+    fixed = I.layer_fixed_set_3d(CUBE_L, CUBE_L, CUBE_L, CUBE_F)
+    assign = I.all_assignments(CUBE_F)
+    # K5 regions: the 2x2x2-ish blocks of the cube (disjoint, <= 12 vertices each)
+    offs, verts = [0], []
+    L = CUBE_L
+    for z0 in range(0, L, 2):
+        for y0 in range(0, L, 2):
+            for x0 in range(0, L, 3):
+                verts += [(z * L + y) * L + x for z in range(z0, min(z0 + 2, L)) for y in range(y0, min(y0 + 2, L))
+                          for x in range(x0, min(x0 + 3, L))]
+                offs.append(len(verts))
+    return inst, fixed, assign, np.array(offs, np.int32), np.array(verts, np.int32)
+
+
+# ----------------------------------------------------------------------------------------------
+# reference arm: the oracle, as it stands, on the host cores, on a bounded sample of the same step
+# ----------------------------------------------------------------------------------------------
+def oracle_sample(seed: int, rows: int = 32, leaves: int = 4):
+    """One bounded sample of the step through oracle/: `rows` rows of one GEMM batch entry (OpenMP over
+    rows) and `leaves` leaves of the cube (naive loop-nest contraction, one thread per leaf).
+    Returns (tropical FMAs done, seconds, threads used, description)."""
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+    oracle.build()
+    n = GEMM_N
+    Ae, Ac, Be, Bc = I.gemm_operands(1, n, n, n, seed)
+    Ae, Ac = Ae[:, :rows].astype(np.int64), Ac[:, :rows]
+    Be64 = Be.astype(np.int64)
+    z = lambda a: np.zeros(a.shape, np.uint8)
+    inst, fixed, assign, _, _ = cube_problem(seed)
+    tree = _cube_tree(inst, fixed)
+    cores = os.cpu_count() or 1
+    t0 = time.perf_counter()
+    oracle.gemm(Ae, z(Ae), Ac, Be64, z(Be64), Bc)
+    with ThreadPoolExecutor(max_workers=min(leaves, cores)) as ex:
+        list(ex.map(lambda b: oracle.contract_tree(inst, tree[0], tree[1], fixed, assign[b]), range(leaves)))
+    dt = time.perf_counter() - t0
+    fma = float(rows) * n * n + leaves * I.tree_fma(inst.input_index_sets(fixed), tree)
+    return fma, dt, cores, (f"oracle/: {rows} rows of one {n}^3 GEMM entry (OpenMP) + {leaves} of {1 << CUBE_F} cube leaves "
+                            f"(naive loop-nest tree contraction, one thread each)")
+
+
+def _cube_tree(inst, fixed):
+    """Contraction tree of the cube used by BOTH arms: bucket elimination along a min-degree order
+    (instances.py: pure graph structure)."""
+    return I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    vals = []
+    for s in range(args.warmup + args.steps):
+        fma, dt, cores, desc = oracle_sample(args.seed + s, rows=args.ref_rows, leaves=args.ref_leaves)
+        if s >= args.warmup:
+            vals.append((fma, dt))
+    tot_f = sum(f for f, _ in vals); tot_t = sum(t for _, t in vals)
+    v = 2.0 * tot_f / tot_t / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "Gop/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(args.steps, 1), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32 energy + uint64 count (oracle: int64 + 256-bit)",
+            "data": "synthetic", "config": _config(args),
+            "cpu_baseline": {"value": v, "unit": "Gop/s", "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": "Gop/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def _config(args):
+    return {"workload": (f"BASELINE configs[3]: raw batched counting-tropical GEMM M=N=K={GEMM_N} batch {GEMM_BATCH} "
+                         f"(energies U[-64,64], counts U{{1..4}}) + {CUBE_L}x{CUBE_L}x{CUBE_L} open +-J cube, "
+                         f"f={CUBE_F} fixed spins of the central layer, all {1 << CUBE_F} leaves, per GPU"),
+            "gemm": {"M": GEMM_N, "N": GEMM_N, "K": GEMM_N, "batch_per_gpu": GEMM_BATCH, "count_bits": 3},
+            "cube": {"L": CUBE_L, "n_fixed": CUBE_F, "leaves_per_gpu": 1 << CUBE_F},
+            "l2_policy": "inputs larger than L2 (2.4 GB of GEMM planes, multi-GB contraction arena); no flush",
+            "seed": args.seed}
+
+
+# ----------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2602_05470_b200 import binding as bb
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    bb.load()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_peak, peak_kind, sm_max = _peaks()
+    seed = args.seed + 1000 * rank
+    stream = torch.cuda.Stream()
+    sp = stream.cuda_stream
+
+    # ---- inputs (a): GEMM planes, resident in HBM
+    n, gb = GEMM_N, GEMM_BATCH
+    Ae, Ac, Be, Bc = I.gemm_operands(gb, n, n, n, seed)
+    pin = lambda a: torch.from_numpy(a.view(np.int64) if a.dtype == np.uint64 else a).pin_memory()
+    hAe, hAc, hBe, hBc = pin(Ae), pin(Ac), pin(Be), pin(Bc)
+    dAe, dAc, dBe, dBc = (t.cuda(non_blocking=True) for t in (hAe, hAc, hBe, hBc))
+    dCe = torch.empty((gb, n, n), dtype=torch.int32, device="cuda")
+    dCc = torch.empty((gb, n, n), dtype=torch.int64, device="cuda")
+    hCe = torch.empty((gb, n, n), dtype=torch.int32).pin_memory()
+    hCc = torch.empty((gb, n, n), dtype=torch.int64).pin_memory()
+    gemm_fma = float(gb) * n * n * n
+
+    # ---- inputs (b): cube
+    inst, fixed, assign, roffs, rverts = cube_problem(seed)
+    tree = _cube_tree(inst, fixed)
+    B = len(assign)
+    h_dev = bb.Handle(inst, tree=tree, max_elements_per_leaf=1 << 26, flags=bb.BBTN_IO_DEVICE)
+    h_host = bb.Handle(inst, tree=tree, max_elements_per_leaf=1 << 26)
+    info = h_dev.plan_query(fixed, B)
+    cube_fma = info["fma_variant"] * B + info["fma_invariant"]
+    d_assign = torch.from_numpy(assign).cuda()
+    d_energy = torch.empty(B, dtype=torch.int32, device="cuda")
+    d_count = torch.empty(B, dtype=torch.int64, device="cuda")
+    d_bound = torch.empty(B, dtype=torch.int32, device="cuda")
+    step_fma = gemm_fma + cube_fma
+    launches_per_step = 1 + 2 + info["n_kernel_launches"]
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    gemm_ev = []
+
+    def step_device(record=False):
+        with torch.cuda.stream(stream):
+            h_dev.region_bound_device(roffs, rverts, fixed, d_assign, d_bound, stream=sp)
+            h_dev.contract_batch_device(fixed, d_assign, d_energy, d_count, stream=sp)
+            if record:
+                a, b = ev(), ev()
+                a.record(stream)
+            bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=3, stream=sp)
+            if record:
+                b.record(stream)
+                gemm_ev.append((a, b))
+
+    def step_host():
+        bound = h_host.region_bound(roffs, rverts, fixed, assign, stream=sp)
+        e, c = h_host.contract_batch(fixed, assign, stream=sp)
+        bb.tropical_gemm_batched_host(hAe, hAc, hBe, hBc, hCe, hCc, count_bits=3, stream=sp)
+        return bound, e, c
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        step_device()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    t_wall0 = time.time()
+    e0, e1 = ev(), ev()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step_device(record=True)
+    e1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    ms = e0.elapsed_time(e1)
+    gemm_ms = float(np.mean([a.elapsed_time(b) for a, b in gemm_ev]))
+    energy_dev = d_energy.cpu().numpy().copy(); count_dev = d_count.cpu().numpy().copy()
+
+    # ---- end-to-end timing through the host-pointer calls
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for _ in range(min(args.warmup, 2)):
+        step_host()
+    barrier()
+    a, b = ev(), ev()
+    a.record(stream)
+    for _ in range(e2e_steps):
+        bound, e_h, c_h = step_host()
+    b.record(stream)
+    barrier()
+    ms_e2e = a.elapsed_time(b)
+    assert (e_h == energy_dev).all() and (c_h.view(np.int64) == count_dev).all(), "host and device paths disagree"
+    h2d = Ae.nbytes + Ac.nbytes + Be.nbytes + Bc.nbytes + 2 * assign.nbytes
+    d2h = hCe.numel() * 4 + hCc.numel() * 8 + B * (4 + 8 + 4)
+
+    if world > 1:
+        t = torch.tensor([ms, ms_e2e, gemm_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_e2e, gemm_ms = (float(x) for x in t.cpu())
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    value = 2.0 * step_fma * world * args.steps / (ms * 1e-3) / 1e9
+    e2e_value = 2.0 * step_fma * world * e2e_steps / (ms_e2e * 1e-3) / 1e9
+
+    # ---- ALU roofline of the dominant kernel (K3 tiled GEMM), against the committed microbenchmark
+    mb = {}
+    for which, name in ((0, "iadd3"), (1, "imnmx"), (2, "viaddmnmx"), (3, "imad"), (4, "iadd3+imad"), (6, "opmix_u32"), (5, "opmix_u64")):
+        t_ms, ops = bb.int32_microbench(which, args.microbench_iters)
+        mb[name] = ops / (t_ms * 1e-3) / 1e9          # G lane-ops/s (which <= 4) or GFMA/s (op mix)
+    int_peak = max(mb["iadd3+imad"], mb["iadd3"], mb["imnmx"], mb["imad"])
+    alu_peak = max(mb["iadd3"], mb["imnmx"], mb["viaddmnmx"])
+    gemm_gfma = gemm_fma / (gemm_ms * 1e-3) / 1e9
+    achieved = INT_OPS_PER_FMA[32] * gemm_gfma
+    roofline = {"bound": "alu", "kernel": "gemm_tiled_kernel (K3)", "achieved": achieved, "peak": int_peak, "unit": "Gop/s",
+                "frac": achieved / int_peak, "traffic": None,
+                "note": (f"op = int32 lane-instruction; achieved = {INT_OPS_PER_FMA[32]} algorithmic int32 instructions per tropical FMA "
+                         "(fused add-max, tie add, tie compare, 32x32+64 multiply-add) x GFMA/s of the K3 launch; peak = committed "
+                         "microbenchmark (bbtn_int32_microbench), best of IADD3 / IMNMX / IMAD / mixed IADD3+IMAD issue, same run"),
+                "gemm_gfma_per_s": gemm_gfma, "gemm_gop_per_s": 2 * gemm_gfma, "gemm_ms_per_launch": gemm_ms,
+                "frac_of_opmix_ceiling": gemm_gfma / mb["opmix_u32"],
+                "frac_of_alu_pipe_peak_2ops": 2 * gemm_gfma / alu_peak,
+                "microbench_Gops": mb, "share_of_step": gemm_ms * args.steps / ms,
+                "hbm_peak_gbs": hbm_peak, "hbm_peak_kind": peak_kind}
+
+    # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        fma, dt, cores, desc = oracle_sample(args.seed, rows=args.ref_rows, leaves=args.ref_leaves)
+        cpu = {"value": 2.0 * fma / dt / 1e9, "unit": "Gop/s", "cores": cores, "kind": "oracle", "sample": desc,
+               "seconds": dt}
+
+    line = {"metric": METRIC, "value": value, "unit": "Gop/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "int32 energy + uint64 count", "data": "synthetic", "config": _config(args),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": "Gop/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
+            "gpu_launches": int(launches_per_step * args.steps),
+            "roofline": roofline, "cpu_baseline": cpu,
+            "plan": {k: info[k] for k in ("n_nodes", "n_variant_nodes", "max_rank", "n_gemm_tiled", "n_absorb", "n_permute",
+                                          "n_trace", "n_kernel_launches", "workspace_bytes")},
+            "fma_per_step": {"gemm": gemm_fma, "cube": cube_fma},
+            "result_check": {"cube_E0": int(energy_dev.min()),
+                             "cube_count_mod_2_64": int(sum(int(x) for x in count_dev.view(np.uint64)[energy_dev == energy_dev.min()]) & ((1 << 64) - 1))}}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--ref-rows", type=int, default=128)
+    ap.add_argument("--ref-leaves", type=int, default=16)
+    ap.add_argument("--microbench-iters", type=int, default=4000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3          # timing rule: W >= 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -100,6 +100,8 @@ typedef struct {
   double  fma_invariant;      /* tropical FMAs in leaf-invariant nodes (once per call)             */
   double  bytes_per_call;     /* algorithmic bytes read+written by all kernels for this B          */
   int64_t workspace_bytes;    /* device memory the plan holds for this B                           */
+  int32_t n_kernel_launches;  /* kernels one bbtn_contract_batch enqueues per count ring (K1..K4)  */
+  int32_t reserved;
 } bbtn_plan_info;
 
 /* Build a handle: validates and copies the problem (graph, weights, tree).  Host only: device
@@ -160,6 +162,17 @@ int bbtn_solve_bb(bbtn_handle *h,
                   int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats,
                   void *cuda_stream);
 
+/* Host-side (+) over leaf results in reported units (Eq. 3's outer sum; "the final
+ * result is obtained by summing the contractions of each branch"): keeps the best
+ * energy (Ising: lowest, MIS: highest), adds the counts of the leaves that attain it (mod 2^64,
+ * and mod P1/P2 when count_mod != NULL).  Infeasible leaves (BBTN_NEG_INF) are neutral; if all n
+ * are infeasible (or n == 0) the result is (BBTN_NEG_INF, 0).  Part of S6 (plain C++, no device):
+ * bbtn_solve_bb uses it per batch, a multi-process driver uses it across ranks.
+ *   kind: bbtn_kind; energy/count [n]; count_mod [n][2] or NULL; out_count_mod [2] or NULL. */
+int bbtn_oplus_combine(int32_t kind, int64_t n, const int32_t *energy, const uint64_t *count,
+                       const uint32_t *count_mod, int32_t *out_energy, uint64_t *out_count,
+                       uint32_t *out_count_mod);
+
 /* Raw batched counting-tropical GEMM (K3 alone; the config-4 sweep):
  *   C[b,m,n] = (+)_k A[b,m,k] (.) B[b,k,n]
  * ALL pointers are DEVICE pointers.  Row-major: A [batch][M][K], B [batch][K][N], C [batch][M][N];
@@ -174,6 +187,17 @@ int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,
                                int32_t *Ce, uint64_t *Cc,
                                int64_t strideA, int64_t strideB, int64_t strideC,
                                int32_t count_bits, void *cuda_stream);
+
+/* Same operation with HOST pointers (the end-to-end form of the config-4 sweep): the operands are
+ * copied to library-owned device staging buffers on `cuda_stream` (pass pinned memory for full
+ * PCIe speed), K3 runs, C is copied back and the call returns after the results landed.
+ * On BBTN_ECUDA during the copy-back the contents of Ce/Cc are unspecified. */
+int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t K,
+                                    const int32_t *Ae, const uint64_t *Ac,
+                                    const int32_t *Be, const uint64_t *Bc,
+                                    int32_t *Ce, uint64_t *Cc,
+                                    int64_t strideA, int64_t strideB, int64_t strideC,
+                                    int32_t count_bits, void *cuda_stream);
 
 /* Raw batched bit permutation (K2 alone): dst[b][pi(i)] = src[b][i] for i in [0, 2^rank), where
  * bit j of pi(i) is bit perm[j] of i (perm is a HOST array, a permutation of 0..rank-1).

@@ -24,7 +24,8 @@ BBTN_FORCE_STREAMING, BBTN_FORCE_TILED = 0x10, 0x20
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
 EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb",
-           "bbtn_tropical_gemm_batched", "bbtn_permute_batched", "bbtn_int32_microbench",
+           "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
+           "bbtn_permute_batched", "bbtn_int32_microbench",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
 
 
@@ -45,7 +46,8 @@ class _PlanInfo(C.Structure):
     _fields_ = [("n_nodes", C.c_int32), ("n_variant_nodes", C.c_int32), ("max_rank", C.c_int32),
                 ("n_gemm_tiled", C.c_int32), ("n_absorb", C.c_int32), ("n_permute", C.c_int32), ("n_trace", C.c_int32),
                 ("rho", C.c_int64), ("fma_variant", C.c_double), ("fma_invariant", C.c_double),
-                ("bytes_per_call", C.c_double), ("workspace_bytes", C.c_int64)]
+                ("bytes_per_call", C.c_double), ("workspace_bytes", C.c_int64),
+                ("n_kernel_launches", C.c_int32), ("reserved", C.c_int32)]
 
 
 def load():
@@ -64,6 +66,8 @@ def load():
     lib.bbtn_region_bound.argtypes = [vp, vp, vp, i32, vp, i32, vp, i64, vp, vp]
     lib.bbtn_solve_bb.argtypes = [vp, vp, i32, i32, vp, vp, i32, i64, i32, i32, vp, vp, vp, vp, vp]
     lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
+    lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
+    lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
     lib.bbtn_permute_batched.argtypes = [i32, vp, i64, vp, vp, vp, vp, vp]
     lib.bbtn_int32_microbench.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     lib.bbtn_destroy.argtypes = [vp]
@@ -168,6 +172,13 @@ class Handle:
                                         _ptr(bound), _stream(stream)), self._h)
         return bound
 
+    # -- bbtn_region_bound, device pointers (handle built with BBTN_IO_DEVICE); torch tensors
+    def region_bound_device(self, region_offsets, region_vertices, fixed, assign_t, bound_t, stream=None):
+        ro, rv = _np(region_offsets, np.int32), _np(region_vertices, np.int32)
+        fx = np.zeros(0, np.int32) if fixed is None else _np(fixed, np.int32)
+        _check(load().bbtn_region_bound(self._h, _ptr(ro), _ptr(rv), len(ro) - 1, _ptr(fx), len(fx), _ptr(assign_t),
+                                        int(bound_t.shape[0]), _ptr(bound_t), _stream(stream)), self._h)
+
     def solve_bb(self, branch_vertices, chunk, region_offsets, region_vertices, max_batch=1024,
                  incumbent_hint=BBTN_NEG_INF, use_pruning=True, stream=None):
         bv = _np(branch_vertices, np.int32)
@@ -199,6 +210,33 @@ def tropical_gemm_batched(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64
     _check(load().bbtn_tropical_gemm_batched(batch, M, N, K, _ptr(Ae), _ptr(Ac), _ptr(Be), _ptr(Bc), _ptr(Ce), _ptr(Cc),
                                              M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, _stream(stream)))
     return Ce, Cc
+
+
+def tropical_gemm_batched_host(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, stream=None):
+    """bbtn_tropical_gemm_batched_host: same layouts on HOST arrays (numpy, or pinned CPU torch tensors with
+    int64 storage for the counts); copies in, runs K3, copies C back."""
+    shp = lambda a: tuple(a.shape)
+    a3, b3 = len(shp(Ae)) == 3, len(shp(Be)) == 3
+    batch = shp(Ae)[0] if a3 else (shp(Be)[0] if b3 else 1)
+    M, K = shp(Ae)[-2:]
+    N = shp(Be)[-1]
+    assert shp(Be)[-2] == K
+    if Ce is None:
+        Ce = np.empty((batch, M, N), np.int32); Cc = np.empty((batch, M, N), np.uint64)
+    _check(load().bbtn_tropical_gemm_batched_host(batch, M, N, K, _ptr(Ae), _ptr(Ac), _ptr(Be), _ptr(Bc), _ptr(Ce), _ptr(Cc),
+                                                  M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, _stream(stream)))
+    return Ce, Cc
+
+
+def oplus_combine(kind, energy, count, count_mod=None):
+    """bbtn_oplus_combine: (+) over leaf results in reported units (Eq. 3's outer sum).  Host only."""
+    e = _np(energy, np.int32); c = _np(count, np.uint64)
+    cm = None if count_mod is None else _np(count_mod, np.uint32)
+    oe = C.c_int32(); oc = C.c_uint64(); om = (C.c_uint32 * 2)()
+    k = {"ising": 0, "mis": 1, 0: 0, 1: 1}[kind]
+    _check(load().bbtn_oplus_combine(k, len(e), _ptr(e), _ptr(c), _ptr(cm), C.addressof(oe), C.addressof(oc),
+                                     C.addressof(om) if cm is not None else None))
+    return (oe.value, oc.value) if cm is None else (oe.value, oc.value, (om[0], om[1]))
 
 
 def permute_batched(perm, src_e, src_c, dst_e=None, dst_c=None, stream=None):

@@ -207,6 +207,10 @@ int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, int64
   info->fma_variant = pl.fma_variant; info->fma_invariant = pl.fma_invariant;
   info->bytes_per_call = pl.bytes_variant * (double)B + pl.bytes_invariant;
   info->workspace_bytes = (pl.arena_variant_elems * B + pl.arena_invariant_elems) * 12;
+  int n_var = 0, n_inv = 0;
+  for (const InputRec &r : pl.inputs) if (r.rank > 0) (r.variant ? n_var : n_inv)++;
+  // K1: variant tensors, invariant tensors, offset[b]; K4: finalize
+  info->n_kernel_launches = (int32_t)pl.steps.size() + (n_var > 0) + (n_inv > 0) + 2;
   return BBTN_OK;
 }
 
@@ -280,6 +284,35 @@ int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, c
   launch_gemm_tiled(batch, 1, M, N, K, 0, Ae, Ac, Be, Bc, Ce, Cc, strideA, strideB, strideC, RING_U64, count_bits,
                     (cudaStream_t)stream);
   CUDA_TRY(nullptr, cudaGetLastError());
+  return BBTN_OK;
+}
+
+int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac,
+                                    const int32_t *Be, const uint64_t *Bc, int32_t *Ce, uint64_t *Cc,
+                                    int64_t strideA, int64_t strideB, int64_t strideC, int32_t count_bits, void *stream) {
+  if (batch < 1 || M < 1 || N < 1 || K < 1 || !Ae || !Ac || !Be || !Bc || !Ce || !Cc || strideA < 0 || strideB < 0 || strideC < 0)
+    return fail(nullptr, BBTN_EINVAL, "bad GEMM arguments");
+  if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
+  if ((strideA && strideA < (int64_t)M * K) || (strideB && strideB < (int64_t)K * N))
+    return fail(nullptr, BBTN_EINVAL, "operand stride smaller than the operand");
+  if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  static thread_local DevBuf st_e[3], st_c[3];
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t nA = (size_t)(strideA ? (batch - 1) * strideA : 0) + (size_t)M * K;
+  const size_t nB = (size_t)(strideB ? (batch - 1) * strideB : 0) + (size_t)K * N;
+  const size_t nC = (size_t)(batch - 1) * strideC + (size_t)M * N;
+  const size_t n[3] = {nA, nB, nC};
+  for (int i = 0; i < 3; i++) { CUDA_TRY(nullptr, st_e[i].ensure(n[i] * 4)); CUDA_TRY(nullptr, st_c[i].ensure(n[i] * 8)); }
+  CUDA_TRY(nullptr, cudaMemcpyAsync(st_e[0].p, Ae, nA * 4, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(nullptr, cudaMemcpyAsync(st_c[0].p, Ac, nA * 8, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(nullptr, cudaMemcpyAsync(st_e[1].p, Be, nB * 4, cudaMemcpyHostToDevice, st));
+  CUDA_TRY(nullptr, cudaMemcpyAsync(st_c[1].p, Bc, nB * 8, cudaMemcpyHostToDevice, st));
+  launch_gemm_tiled(batch, 1, M, N, K, 0, (const int32_t *)st_e[0].p, st_c[0].p, (const int32_t *)st_e[1].p, st_c[1].p,
+                    (int32_t *)st_e[2].p, st_c[2].p, strideA, strideB, strideC, RING_U64, count_bits, st);
+  CUDA_TRY(nullptr, cudaGetLastError());
+  CUDA_TRY(nullptr, cudaMemcpyAsync(Ce, st_e[2].p, nC * 4, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(nullptr, cudaMemcpyAsync(Cc, st_c[2].p, nC * 8, cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(nullptr, cudaStreamSynchronize(st));
   return BBTN_OK;
 }
 

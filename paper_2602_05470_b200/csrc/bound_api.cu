@@ -99,6 +99,15 @@ int build_bound_plan(bbtn_handle *h, const int32_t *roff, const int32_t *rv, int
   return BBTN_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+int bbtn_oplus_combine(int32_t kind, int64_t n, const int32_t *energy, const uint64_t *count, const uint32_t *count_mod,
+                       int32_t *out_energy, uint64_t *out_count, uint32_t *out_count_mod);
+}
+
+namespace {
 struct BB {
   bbtn_handle *h; cudaStream_t st;
   const int32_t *branch; int n_branch, chunk;
@@ -115,16 +124,16 @@ struct BB {
     int rc = bbtn_contract_batch(h, branch, d, asg.data(), B, e.data(), c.data(), crt ? cm.data() : nullptr, st);
     if (rc) return rc;
     stats[2] += B; stats[3] += 1;
-    for (int64_t b = 0; b < B; b++) {
-      if (e[b] == BBTN_NEG_INF) continue;
-      const bool better = !have_best || (ising ? e[b] < best : e[b] > best);
-      if (better) { best = e[b]; cnt = 0; m1 = m2 = 0; have_best = true; }
-      if (e[b] == best) {
-        cnt += c[b];
-        if (crt) { m1 = (m1 + cm[2 * b]) % BBTN_P1; m2 = (m2 + cm[2 * b + 1]) % BBTN_P2; }
-      }
-      if (!have_inc || (ising ? e[b] < inc : e[b] > inc)) { inc = e[b]; have_inc = true; }
-    }
+    // (+) over the batch, then into the running result (Eq. 3's outer sum)
+    int32_t e2[2] = {have_best ? best : BBTN_NEG_INF, BBTN_NEG_INF}; uint64_t c2[2] = {cnt, 0}; uint32_t cm2[4] = {(uint32_t)m1, (uint32_t)m2, 0, 0};
+    rc = bbtn_oplus_combine(ising ? BBTN_ISING : BBTN_MIS, B, e.data(), c.data(), crt ? cm.data() : nullptr, &e2[1], &c2[1], crt ? &cm2[2] : nullptr);
+    if (rc) return rc;
+    uint32_t om[2] = {0, 0};
+    rc = bbtn_oplus_combine(ising ? BBTN_ISING : BBTN_MIS, 2, e2, c2, crt ? cm2 : nullptr, &best, &cnt, crt ? om : nullptr);
+    if (rc) return rc;
+    m1 = om[0]; m2 = om[1];
+    have_best = best != BBTN_NEG_INF;
+    if (have_best && (!have_inc || (ising ? best < inc : best > inc))) { inc = best; have_inc = true; }
     return BBTN_OK;
   }
 
@@ -166,7 +175,6 @@ struct BB {
     return BBTN_OK;
   }
 };
-
 }  // namespace
 
 extern "C" {
@@ -199,6 +207,26 @@ int bbtn_region_bound(bbtn_handle *h, const int32_t *region_offsets, const int32
     CUDA_TRY(h, cudaStreamSynchronize(st));
     std::memcpy(bound, tmp.data(), (size_t)B * 4);
   }
+  return BBTN_OK;
+}
+
+int bbtn_oplus_combine(int32_t kind, int64_t n, const int32_t *energy, const uint64_t *count, const uint32_t *count_mod,
+                       int32_t *out_energy, uint64_t *out_count, uint32_t *out_count_mod) {
+  if ((kind != BBTN_ISING && kind != BBTN_MIS) || n < 0 || (n > 0 && (!energy || !count)) || !out_energy || !out_count ||
+      (out_count_mod && n > 0 && !count_mod))
+    return fail(nullptr, BBTN_EINVAL, "bad oplus_combine arguments");
+  bool have = false; int32_t best = BBTN_NEG_INF; uint64_t cnt = 0, m1 = 0, m2 = 0;
+  for (int64_t b = 0; b < n; b++) {
+    if (energy[b] == BBTN_NEG_INF) continue;
+    if (!have || (kind == BBTN_ISING ? energy[b] < best : energy[b] > best)) { best = energy[b]; cnt = 0; m1 = m2 = 0; have = true; }
+    if (energy[b] == best) {
+      cnt += count[b];
+      if (out_count_mod) { m1 = (m1 + count_mod[2 * b]) % BBTN_P1; m2 = (m2 + count_mod[2 * b + 1]) % BBTN_P2; }
+    }
+  }
+  *out_energy = have ? best : BBTN_NEG_INF;
+  *out_count = have ? cnt : 0;
+  if (out_count_mod) { out_count_mod[0] = (uint32_t)m1; out_count_mod[1] = (uint32_t)m2; }
   return BBTN_OK;
 }
 

@@ -264,6 +264,63 @@ def elimination_tree(index_sets: list[list[int]], order) -> tuple[np.ndarray, np
     return np.array(tl, np.int32), np.array(tr, np.int32)
 
 
+def min_degree_order(inst: "Instance", fixed=()) -> np.ndarray:
+    """Greedy min-degree elimination order of the free vertices (ties: fewest fill edges, then lowest
+    id) on the graph with `fixed` removed.  Graph structure only."""
+    n = inst.n_vertices
+    fx = set(int(v) for v in fixed)
+    adj = [set() for _ in range(n)]
+    for u, v in zip(inst.edge_u, inst.edge_v):
+        u, v = int(u), int(v)
+        if u in fx or v in fx:
+            continue
+        adj[u].add(v); adj[v].add(u)
+    alive = [v for v in range(n) if v not in fx]
+    order = []
+
+    def fill(v):
+        nb = list(adj[v])
+        return sum(1 for i in range(len(nb)) for j in range(i + 1, len(nb)) if nb[j] not in adj[nb[i]])
+
+    while alive:
+        dmin = min(len(adj[x]) for x in alive)
+        v = min((x for x in alive if len(adj[x]) == dmin), key=lambda x: (fill(x), x))
+        alive.remove(v)
+        order.append(v)
+        nb = list(adj[v])
+        for a in nb:
+            adj[a].discard(v)
+        for i in range(len(nb)):
+            for j in range(i + 1, len(nb)):
+                adj[nb[i]].add(nb[j]); adj[nb[j]].add(nb[i])
+        adj[v].clear()
+    return np.array(order, np.int32)
+
+
+def tree_fma(index_sets: list[list[int]], tree) -> float:
+    """Loop-nest size of a contraction tree: sum over steps of 2^|I_L u I_R| (steps with a rank-0
+    operand cost nothing).  A cost model on index sets; no arithmetic of the method."""
+    sets = [set(s) for s in index_sets]
+    occ: dict[int, int] = {}
+    for s in sets:
+        for i in s:
+            occ[i] = occ.get(i, 0) + 1
+    sub = [{i: 1 for i in s} for s in sets]
+    live = list(sets)
+    fma = 0.0
+    for l, r in zip(tree[0], tree[1]):
+        l, r = int(l), int(r)
+        un = live[l] | live[r]
+        cnt = dict(sub[l])
+        for i, c in sub[r].items():
+            cnt[i] = cnt.get(i, 0) + c
+        cnt = {i: c for i, c in cnt.items() if c < occ[i]}
+        if live[l] and live[r]:
+            fma += float(1 << len(un))
+        live.append({i for i in un if i in cnt}); sub.append(cnt)
+    return fma
+
+
 def sequential_tree(n_inputs: int, perm=None) -> tuple[np.ndarray, np.ndarray]:
     """Left-deep chain ((t0 t1) t2) ... in the given input order (a deliberately
     bad but valid tree, used for tree-independence tests on tiny instances)."""
