@@ -94,7 +94,11 @@ __global__ void __launch_bounds__(NT) gemm_tiled_kernel(int64_t G, int M, int N,
 void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                        const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc, int32_t *Ce, void *Cc,
                        int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, cudaStream_t st) {
-  (void)count_bits;
+  if (ring == RING_U64) {
+    launch_gemm_tiled_u64(batch, G, M, N, K, a_kmajor, Ae, (const uint64_t *)Ac, Be, (const uint64_t *)Bc, Ce, (uint64_t *)Cc,
+                          sA, sB, sC, count_bits, st);
+    return;
+  }
   const int64_t n_cta = (int64_t)((N + BN - 1) / BN) * ((M + BM - 1) / BM) * batch * G;
   dim3 grid((unsigned)n_cta);
   BBTN_RING_DISPATCH(ring, {

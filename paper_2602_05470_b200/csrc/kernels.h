@@ -39,6 +39,11 @@ void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmaj
                        const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc, int32_t *Ce, void *Cc,
                        int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, cudaStream_t st);
 
+// K3 v2 for the mod-2^64 ring (gemm_tiled.cu): chunked two-pass kernel, 4 integer instructions per FMA.
+void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
+                           const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
+                           int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, cudaStream_t st);
+
 // K4: (E[b], c[b]) = offset[b] (.) root[b]; canonicalise; convert to reported units.
 //   root_e == nullptr: the network is all scalars.  root_stride 0: root is leaf-invariant.
 void launch_finalize(int kind, int64_t B, const int32_t *root_e, const void *root_c, int64_t root_stride,
