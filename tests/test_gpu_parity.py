@@ -49,7 +49,8 @@ def test_gemm_matches_oracle(bb, oracle, B, M, N, K, seed, frac, wide):
     Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed, neg_inf_frac=frac, wide_counts=wide)
     want_e, want_c = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
-    for bits in (64, 32) if not wide else (64,):
+    # 64: full 64x64 multiply; 32: 32-bit operands, 64-bit accumulators; 3: counts <= 4, 32-bit accumulators
+    for bits in (64, 32, 3) if not wide else (64,):
         Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
         got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
         assert (got_e == want_e).all()
@@ -69,12 +70,14 @@ def test_gemm_large_sampled_rows(bb, oracle):
     n, B = 1024, 2
     Ae, Ac, Be, Bc = I.gemm_operands(B, n, n, n, seed=21)
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
-    Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc)
-    got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
     rows = (I.splitmix64(5, 16, 20) % np.uint64(n)).astype(np.int64)
-    for b in range(B):
-        we, wc = _oracle_gemm(oracle, Ae[b:b + 1, rows], Ac[b:b + 1, rows], Be[b:b + 1], Bc[b:b + 1])
-        assert (got_e[b, rows] == we[0]).all() and (got_c[b, rows] == wc[0]).all()
+    want = [_oracle_gemm(oracle, Ae[b:b + 1, rows], Ac[b:b + 1, rows], Be[b:b + 1], Bc[b:b + 1]) for b in range(B)]
+    for bits in (64, 32, 3):                # 3 is the launch configuration bench.py times
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+        got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
+        for b in range(B):
+            we, wc = want[b]
+            assert (got_e[b, rows] == we[0]).all() and (got_c[b, rows] == wc[0]).all()
 
 
 # ---- K2 alone -------------------------------------------------------------------------
