@@ -208,10 +208,12 @@ int bbtn_permute_batched(int32_t rank, const int32_t *perm, int64_t batch,
 
 /* Integer-pipe microbenchmarks (register-only, no memory traffic) that define the ALU roofline of
  * K3.  which: 0 = IADD3 chain, 1 = IMNMX chain, 2 = fused add-max
- * (VIADDMNMX), 3 = IMAD chain, 4 = mixed IADD3+IMAD (both pipes), 5 = the per-FMA op mix of the
- * counting GEMM (energy pass + count pass, u64 counts), 6 = same with 32-bit-operand counts.
+ * (VIADDMNMX), 3 = IMAD chain, 4 = mixed 3-operand IADD3+IMAD (both pipes), 7 / 8 = mixed two-operand
+ * IADD:IMAD at 1:1 / 2:1, 9 / 10 = the instruction stream of K3's inner loop (fused add-max, add, tie
+ * compare, predicated IMAD, operand LDS.128 from a broadcast table) at 2 / 4+ warps per SM sub-partition;
+ * 5, 6 = earlier op-mix kernels (kept for comparison, not used by bench.py).
  * Runs `iters` unrolled rounds on every SM; returns elapsed milliseconds (CUDA events) and the
- * number of lane-operations (which <= 4) or tropical FMAs (which >= 5) executed. */
+ * number of lane-operations (which <= 4, 7, 8) or tropical FMAs (5, 6, 9, 10) executed. */
 int bbtn_int32_microbench(int32_t which, int32_t iters, double *milliseconds, double *operations,
                           void *cuda_stream);
 

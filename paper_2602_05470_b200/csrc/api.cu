@@ -332,7 +332,7 @@ int bbtn_permute_batched(int32_t rank, const int32_t *perm, int64_t batch, const
 }
 
 int bbtn_int32_microbench(int32_t which, int32_t iters, double *ms, double *ops, void *stream) {
-  if (which < 0 || which > 6 || iters < 1 || !ms || !ops) return fail(nullptr, BBTN_EINVAL, "bad microbench arguments");
+  if (which < 0 || which > 10 || iters < 1 || !ms || !ops) return fail(nullptr, BBTN_EINVAL, "bad microbench arguments");
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device");
   int rc = run_microbench(which, iters, ms, ops, (cudaStream_t)stream);
   if (rc) return fail(nullptr, BBTN_ECUDA, "microbenchmark failed");

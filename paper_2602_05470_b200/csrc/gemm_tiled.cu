@@ -13,26 +13,28 @@
 // ~16 for a literal transcription of (+)/(.).  Pass 2 only ever compares against the final maximum
 // of everything seen so far, so the result is exactly the definition (bit-exact, order-free).
 //
-// CTA tile 128x128, 256 threads, 8x8 outputs per thread (2x2 blocks of 4x4 so that every operand
-// fetch is one LDS.128), BK = 16, three cp.async stages, one barrier per chunk.  Operands stay in
-// their global layout in shared memory (row-major A is consumed four k at a time), so interior tiles
-// move with 16-byte cp.async only; ragged or unaligned tiles take a guarded scalar fill that writes
-// the zero element (-inf, 0) outside the matrix.
+// Pass 1 needs only the ALU pipe and pass 2 is FMA-pipe heavy, so pass 1 of chunk c+1 is interleaved
+// (same instruction stream, independent registers) with pass 2 of chunk c: both pipes stay busy.
+//
+// CTA tile 128x128 (128x64 with 64-bit accumulators), 256 threads, 8x8 (8x4) outputs per thread in
+// 4x4 blocks so that every operand fetch is one LDS.128, BK = 16, one barrier per chunk.  Interior
+// tiles arrive by 16-byte cp.async in their global layout (raw stages); a short cooperative step
+// rewrites each chunk k-major with the counts narrowed to 32 bits when the caller's count_bits
+// allows (converted stages).  Ragged or unaligned tiles take a guarded scalar fill that writes the
+// zero element (-inf, 0) outside the matrix.
 #include "kernels.h"
 #include "ring.cuh"
+#include <type_traits>
 
 namespace bbtn {
 namespace {
 
-constexpr int BM = 128, BN = 128, BK = 16, NT = 256, STAGES = 3;
+constexpr int BM = 128, BK = 16, NT = 256;
+constexpr int RAW_STAGES = 2, CONV_STAGES = 3;
 constexpr int AE_LD = BK + 4;            // row-major A energies: [BM][AE_LD] int32 (row stride 80 B)
 constexpr int AC_LD = BK + 2;            // row-major A counts:   [BM][AC_LD] uint64 (row stride 144 B)
 constexpr int AE_BYTES = BM * AE_LD * 4; // k-major A needs BK*BM*4 <= this
 constexpr int AC_BYTES = BM * AC_LD * 8;
-constexpr int BE_BYTES = BK * BN * 4;
-constexpr int BC_BYTES = BK * BN * 8;
-constexpr int STAGE_BYTES = AE_BYTES + AC_BYTES + BE_BYTES + BC_BYTES;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES;
 
 enum Mode : int { ACC32 = 0, ACC64N = 1, WIDE = 2 };
 // ACC32 : operand counts < 2^16 and K * max product < 2^32: 32-bit accumulators, one IMAD per FMA
@@ -48,10 +50,6 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// 16-byte granule g (two counts) of a B-count row is stored at g ^ ((g >> 3) & 1): the eight lanes of a
-// quarter warp read granules 2*tx (+1), which would otherwise collide pairwise on the banks.
-__device__ __forceinline__ int bc_swz(int g) { return g ^ ((g >> 3) & 1); }
 
 // pass 2 of one FMA: if (ea + eb == E) c += ca * cb
 template <int MODE>
@@ -83,10 +81,15 @@ struct GemmArgs {
   int vecA, vecB, vecC;     // 16-byte paths allowed (alignment of pointers, strides and leading dimensions)
 };
 
-template <int NCB> struct Tile {
+// shared memory: RAW_STAGES raw stages (cp.async targets, operands in their global layout, uint64 counts)
+// followed by CONV_STAGES converted stages (k-major, counts narrowed to CT) that the FMA loops read.
+template <int NCB, class CT> struct Tile {
   static constexpr int BNt = 64 * NCB;
   static constexpr int BE = BK * BNt * 4, BC = BK * BNt * 8;
-  static constexpr int STAGE = AE_BYTES + AC_BYTES + BE + BC;
+  static constexpr int RAW = AE_BYTES + AC_BYTES + BE + BC;
+  static constexpr int CAE = BK * BM * 4, CAC = BK * BM * (int)sizeof(CT), CBE = BK * BNt * 4, CBC = BK * BNt * (int)sizeof(CT);
+  static constexpr int CONV = CAE + CAC + CBE + CBC;
+  static constexpr int SMEM = RAW_STAGES * RAW + CONV_STAGES * CONV;
 };
 
 // ---- global -> shared for one chunk (k0 .. k0+BK) of one operand ------------------------------
@@ -137,10 +140,9 @@ __device__ __forceinline__ void fill_A(const GemmArgs &p, const int32_t *__restr
   }
 }
 
-template <int NCB>
+template <int BNt>
 __device__ __forceinline__ void fill_B(const GemmArgs &p, const int32_t *__restrict__ be, const uint64_t *__restrict__ bc,
                                        int n0, int k0, unsigned char *sBe, unsigned char *sBc) {
-  constexpr int BNt = Tile<NCB>::BNt;
   const int t = threadIdx.x;
   const bool fast = p.vecB && n0 + BNt <= p.N && k0 + BK <= p.K;
   if (fast) {
@@ -152,7 +154,7 @@ __device__ __forceinline__ void fill_B(const GemmArgs &p, const int32_t *__restr
 #pragma unroll
     for (int idx = t; idx < BK * BNt / 2; idx += NT) {
       const int kk = idx / (BNt / 2), q = idx % (BNt / 2);
-      cp_async16(sBc + (kk * (BNt / 2) + bc_swz(q)) * 16, bc + (int64_t)(k0 + kk) * p.N + n0 + 2 * q);
+      cp_async16(sBc + (kk * (BNt / 2) + q) * 16, bc + (int64_t)(k0 + kk) * p.N + n0 + 2 * q);
     }
   } else {
     int32_t *se = reinterpret_cast<int32_t *>(sBe);
@@ -163,18 +165,87 @@ __device__ __forceinline__ void fill_B(const GemmArgs &p, const int32_t *__restr
       int32_t e = NEG_INF; uint64_t c = 0;
       if (gn < p.N && gk < p.K) { e = be[(int64_t)gk * p.N + gn]; c = bc[(int64_t)gk * p.N + gn]; }
       se[kk * BNt + n] = e;
-      sc[kk * BNt + bc_swz(n >> 1) * 2 + (n & 1)] = c;
+      sc[kk * BNt + n] = c;
     }
   }
 }
 
+// ---- raw stage -> converted stage (k-major, counts narrowed to CT) ---------------------------
+template <class CT> __device__ __forceinline__ void store_pair(CT *dst, uint64_t x, uint64_t y);
+template <> __device__ __forceinline__ void store_pair<uint32_t>(uint32_t *dst, uint64_t x, uint64_t y) {
+  *reinterpret_cast<uint2 *>(dst) = make_uint2((uint32_t)x, (uint32_t)y);
+}
+template <> __device__ __forceinline__ void store_pair<uint64_t>(uint64_t *dst, uint64_t x, uint64_t y) {
+  *reinterpret_cast<ulonglong2 *>(dst) = make_ulonglong2(x, y);
+}
+
+template <bool A_KMAJOR, int NCB, class CT>
+__device__ __forceinline__ void convert_stage(const unsigned char *raw, unsigned char *conv) {
+  using T = Tile<NCB, CT>;
+  constexpr int BNt = T::BNt;
+  const int t = threadIdx.x;
+  const unsigned char *rAe = raw, *rAc = raw + AE_BYTES, *rBe = raw + AE_BYTES + AC_BYTES, *rBc = rBe + T::BE;
+  int32_t *cAe = reinterpret_cast<int32_t *>(conv);
+  CT *cAc = reinterpret_cast<CT *>(conv + T::CAE);
+  int32_t *cBe = reinterpret_cast<int32_t *>(conv + T::CAE + T::CAC);
+  CT *cBc = reinterpret_cast<CT *>(conv + T::CAE + T::CAC + T::CBE);
+  if (A_KMAJOR) {
+#pragma unroll
+    for (int idx = t; idx < BK * BM / 4; idx += NT)
+      *reinterpret_cast<int4 *>(cAe + 4 * idx) = *reinterpret_cast<const int4 *>(rAe + 16 * idx);
+#pragma unroll
+    for (int idx = t; idx < BK * BM / 2; idx += NT) {
+      const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rAc + 16 * idx);
+      store_pair<CT>(cAc + 2 * idx, v.x, v.y);
+    }
+  } else {
+    // transpose: lane = row, so the k-major stores of a warp are contiguous; raw row strides (80 B, 144 B)
+    // keep the 16-byte reads of a quarter warp on distinct banks
+    const int r = t % BM, kb = (t / BM) * (BK / 2);
+#pragma unroll
+    for (int q = 0; q < BK / 8; q++) {
+      const int4 v = *reinterpret_cast<const int4 *>(rAe + (r * AE_LD + kb + 4 * q) * 4);
+      cAe[(kb + 4 * q + 0) * BM + r] = v.x; cAe[(kb + 4 * q + 1) * BM + r] = v.y;
+      cAe[(kb + 4 * q + 2) * BM + r] = v.z; cAe[(kb + 4 * q + 3) * BM + r] = v.w;
+    }
+#pragma unroll
+    for (int q = 0; q < BK / 4; q++) {
+      const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rAc + (r * AC_LD + kb + 2 * q) * 8);
+      cAc[(kb + 2 * q + 0) * BM + r] = (CT)v.x; cAc[(kb + 2 * q + 1) * BM + r] = (CT)v.y;
+    }
+  }
+#pragma unroll
+  for (int idx = t; idx < BK * BNt / 4; idx += NT)
+    *reinterpret_cast<int4 *>(cBe + 4 * idx) = *reinterpret_cast<const int4 *>(rBe + 16 * idx);
+#pragma unroll
+  for (int idx = t; idx < BK * BNt / 2; idx += NT) {
+    const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rBc + 16 * idx);
+    store_pair<CT>(cBc + 2 * idx, v.x, v.y);
+  }
+}
+
+__device__ __forceinline__ void load4(const uint32_t *src, uint64_t *dst) {
+  const uint4 v = *reinterpret_cast<const uint4 *>(src);
+  dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
+}
+__device__ __forceinline__ void load4(const uint64_t *src, uint64_t *dst) {
+  const ulonglong2 v0 = *reinterpret_cast<const ulonglong2 *>(src), v1 = *reinterpret_cast<const ulonglong2 *>(src + 2);
+  dst[0] = v0.x; dst[1] = v0.y; dst[2] = v1.x; dst[3] = v1.y;
+}
+__device__ __forceinline__ void load4(const int32_t *src, int32_t *dst) {
+  const int4 v = *reinterpret_cast<const int4 *>(src);
+  dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
+}
+
 // ---- the kernel -----------------------------------------------------------------------------
 template <int MODE, bool A_KMAJOR, int NCB>
-__global__ void __launch_bounds__(NT, 1) gemm_tiled2_kernel(const GemmArgs p) {
+__global__ void __launch_bounds__(NT, 1) gemm_tiled3_kernel(const GemmArgs p) {
   using Acc = typename AccT<MODE>::T;
-  constexpr int BNt = Tile<NCB>::BNt, STAGE = Tile<NCB>::STAGE, BEb = Tile<NCB>::BE;
-  constexpr int TN = 4 * NCB;
+  using CT = typename std::conditional<MODE == WIDE, uint64_t, uint32_t>::type;
+  using T = Tile<NCB, CT>;
+  constexpr int BNt = T::BNt, TN = 4 * NCB;
   extern __shared__ __align__(16) unsigned char smem[];
+  unsigned char *conv_base = smem + RAW_STAGES * T::RAW;
 
   const int tiles_n = (p.N + BNt - 1) / BNt, tiles_m = (p.M + BM - 1) / BM;
   const int64_t bg = blockIdx.x / (tiles_n * tiles_m);
@@ -188,8 +259,6 @@ __global__ void __launch_bounds__(NT, 1) gemm_tiled2_kernel(const GemmArgs p) {
   // a warp covers 8 tx x 4 ty: A fetches touch 4 distinct 16-byte granules, B fetches 8
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int tx = (w & 1) * 8 + (lane & 7), ty = (w >> 1) * 4 + (lane >> 3);
-  const int sw = (tx >> 2) & 1;                       // granule swizzle of the B counts
-  const int bc_off0 = (2 * tx + sw) * 16, bc_off1 = (2 * tx + 1 - sw) * 16;
 
   int32_t E[8][TN]; Acc C[8][TN];
 #pragma unroll
@@ -198,115 +267,108 @@ __global__ void __launch_bounds__(NT, 1) gemm_tiled2_kernel(const GemmArgs p) {
     for (int j = 0; j < TN; j++) { E[i][j] = NEG_INF; C[i][j] = 0; }
 
   const int n_chunks = (p.K + BK - 1) / BK;
-  auto stage_ptr = [&](int c) { return smem + (c % STAGES) * STAGE; };
-  auto issue = [&](int c) {
+  auto issue = [&](int c) {                          // global -> raw stage c % RAW_STAGES
     if (c < n_chunks) {
-      unsigned char *s = stage_ptr(c);
+      unsigned char *s = smem + (c % RAW_STAGES) * T::RAW;
       fill_A<A_KMAJOR>(p, ae, ac, m0, c * BK, s, s + AE_BYTES);
-      fill_B<NCB>(p, be, bc, n0, c * BK, s + AE_BYTES + AC_BYTES, s + AE_BYTES + AC_BYTES + BEb);
+      fill_B<BNt>(p, be, bc, n0, c * BK, s + AE_BYTES + AC_BYTES, s + AE_BYTES + AC_BYTES + T::BE);
     }
     cp_async_commit();
   };
+  auto convert = [&](int c) {                        // raw stage -> converted stage c % CONV_STAGES
+    if (c < n_chunks)
+      convert_stage<A_KMAJOR, NCB, CT>(smem + (c % RAW_STAGES) * T::RAW, conv_base + (c % CONV_STAGES) * T::CONV);
+  };
+
+  // one unit: pass 2 of chunk `c` on row block rb, interleaved with pass 1 of chunk c+1 on the same rows
+  auto unit = [&](auto do_p1, auto rb_tag, int c) {
+    constexpr bool P1 = decltype(do_p1)::value;
+    constexpr int rb = decltype(rb_tag)::value;
+    const unsigned char *s2 = conv_base + (c % CONV_STAGES) * T::CONV;
+    const unsigned char *s1 = conv_base + ((c + 1) % CONV_STAGES) * T::CONV;
+    const int mrow = rb * 64 + ty * 4;
+    const int32_t *a2e = reinterpret_cast<const int32_t *>(s2) + mrow;
+    const CT *a2c = reinterpret_cast<const CT *>(s2 + T::CAE) + mrow;
+    const int32_t *b2e = reinterpret_cast<const int32_t *>(s2 + T::CAE + T::CAC) + tx * 4;
+    const CT *b2c = reinterpret_cast<const CT *>(s2 + T::CAE + T::CAC + T::CBE) + tx * 4;
+    const int32_t *a1e = reinterpret_cast<const int32_t *>(s1) + mrow;
+    const int32_t *b1e = reinterpret_cast<const int32_t *>(s1 + T::CAE + T::CAC) + tx * 4;
+    int32_t En[4][TN];
+    if (P1) {
 #pragma unroll
-  for (int c = 0; c < STAGES - 1; c++) issue(c);
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) En[i][j] = E[rb * 4 + i][j];
+    }
+#pragma unroll 4
+    for (int kk = 0; kk < BK; kk++) {
+      int32_t a2[4], b2[TN]; uint64_t ca[4], cb[TN];
+      load4(a2e + kk * BM, a2); load4(a2c + kk * BM, ca);
+#pragma unroll
+      for (int q = 0; q < NCB; q++) { load4(b2e + kk * BNt + q * 64, b2 + 4 * q); load4(b2c + kk * BNt + q * 64, cb + 4 * q); }
+      int32_t a1[4], b1[TN];
+      if (P1) {
+        load4(a1e + kk * BM, a1);
+#pragma unroll
+        for (int q = 0; q < NCB; q++) load4(b1e + kk * BNt + q * 64, b1 + 4 * q);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) {
+          if (P1) En[i][j] = __viaddmax_s32(a1[i], b1[j], En[i][j]);
+          tie_fma<MODE>(C[rb * 4 + i][j], a2[i], b2[j], E[rb * 4 + i][j], ca[i], cb[j]);
+        }
+    }
+    if (P1) {                                        // a new maximum drops the count of the old one
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) {
+          if (En[i][j] != E[rb * 4 + i][j]) C[rb * 4 + i][j] = 0;
+          E[rb * 4 + i][j] = En[i][j];
+        }
+    }
+  };
 
-  for (int c = 0; c < n_chunks; c++) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    issue(c + STAGES - 1);
-    const unsigned char *s = stage_ptr(c);
-    const int32_t *sAe = reinterpret_cast<const int32_t *>(s);
-    const uint64_t *sAc = reinterpret_cast<const uint64_t *>(s + AE_BYTES);
-    const int32_t *sBe = reinterpret_cast<const int32_t *>(s + AE_BYTES + AC_BYTES);
-    const unsigned char *sBc = s + AE_BYTES + AC_BYTES + BEb;
-
+  // ---- prologue: chunks 0 and 1 converted, chunk 2 in flight, pass 1 of chunk 0 done ----
+  issue(0); issue(1);
+  cp_async_wait<0>();
+  __syncthreads();
+  convert(0); convert(1);
+  __syncthreads();
+  issue(2);
+  {
+    const unsigned char *s1 = conv_base;
 #pragma unroll
     for (int rb = 0; rb < 2; rb++) {
-      const int mrow = rb * 64 + ty * 4;
-      // ---------------- pass 1: E <- max(E, ea + eb) ----------------
-      int32_t old[4][TN];
+      const int32_t *a1e = reinterpret_cast<const int32_t *>(s1) + rb * 64 + ty * 4;
+      const int32_t *b1e = reinterpret_cast<const int32_t *>(s1 + T::CAE + T::CAC) + tx * 4;
+#pragma unroll 4
+      for (int kk = 0; kk < BK; kk++) {
+        int32_t a1[4], b1[TN];
+        load4(a1e + kk * BM, a1);
 #pragma unroll
-      for (int i = 0; i < 4; i++)
+        for (int q = 0; q < NCB; q++) load4(b1e + kk * BNt + q * 64, b1 + 4 * q);
 #pragma unroll
-        for (int j = 0; j < TN; j++) old[i][j] = E[rb * 4 + i][j];
-#pragma unroll 1
-      for (int k4 = 0; k4 < BK / 4; k4++) {
-        int32_t a[4][4];                               // [kk][i]
-        if (A_KMAJOR) {
+        for (int i = 0; i < 4; i++)
 #pragma unroll
-          for (int kk = 0; kk < 4; kk++) {
-            const int4 v = *reinterpret_cast<const int4 *>(sAe + (k4 * 4 + kk) * BM + mrow);
-            a[kk][0] = v.x; a[kk][1] = v.y; a[kk][2] = v.z; a[kk][3] = v.w;
-          }
-        } else {
-#pragma unroll
-          for (int i = 0; i < 4; i++) {
-            const int4 v = *reinterpret_cast<const int4 *>(sAe + (mrow + i) * AE_LD + k4 * 4);
-            a[0][i] = v.x; a[1][i] = v.y; a[2][i] = v.z; a[3][i] = v.w;
-          }
-        }
-#pragma unroll
-        for (int kk = 0; kk < 4; kk++) {
-          int32_t bv[TN];
-#pragma unroll
-          for (int cb = 0; cb < NCB; cb++) {
-            const int4 v = *reinterpret_cast<const int4 *>(sBe + (k4 * 4 + kk) * BNt + cb * 64 + tx * 4);
-            bv[cb * 4 + 0] = v.x; bv[cb * 4 + 1] = v.y; bv[cb * 4 + 2] = v.z; bv[cb * 4 + 3] = v.w;
-          }
-#pragma unroll
-          for (int i = 0; i < 4; i++)
-#pragma unroll
-            for (int j = 0; j < TN; j++) E[rb * 4 + i][j] = __viaddmax_s32(a[kk][i], bv[j], E[rb * 4 + i][j]);
-        }
+          for (int j = 0; j < TN; j++) E[rb * 4 + i][j] = __viaddmax_s32(a1[i], b1[j], E[rb * 4 + i][j]);
       }
-      // ---------------- reset: a new maximum drops the count of the old one ----------------
-#pragma unroll
-      for (int i = 0; i < 4; i++)
-#pragma unroll
-        for (int j = 0; j < TN; j++)
-          if (E[rb * 4 + i][j] != old[i][j]) C[rb * 4 + i][j] = 0;
-      // ---------------- pass 2: ties add their count products ----------------
-#pragma unroll 1
-      for (int k4 = 0; k4 < BK / 4; k4++) {
-        int32_t a[4][4]; uint64_t ca[4][4];            // [kk][i]
-        if (A_KMAJOR) {
-#pragma unroll
-          for (int kk = 0; kk < 4; kk++) {
-            const int4 v = *reinterpret_cast<const int4 *>(sAe + (k4 * 4 + kk) * BM + mrow);
-            a[kk][0] = v.x; a[kk][1] = v.y; a[kk][2] = v.z; a[kk][3] = v.w;
-            const ulonglong2 c0 = *reinterpret_cast<const ulonglong2 *>(sAc + (k4 * 4 + kk) * BM + mrow);
-            const ulonglong2 c1 = *reinterpret_cast<const ulonglong2 *>(sAc + (k4 * 4 + kk) * BM + mrow + 2);
-            ca[kk][0] = c0.x; ca[kk][1] = c0.y; ca[kk][2] = c1.x; ca[kk][3] = c1.y;
-          }
-        } else {
-#pragma unroll
-          for (int i = 0; i < 4; i++) {
-            const int4 v = *reinterpret_cast<const int4 *>(sAe + (mrow + i) * AE_LD + k4 * 4);
-            a[0][i] = v.x; a[1][i] = v.y; a[2][i] = v.z; a[3][i] = v.w;
-            const ulonglong2 c0 = *reinterpret_cast<const ulonglong2 *>(sAc + (mrow + i) * AC_LD + k4 * 4);
-            const ulonglong2 c1 = *reinterpret_cast<const ulonglong2 *>(sAc + (mrow + i) * AC_LD + k4 * 4 + 2);
-            ca[0][i] = c0.x; ca[1][i] = c0.y; ca[2][i] = c1.x; ca[3][i] = c1.y;
-          }
-        }
-#pragma unroll
-        for (int kk = 0; kk < 4; kk++) {
-          int32_t bv[TN]; uint64_t cbv[TN];
-#pragma unroll
-          for (int cb = 0; cb < NCB; cb++) {
-            const int4 v = *reinterpret_cast<const int4 *>(sBe + (k4 * 4 + kk) * BNt + cb * 64 + tx * 4);
-            bv[cb * 4 + 0] = v.x; bv[cb * 4 + 1] = v.y; bv[cb * 4 + 2] = v.z; bv[cb * 4 + 3] = v.w;
-            const unsigned char *row = sBc + ((k4 * 4 + kk) * (BNt / 2) + cb * 32) * 16;
-            const ulonglong2 c0 = *reinterpret_cast<const ulonglong2 *>(row + bc_off0);
-            const ulonglong2 c1 = *reinterpret_cast<const ulonglong2 *>(row + bc_off1);
-            cbv[cb * 4 + 0] = c0.x; cbv[cb * 4 + 1] = c0.y; cbv[cb * 4 + 2] = c1.x; cbv[cb * 4 + 3] = c1.y;
-          }
-#pragma unroll
-          for (int i = 0; i < 4; i++)
-#pragma unroll
-            for (int j = 0; j < TN; j++)
-              tie_fma<MODE>(C[rb * 4 + i][j], a[kk][i], bv[j], E[rb * 4 + i][j], ca[kk][i], cbv[j]);
-        }
-      }
+    }
+  }
+
+  for (int c = 0; c < n_chunks; c++) {
+    cp_async_wait<0>();
+    __syncthreads();
+    convert(c + 2);
+    issue(c + 3);
+    if (c + 1 < n_chunks) {
+      unit(std::true_type{}, std::integral_constant<int, 0>{}, c);
+      unit(std::true_type{}, std::integral_constant<int, 1>{}, c);
+    } else {
+      unit(std::false_type{}, std::integral_constant<int, 0>{}, c);
+      unit(std::false_type{}, std::integral_constant<int, 1>{}, c);
     }
   }
   cp_async_wait<0>();
@@ -317,12 +379,12 @@ __global__ void __launch_bounds__(NT, 1) gemm_tiled2_kernel(const GemmArgs p) {
     const int gm = m0 + (i >> 2) * 64 + ty * 4 + (i & 3);
     if (gm >= p.M) continue;
 #pragma unroll
-    for (int cb = 0; cb < NCB; cb++) {
-      const int gn = n0 + cb * 64 + tx * 4;
+    for (int q = 0; q < NCB; q++) {
+      const int gn = n0 + q * 64 + tx * 4;
       int32_t e[4]; uint64_t c[4];
 #pragma unroll
       for (int j = 0; j < 4; j++) {
-        e[j] = E[i][cb * 4 + j]; c[j] = (uint64_t)C[i][cb * 4 + j];
+        e[j] = E[i][q * 4 + j]; c[j] = (uint64_t)C[i][q * 4 + j];
         if (e[j] < ZERO_BELOW) { e[j] = NEG_INF; c[j] = 0; }
       }
       const int64_t o = (int64_t)gm * p.N + gn;
@@ -341,15 +403,16 @@ __global__ void __launch_bounds__(NT, 1) gemm_tiled2_kernel(const GemmArgs p) {
 
 template <int MODE, bool A_KMAJOR, int NCB>
 void launch_one(const GemmArgs &a, int64_t batch, cudaStream_t st) {
-  constexpr int BNt = Tile<NCB>::BNt;
-  constexpr int smem = STAGES * Tile<NCB>::STAGE;
+  using CT = typename std::conditional<MODE == WIDE, uint64_t, uint32_t>::type;
+  using T = Tile<NCB, CT>;
+  static_assert(T::SMEM <= 227 * 1024, "shared memory budget");
   static bool configured = false;                      // per instantiation; the attribute is per function
   if (!configured) {
-    cudaFuncSetAttribute(gemm_tiled2_kernel<MODE, A_KMAJOR, NCB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(gemm_tiled3_kernel<MODE, A_KMAJOR, NCB>, cudaFuncAttributeMaxDynamicSharedMemorySize, T::SMEM);
     configured = true;
   }
-  const int64_t n_cta = (int64_t)((a.N + BNt - 1) / BNt) * ((a.M + BM - 1) / BM) * batch * a.G;
-  gemm_tiled2_kernel<MODE, A_KMAJOR, NCB><<<dim3((unsigned)n_cta), NT, smem, st>>>(a);
+  const int64_t n_cta = (int64_t)((a.N + T::BNt - 1) / T::BNt) * ((a.M + BM - 1) / BM) * batch * a.G;
+  gemm_tiled3_kernel<MODE, A_KMAJOR, NCB><<<dim3((unsigned)n_cta), NT, T::SMEM, st>>>(a);
 }
 
 inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }

@@ -78,6 +78,73 @@ __global__ void __launch_bounds__(256) opmix_kernel(int iters, int32_t seed, uin
   if (s == 0x123456789abcdefull) sink[0] = s;
 }
 
+// two-pipe mixes with two-register operands (fewer register-file reads than the 3-operand mix above):
+// WHICH 7: IADD (ALU) : IMAD reg*imm+reg (FMA pipe) = 1:1;  WHICH 8: 2:1.  16 independent chains.
+template <int WHICH>
+__global__ void __launch_bounds__(256) mix2_kernel(int iters, int32_t seed, int32_t *sink) {
+  constexpr int N = 16;
+  int32_t r[N];
+#pragma unroll
+  for (int i = 0; i < N; i++) r[i] = seed * (i + 1) + threadIdx.x;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int u = 0; u < 8; u++) {
+#pragma unroll
+      for (int i = 0; i < N; i++) {
+        const bool fma = WHICH == 7 ? (i & 1) : (i % 3 == 2);
+        if (fma) asm volatile("mad.lo.s32 %0, %0, 5, %1;" : "+r"(r[i]) : "r"(r[i ^ 2]));
+        else asm volatile("add.s32 %0, %0, %1;" : "+r"(r[i]) : "r"(r[i ^ 4]));
+      }
+    }
+  }
+  int32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < N; i++) s ^= r[i];
+  if (s == 0x7fffffff) sink[0] = s;
+}
+
+// WHICH 9/10: the instruction mix of K3's inner loop on registers only (no operand fetch): per tropical
+// FMA one fused add-max into the next-chunk maximum, and add + tie compare + predicated multiply-add
+// against the current maximum (gemm_tiled.cu, pass 1 of chunk c+1 interleaved with pass 2 of chunk c).
+__global__ void __launch_bounds__(256) k3mix_kernel(int iters, int32_t seed, uint32_t *sink) {
+  // operands come from a small shared table read at warp-uniform addresses (one wavefront per LDS.128), so
+  // the loop has K3's instruction stream, operand fetches included, without its shared-memory bandwidth
+  __shared__ __align__(16) int32_t tab[16][36];
+  for (int i = threadIdx.x; i < 16 * 36; i += blockDim.x) tab[i / 36][i % 36] = (i % 36 >= 24) ? 1 + ((seed + i) & 3) : ((seed * 7 + i * 13) & 63);
+  __syncthreads();
+  int32_t En[4][8], E[4][8]; uint32_t C[4][8];
+#pragma unroll
+  for (int i = 0; i < 4; i++)
+#pragma unroll
+    for (int j = 0; j < 8; j++) { En[i][j] = NEG_INF; E[i][j] = 64 + (int)((threadIdx.x + i + j) & 7); C[i][j] = 0; }
+  for (int it = 0; it < iters; it++) {
+#pragma unroll 4
+    for (int kk = 0; kk < 16; kk++) {
+      int32_t v[36];
+#pragma unroll
+      for (int q = 0; q < 9; q++) {
+        const int4 x = *reinterpret_cast<const int4 *>(&tab[kk][4 * q]);
+        v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
+      }
+      // v[0..3] a1, v[4..11] b1, v[12..15] a2, v[16..23] b2, v[24..27] ca, v[28..35] cb
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+          En[i][j] = __viaddmax_s32(v[i], v[4 + j], En[i][j]);
+          asm("{\n\t.reg .pred p;\n\t.reg .s32 s;\n\tadd.s32 s, %1, %2;\n\tsetp.eq.s32 p, s, %3;\n\t@p mad.lo.u32 %0, %4, %5, %0;\n\t}"
+              : "+r"(C[i][j]) : "r"(v[12 + i]), "r"(v[16 + j]), "r"(E[i][j]), "r"(v[24 + i]), "r"(v[28 + j]));
+        }
+    }
+  }
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < 4; i++)
+#pragma unroll
+    for (int j = 0; j < 8; j++) s += C[i][j] + (uint32_t)En[i][j];
+  if (s == 0x12345678u) sink[0] = s;
+}
+
 }  // namespace
 
 int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t st) {
@@ -85,9 +152,14 @@ int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t s
   if (cudaMalloc(&sink, 64) != cudaSuccess) return 3;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
-  const int grid = 148 * 8, block = 256;
+  int grid = 148 * 8, block = 256;
+  if (which == 9) { grid = 148; block = 256; }          // 2 warps per SM sub-partition, as K3 runs
+  if (which == 10) { grid = 148 * 4; block = 256; }     // same mix, 4+ warps per sub-partition
   auto launch = [&](int n) {
     switch (which) {
+      case 7: mix2_kernel<7><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 8: mix2_kernel<8><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 9: case 10: k3mix_kernel<<<grid, block, 0, st>>>(n, 12345, (uint32_t *)sink); break;
       case 0: pipe_kernel<0><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
       case 1: pipe_kernel<1><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
       case 2: pipe_kernel<2><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
@@ -112,6 +184,10 @@ int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t s
   if (which <= 4) {
     double per_round = CH;                     // one instruction per chain per round
     *ops = threads * (double)iters * UNROLL * per_round;
+  } else if (which == 7 || which == 8) {
+    *ops = threads * (double)iters * 8.0 * 16.0;   // lane-instructions
+  } else if (which == 9 || which == 10) {
+    *ops = threads * (double)iters * 16.0 * 32.0;   // tropical FMAs (4 instructions each + 9 LDS.128 per 32)
   } else {
     *ops = threads * (double)iters * 64.0;     // tropical FMAs
   }
