@@ -95,7 +95,7 @@ template <> struct Vec4<uint32_t> {
 };
 
 template <class CT>
-__global__ void __launch_bounds__(256, 3) permute_vec_kernel(PermVecArgs p, const int32_t *__restrict__ src_e,
+__global__ void __launch_bounds__(256, 2) permute_vec_kernel(PermVecArgs p, const int32_t *__restrict__ src_e,
                                                           const CT *__restrict__ src_c, int32_t *__restrict__ dst_e,
                                                           CT *__restrict__ dst_c) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -201,7 +201,7 @@ bool launch_permute_vec(int rank, const int32_t *perm, const int *inv, int64_t b
   p.n_outer = 0;
   for (int s = 0; s < rank; s++) if (!in_tile[s]) { p.outer_src[p.n_outer] = 1u << s; p.outer_dst[p.n_outer] = 1u << inv[s]; p.n_outer++; }
   const int64_t n_tiles = ((int64_t)1 << p.n_outer) * batch;
-  const int64_t cap = 148 * 3;
+  const int64_t cap = 148 * 8;
   const int grid = (int)(n_tiles < cap ? n_tiles : cap);
   const size_t csz = ring == 0 ? 8 : 4;
   const size_t smem = ((size_t)1 << nt) * (csz + 4);
