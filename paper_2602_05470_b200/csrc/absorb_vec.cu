@@ -1,0 +1,170 @@
+// absorb_vec.cu -- K3, streaming form, vectorised (sm_100a).
+//
+//   C[b][o] = (+)_k A[b][fa(o) + ka(k)] (.) B[b][fb(o) + kb(k)]      (PAPER.md:51 Eq. 2 pairwise, :57)
+//
+// This is the HBM-bound shape of the pairwise contraction: a large tensor A absorbs a small one (a bond
+// or vertex tensor, or a narrow intermediate) and at most a few indices are summed, so there is ~1/12
+// tropical FMA per byte and the kernel has to move 12 B per element at memory speed.  The planner lays
+// the output out as "A's surviving bits in A's order, then B's new bits", so runs of consecutive outputs
+// are runs of consecutive (or regularly interleaved) elements of A:
+//   * a thread owns 4 consecutive outputs: 16-byte loads of A, 16-byte stores of C;
+//   * fa/fb are sums of per-bit offsets (all dims are 2), split into a per-thread part (bits 2..11,
+//     computed once), and a per-tile part (bits >= 12, a short loop per 4096 outputs);
+//   * the three ways the lowest two output bits can sit in A are compile-time cases (LP): both are A's
+//     bits 0,1 (FAR: the summed index lies higher), or the summed index is A's bit 0 (K0) or bit 1 (K1),
+//     in which case one 8-element read holds both k for all 4 outputs.
+// Anything else (rank < 4, several summed low bits, unaligned arena offsets) takes the scalar kernel.
+#include "kernels.h"
+#include "ring.cuh"
+
+namespace bbtn {
+namespace {
+
+enum LowPattern : int { LP_FAR = 0, LP_K0 = 1, LP_K1 = 2 };
+
+struct AbsorbVecArgs {
+  int rO, nK, tb;                 // output rank, summed bits, tile bits (<= 12)
+  uint32_t addA[28], addB[28];    // per output bit
+  uint32_t kA[8], kB[8];          // per summed bit
+  int64_t sA, sB, sC, n_tiles;    // batch strides (elements), tiles over all batch entries
+};
+
+template <class CT> struct V4;
+template <> struct V4<uint64_t> {
+  uint64_t v[4];
+  __device__ __forceinline__ void load(const uint64_t *p) {
+    const ulonglong2 a = *reinterpret_cast<const ulonglong2 *>(p), b = *reinterpret_cast<const ulonglong2 *>(p + 2);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  }
+  __device__ __forceinline__ void store(uint64_t *p) const {
+    *reinterpret_cast<ulonglong2 *>(p) = make_ulonglong2(v[0], v[1]);
+    *reinterpret_cast<ulonglong2 *>(p + 2) = make_ulonglong2(v[2], v[3]);
+  }
+};
+template <> struct V4<uint32_t> {
+  uint32_t v[4];
+  __device__ __forceinline__ void load(const uint32_t *p) {
+    const uint4 a = *reinterpret_cast<const uint4 *>(p);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w;
+  }
+  __device__ __forceinline__ void store(uint32_t *p) const { *reinterpret_cast<uint4 *>(p) = make_uint4(v[0], v[1], v[2], v[3]); }
+};
+
+__device__ __forceinline__ void load_e4(const int32_t *p, int32_t *d) {
+  const int4 a = *reinterpret_cast<const int4 *>(p);
+  d[0] = a.x; d[1] = a.y; d[2] = a.z; d[3] = a.w;
+}
+
+template <class R, int LP>
+__global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const int32_t *__restrict__ Ae,
+                                                         const typename R::T *__restrict__ Ac,
+                                                         const int32_t *__restrict__ Be, const typename R::T *__restrict__ Bc,
+                                                         int32_t *__restrict__ Ce, typename R::T *__restrict__ Cc) {
+  using CT = typename R::T;
+  constexpr int VPT = 4;                                    // vectors per thread in a full 4096-output tile
+  const int nvec = 1 << (p.tb - 2);
+  // per-thread part of the addresses: output bits 2 .. tb-1
+  uint32_t ta[VPT], tbo[VPT];
+#pragma unroll
+  for (int j = 0; j < VPT; j++) {
+    const uint32_t o = (uint32_t)(threadIdx.x + 256 * j) << 2;
+    uint32_t a = 0, b = 0;
+    for (int q = 2; q < p.tb; q++) if ((o >> q) & 1u) { a += p.addA[q]; b += p.addB[q]; }
+    ta[j] = a; tbo[j] = b;
+  }
+  const uint32_t ub1 = p.addB[0], ub2 = p.addB[1];
+  const int tiles_per_entry_lg = p.rO - p.tb;
+  const int n_k = 1 << p.nK;
+
+  for (int64_t t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
+    const int64_t b = t >> tiles_per_entry_lg;
+    const uint32_t hi = (uint32_t)(t - (b << tiles_per_entry_lg));
+    uint32_t a_hi = 0, b_hi = 0;
+    for (int q = 0; q < tiles_per_entry_lg; q++) if ((hi >> q) & 1u) { a_hi += p.addA[p.tb + q]; b_hi += p.addB[p.tb + q]; }
+    const int32_t *ae = Ae + b * p.sA + a_hi; const CT *ac = Ac + b * p.sA + a_hi;
+    const int32_t *be = Be + b * p.sB + b_hi; const CT *bc = Bc + b * p.sB + b_hi;
+    int32_t *ce = Ce + b * p.sC + ((int64_t)hi << p.tb); CT *cc = Cc + b * p.sC + ((int64_t)hi << p.tb);
+#pragma unroll
+    for (int j = 0; j < VPT; j++) {
+      const int v = threadIdx.x + 256 * j;
+      if (v >= nvec) break;
+      int32_t acc_e[4]; CT acc_c[4];
+#pragma unroll
+      for (int u = 0; u < 4; u++) { acc_e[u] = NEG_INF; acc_c[u] = 0; }
+      if (LP == LP_FAR) {
+        for (int k = 0; k < n_k; k++) {
+          uint32_t ka = 0, kb = 0;
+          for (int q = 0; q < p.nK; q++) if ((k >> q) & 1) { ka += p.kA[q]; kb += p.kB[q]; }
+          int32_t e4[4]; V4<CT> c4;
+          load_e4(ae + ta[j] + ka, e4); c4.load(ac + ta[j] + ka);
+#pragma unroll
+          for (int u = 0; u < 4; u++) {
+            const uint32_t ib = tbo[j] + kb + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+            oplus<R>(acc_e[u], acc_c[u], e4[u] + be[ib], R::mul(c4.v[u], bc[ib]));
+          }
+        }
+      } else {
+        // nK == 1 and the summed index is A's bit 0 (K0) or bit 1 (K1): 8 consecutive elements of A
+        int32_t e8[8]; V4<CT> c8[2];
+        load_e4(ae + ta[j], e8); load_e4(ae + ta[j] + 4, e8 + 4);
+        c8[0].load(ac + ta[j]); c8[1].load(ac + ta[j] + 4);
+#pragma unroll
+        for (int u = 0; u < 4; u++)
+#pragma unroll
+          for (int k = 0; k < 2; k++) {
+            // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
+            const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
+            const uint32_t ib = tbo[j] + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+            oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], bc[ib]));
+          }
+      }
+      V4<CT> oc;
+#pragma unroll
+      for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[u], acc_c[u]); oc.v[u] = acc_c[u]; }
+      *reinterpret_cast<int4 *>(ce + 4 * v) = make_int4(acc_e[0], acc_e[1], acc_e[2], acc_e[3]);
+      oc.store(cc + 4 * v);
+    }
+  }
+}
+
+inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+}  // namespace
+
+// Returns false when the step does not fit the vectorised form (the caller then runs the scalar kernel).
+bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
+                       int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
+  if (s.rO < 4 || s.nK > 3 || s.rA < 3) return false;
+  if (!al16(Ae) || !al16(Ac) || !al16(Ce) || !al16(Cc)) return false;
+  int lp;
+  if (s.addA[0] == 1u && s.addA[1] == 2u) {
+    lp = LP_FAR;
+    for (int q = 0; q < s.nK; q++) if (s.kA[q] < 4u) return false;
+  } else if (s.nK == 1 && s.kA[0] == 1u && s.addA[0] == 2u && s.addA[1] == 4u) lp = LP_K0;
+  else if (s.nK == 1 && s.kA[0] == 2u && s.addA[0] == 1u && s.addA[1] == 4u) lp = LP_K1;
+  else return false;
+  AbsorbVecArgs p;
+  p.rO = s.rO; p.nK = s.nK; p.tb = s.rO < 12 ? s.rO : 12;
+  for (int i = 0; i < 28; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
+  for (int i = 0; i < 8; i++) { p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
+  // the 16-byte reads of A must stay 4-element aligned: every offset that can be added is a multiple of 4
+  for (int q = 2; q < s.rO; q++) if (p.addA[q] & 3u) return false;
+  p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
+  p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
+  p.sC = (int64_t)1 << s.rO;
+  p.n_tiles = nb << (s.rO - p.tb);
+  const int64_t cap = 148 * 8;
+  const int grid = (int)(p.n_tiles < cap ? p.n_tiles : cap);
+  BBTN_RING_DISPATCH(ring, {
+    using CT = typename R::T;
+    if (lp == LP_FAR)
+      absorb_vec_kernel<R, LP_FAR><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
+    else if (lp == LP_K0)
+      absorb_vec_kernel<R, LP_K0><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
+    else
+      absorb_vec_kernel<R, LP_K1><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
+  });
+  return true;
+}
+
+}  // namespace bbtn

@@ -216,6 +216,7 @@ void launch_construct(int kind, const InputRec *d_inputs, const int32_t *d_list_
 
 void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
+  if (launch_absorb_vec(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st)) return;   // 16-byte form (absorb_vec.cu)
   AbsorbArgs p;
   p.rO = s.rO; p.nK = s.nK;
   for (int i = 0; i < 28; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }

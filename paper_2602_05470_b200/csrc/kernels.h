@@ -28,6 +28,8 @@ void launch_permute(int rank, const int32_t *perm, int64_t batch, const int32_t 
 // K3 (streaming form, permutation fused into the operand addressing) and its long-reduction form.
 void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st);
+bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
+                       int32_t *Ce, void *Cc, int ring, cudaStream_t st);   // false: shape not covered, use launch_absorb's scalar kernel
 void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st);
 
