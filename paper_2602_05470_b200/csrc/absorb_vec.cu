@@ -16,6 +16,7 @@
 // Anything else (rank < 4, several summed low bits, unaligned arena offsets) takes the scalar kernel.
 #include "kernels.h"
 #include "ring.cuh"
+#include <cstdio>
 
 namespace bbtn {
 namespace {
@@ -143,6 +144,9 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
   } else if (s.nK == 1 && s.kA[0] == 1u && s.addA[0] == 2u && s.addA[1] == 4u) lp = LP_K0;
   else if (s.nK == 1 && s.kA[0] == 2u && s.addA[0] == 1u && s.addA[1] == 4u) lp = LP_K1;
   else return false;
+#ifdef BBTN_TRACE_LP
+  fprintf(stderr, "LP %d ring %d nK %d rO %d\n", lp, ring, s.nK, s.rO);
+#endif
   AbsorbVecArgs p;
   p.rO = s.rO; p.nK = s.nK; p.tb = s.rO < 12 ? s.rO : 12;
   for (int i = 0; i < 28; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
