@@ -8,6 +8,8 @@ Workload = BASELINE.json configs[3], the configuration the metric ("counting-tro
 of int32 CUDA-core peak") is quoted on.  ONE STEP is one pass of the whole hot path over one batch:
   (a) raw batched counting-tropical GEMM (K3 tiled): M=N=K=1024, batch 64 per GPU, energies uniform
       in [-64,64], counts uniform in {1..4} (so the caller promises count_bits = 3);
+      followed by K2 on its result: the 2^26-element C planes are bit-permuted (seeded random permutation
+      of the 26 index bits) into the order a following contraction would want;
   (b) the 5x5x5 open +-J cube, 2^f leaves (f = 8 spins of the central layer, all assignments) per
       GPU: K5 region bounds for every leaf, then K1 construct -> K2 permute / K3 GEMM (tiled and
       streaming forms, chosen per tree node by the planner) -> K4 finalize.
@@ -176,7 +178,7 @@ def run_reference(args):
 
 def _config(args):
     return {"workload": (f"BASELINE configs[3]: raw batched counting-tropical GEMM M=N=K={GEMM_N} batch {GEMM_BATCH} "
-                         f"(energies U[-64,64], counts U{{1..4}}) + {CUBE_L}x{CUBE_L}x{CUBE_L} open +-J cube, "
+                         f"(energies U[-64,64], counts U{{1..4}}) + K2 bit-permutation of its 2^26-element result + {CUBE_L}x{CUBE_L}x{CUBE_L} open +-J cube, "
                          f"f={CUBE_F} fixed spins of the central layer, all {1 << CUBE_F} leaves, per GPU"),
             "gemm": {"M": GEMM_N, "N": GEMM_N, "K": GEMM_N, "batch_per_gpu": GEMM_BATCH, "count_bits": 3},
             "cube": {"L": CUBE_L, "n_fixed": CUBE_F, "leaves_per_gpu": 1 << CUBE_F},
@@ -217,6 +219,11 @@ def run_ours(args):
     hCe = torch.empty((gb, n, n), dtype=torch.int32).pin_memory()
     hCc = torch.empty((gb, n, n), dtype=torch.int64).pin_memory()
     gemm_fma = float(gb) * n * n * n
+    perm_rank = int(np.log2(gb * n * n))
+    perm = I.random_bit_permutation(perm_rank, seed)
+    dPe = torch.empty((1, gb * n * n), dtype=torch.int32, device="cuda")
+    dPc = torch.empty((1, gb * n * n), dtype=torch.int64, device="cuda")
+    perm_bytes = 24.0 * gb * n * n
 
     # ---- inputs (b): cube
     inst, fixed, assign, roffs, rverts = cube_problem(seed)
@@ -231,22 +238,28 @@ def run_ours(args):
     d_count = torch.empty(B, dtype=torch.int64, device="cuda")
     d_bound = torch.empty(B, dtype=torch.int32, device="cuda")
     step_fma = gemm_fma + cube_fma
-    launches_per_step = 1 + 2 + info["n_kernel_launches"]
+    launches_per_step = 1 + 1 + 2 + info["n_kernel_launches"]
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    gemm_ev = []
+    gemm_ev, perm_ev, cube_ev = [], [], []
 
     def step_device(record=False):
         with torch.cuda.stream(stream):
             h_dev.region_bound_device(roffs, rverts, fixed, d_assign, d_bound, stream=sp)
+            if record:
+                c0, c1, a, b, q = ev(), ev(), ev(), ev(), ev()
+                c0.record(stream)
             h_dev.contract_batch_device(fixed, d_assign, d_energy, d_count, stream=sp)
             if record:
-                a, b = ev(), ev()
+                c1.record(stream)
                 a.record(stream)
             bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=3, stream=sp)
             if record:
                 b.record(stream)
-                gemm_ev.append((a, b))
+            bb.permute_batched(perm, dCe.view(1, -1), dCc.view(1, -1), dPe, dPc, stream=sp)
+            if record:
+                q.record(stream)
+                gemm_ev.append((a, b)); perm_ev.append((b, q)); cube_ev.append((c0, c1))
 
     def step_host():
         bound = h_host.region_bound(roffs, rverts, fixed, assign, stream=sp)
@@ -279,6 +292,8 @@ def run_ours(args):
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     ms = e0.elapsed_time(e1)
     gemm_ms = float(np.mean([a.elapsed_time(b) for a, b in gemm_ev]))
+    perm_ms = float(np.mean([a.elapsed_time(b) for a, b in perm_ev]))
+    cube_ms = float(np.mean([a.elapsed_time(b) for a, b in cube_ev]))
     energy_dev = d_energy.cpu().numpy().copy(); count_dev = d_count.cpu().numpy().copy()
 
     # ---- end-to-end timing through the host-pointer calls
@@ -330,6 +345,15 @@ def run_ours(args):
                 "frac_of_alu_pipe_peak_2ops": 2 * gemm_gfma / alu_peak,
                 "microbench_Gops": mb, "share_of_step": gemm_ms * args.steps / ms,
                 "hbm_peak_gbs": hbm_peak, "hbm_peak_kind": peak_kind}
+    # the HBM-bound kernels of the same step (rank 0's timings), against the measured copy bandwidth
+    roofline_hbm = [
+        {"kernel": "permute_vec_kernel (K2)", "bound": "hbm", "achieved": perm_bytes / perm_ms / 1e6, "peak": hbm_peak,
+         "unit": "GB/s", "frac": perm_bytes / perm_ms / 1e6 / hbm_peak, "ms_per_launch": perm_ms,
+         "algorithmic_bytes": perm_bytes, "what": f"2^{perm_rank} elements x 24 B (12 read + 12 written), seeded random bit permutation"},
+        {"kernel": "absorb_vec_kernel + K1/K4 (S1-S4 of the cube, one CUDA-graph replay)", "bound": "hbm",
+         "achieved": info["bytes_per_call"] / cube_ms / 1e6, "peak": hbm_peak, "unit": "GB/s",
+         "frac": info["bytes_per_call"] / cube_ms / 1e6 / hbm_peak, "ms_per_call": cube_ms,
+         "algorithmic_bytes": info["bytes_per_call"], "what": "planner byte total: 12 B per element read or written by every tree node"}]
 
     # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
     cpu = None
@@ -343,9 +367,10 @@ def run_ours(args):
             "dtype": "int32 energy + uint64 count", "data": "synthetic", "config": _config(args),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "Gop/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "note": "host-pointer calls: region_bound + contract_batch + tropical_gemm_batched_host (K2 has no host-pointer form and is left out)",
                     "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches_per_step * args.steps),
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "roofline_hbm_kernels": roofline_hbm, "cpu_baseline": cpu,
             "plan": {k: info[k] for k in ("n_nodes", "n_variant_nodes", "max_rank", "n_gemm_tiled", "n_absorb", "n_permute",
                                           "n_trace", "n_kernel_launches", "workspace_bytes")},
             "fma_per_step": {"gemm": gemm_fma, "cube": cube_fma},

@@ -1,0 +1,122 @@
+"""time-to-exact (E0, count) on the BASELINE.json lattice configurations, through the C ABI only.
+
+    python -m paper_2602_05470_b200.time_to_solve [--configs 1 2 3 4b 5] [--king-sizes 16 20 24 28] [--repeat 5]
+
+Prints one JSON line per solve: instance, fixed set / batch, contraction width, planner FMAs and bytes,
+milliseconds (warm plan; plan build and first-call allocation excluded and reported separately), result.
+The second half of BASELINE.json's metric ("time-to-exact E0+count"); the first half is bench.py.
+No oracle here: correctness of the same instances is checked by tests/ (goldens written by the oracle).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import time
+
+import numpy as np
+
+from . import binding as bb
+from . import instances as I
+
+MASK64 = (1 << 64) - 1
+
+
+def _sync():
+    import torch
+    torch.cuda.synchronize()
+
+
+def _timed(fn, repeat):
+    t0 = time.perf_counter(); out = fn(); _sync(); first = (time.perf_counter() - t0) * 1e3
+    ts = []
+    for _ in range(repeat):
+        t0 = time.perf_counter(); out = fn(); _sync(); ts.append((time.perf_counter() - t0) * 1e3)
+    return out, first, float(np.median(ts)), float(np.min(ts))
+
+
+def _leaf_sum(kind, e, c):
+    best = int(e.min()) if kind == "ising" else int(e.max())
+    return best, sum(int(x) for x in c[e == best]) & MASK64
+
+
+def solve_unbranched(name, inst, tree=None, repeat=5, cap=1 << 28):
+    h = bb.Handle(inst, tree=tree, max_elements_per_leaf=cap)
+    info = h.plan_query(None, 1)
+    (e, c), first, med, mn = _timed(lambda: h.contract_batch(), repeat)
+    h.close()
+    return {"instance": name, "mode": "unbranched", "n_vertices": inst.n_vertices, "n_edges": inst.n_edges,
+            "width": info["max_rank"], "kernel_launches": info["n_kernel_launches"], "fma": info["fma_variant"] + info["fma_invariant"],
+            "first_call_ms": first, "ms_median": med, "ms_min": mn, "energy": int(e[0]), "count_mod_2_64": int(c[0])}
+
+
+def solve_branched(name, inst, fixed, tree, repeat=5, cap=1 << 26):
+    assign = I.all_assignments(len(fixed))
+    B = len(assign)
+    h = bb.Handle(inst, tree=tree, max_elements_per_leaf=cap)
+    info = h.plan_query(fixed, B)
+    (e, c), first, med, mn = _timed(lambda: h.contract_batch(fixed, assign), repeat)
+    h.close()
+    best, cnt = _leaf_sum(inst.kind, e, c)
+    fma = info["fma_variant"] * B + info["fma_invariant"]
+    return {"instance": name, "mode": f"all 2^{len(fixed)} leaves of one fixed set, one bbtn_contract_batch call (host pointers)",
+            "n_vertices": inst.n_vertices, "n_edges": inst.n_edges, "n_fixed": len(fixed), "leaves": B, "width": info["max_rank"],
+            "nodes": info["n_nodes"], "variant_nodes": info["n_variant_nodes"], "fma": fma, "bytes": info["bytes_per_call"],
+            "workspace_bytes": info["workspace_bytes"], "first_call_ms": first, "ms_median": med, "ms_min": mn,
+            "gfma_per_s": fma / med / 1e6, "algorithmic_gb_per_s": info["bytes_per_call"] / med / 1e6,
+            "energy": best, "count_mod_2_64": cnt}
+
+
+def solve_king_bb(L, seed=1, block=4, chunk=4, max_batch=1024):
+    k = I.kings_subgraph(L, L, 0.8, seed)
+    ids = -np.ones((L, L), int)
+    ids[k.meta["keep"]] = np.arange(k.n_vertices)
+    offs, verts = [0], []
+    for r0 in range(0, L, block):
+        for c0 in range(0, L, block):
+            verts += [int(ids[r][c]) for r in range(r0, min(r0 + block, L)) for c in range(c0, min(c0 + block, L)) if ids[r][c] >= 0]
+            offs.append(len(verts))
+    branch = np.array([ids[L // 2][c] for c in range(L) if ids[L // 2][c] >= 0], np.int32)
+    h = bb.Handle(k, max_elements_per_leaf=1 << 26)
+    t0 = time.perf_counter()
+    out = h.solve_bb(branch, chunk, offs, verts, max_batch=max_batch, use_pruning=True)
+    dt = time.perf_counter() - t0
+    h.close()
+    return {"instance": f"king {L}x{L} p0.8 seed {seed}", "mode": f"host B&B on the middle row ({len(branch)} vertices), {block}x{block} regions, K5 pruning",
+            "n_vertices": k.n_vertices, "n_edges": k.n_edges, "seconds": dt, "energy": out["energy"], "count_mod_2_64": out["count"],
+            "nodes_generated": out["generated"], "nodes_pruned": out["pruned"], "leaves_contracted": out["contracted"],
+            "contract_calls": out["calls"]}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", nargs="*", default=["1", "2", "3", "4b", "5"])
+    ap.add_argument("--king-sizes", nargs="*", type=int, default=[16, 20, 24])
+    ap.add_argument("--repeat", type=int, default=5)
+    a = ap.parse_args()
+    bb.load()
+    emit = lambda d: print(json.dumps(d), flush=True)
+    if "1" in a.configs:
+        for seed in (1, 2, 3):
+            emit(solve_unbranched(f"config1 ising 6x6 seed {seed}", I.ising_lattice_2d(6, 6, seed), repeat=a.repeat))
+    if "2" in a.configs:
+        for seed in (1, 2, 3):
+            emit(solve_unbranched(f"config2 king 12x12 p0.8 seed {seed}", I.kings_subgraph(12, 12, 0.8, seed), repeat=a.repeat))
+    if "3" in a.configs:
+        inst = I.ising_lattice_2d(24, 24, 1)
+        for f in (8, 10, 12):
+            fixed = I.slit_fixed_set_2d(24, 24, f)
+            tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(24, 24, f))
+            emit(solve_branched("config3 ising 24x24 seed 1", inst, fixed, tree, repeat=a.repeat))
+    if "4b" in a.configs:
+        inst = I.ising_lattice_3d(5, 5, 5, 1)
+        for f in (6, 8, 10):
+            fixed = I.layer_fixed_set_3d(5, 5, 5, f)
+            tree = I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+            emit(solve_branched("config4b ising 5x5x5 seed 1", inst, fixed, tree, repeat=a.repeat))
+    if "5" in a.configs:
+        for L in a.king_sizes:
+            emit(solve_king_bb(L))
+
+
+if __name__ == "__main__":
+    main()

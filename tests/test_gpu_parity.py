@@ -1,5 +1,7 @@
 """Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element,
 on the same seeded inputs.  Integer work: the bar is BIT-EXACT for energies and counts."""
+import os
+
 import numpy as np
 import pytest
 
@@ -358,3 +360,52 @@ def test_solve_bb_matches_unbranched(bb, oracle, case):
         if not pruning and inst.kind == "ising":
             assert out["contracted"] == 1 << len(branch)
     assert out["contracted"] <= 1 << len(branch)
+
+
+# ---- BASELINE configs at FULL size vs goldens written by the oracle (tests/golden/make_config_goldens.py) ----
+def _goldens():
+    import json
+    with open(os.path.join(os.path.dirname(__file__), "golden", "config_goldens.json")) as f:
+        return json.load(f)["cases"]
+
+
+def _expect(name):
+    g = _goldens()[name]
+    return int(g["energy"]), int(g["count"]) & MASK64
+
+
+def test_config3_full_size_24x24_all_leaves(bb):
+    # the launch configuration time_to_solve.py times: slit of f spins, all 2^f leaves in one call
+    from paper_2602_05470_b200 import time_to_solve as T
+    inst = I.ising_lattice_2d(24, 24, 1)
+    for f in (8, 10):
+        fixed = I.slit_fixed_set_2d(24, 24, f)
+        tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(24, 24, f))
+        out = T.solve_branched("config3", inst, fixed, tree, repeat=1)
+        assert (out["energy"], out["count_mod_2_64"]) == _expect("config3 ising 24x24 seed 1")
+
+
+def test_config4b_full_size_cube_all_leaves(bb):
+    from paper_2602_05470_b200 import time_to_solve as T
+    inst = I.ising_lattice_3d(5, 5, 5, 1)
+    fixed = I.layer_fixed_set_3d(5, 5, 5, 8)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+    out = T.solve_branched("config4b", inst, fixed, tree, repeat=1)
+    assert (out["energy"], out["count_mod_2_64"]) == _expect("config4b ising 5x5x5 seed 1")
+
+
+@pytest.mark.parametrize("L", [16, 20, 24])
+def test_config5_shape_kings_branch_and_bound(bb, L):
+    # config 5's pipeline (K5 bounds + host B&B + batched leaves) at the sizes it reaches this round
+    from paper_2602_05470_b200 import time_to_solve as T
+    out = T.solve_king_bb(L)
+    assert (out["energy"], out["count_mod_2_64"]) == _expect(f"config5-shape king {L}x{L} p0.8 seed 1")
+    assert out["leaves_contracted"] + out["nodes_pruned"] <= out["nodes_generated"]
+
+
+def test_config1_config2_full_size_goldens(bb):
+    for seed in (1, 2):
+        e, c = bb.Handle(I.ising_lattice_2d(6, 6, seed)).contract_batch()
+        assert (int(e[0]), int(c[0])) == _expect(f"config1 ising 6x6 seed {seed}")
+    e, c = bb.Handle(I.kings_subgraph(12, 12, 0.8, 1)).contract_batch()
+    assert (int(e[0]), int(c[0])) == _expect("config2 king 12x12 p0.8 seed 1")
