@@ -335,7 +335,9 @@ def run_ours(args):
     gemm_gfma = gemm_fma / (gemm_ms * 1e-3) / 1e9
     achieved = INT_OPS_PER_FMA[32] * gemm_gfma
     roofline = {"bound": "alu", "kernel": "gemm_tiled_kernel (K3)", "achieved": achieved, "peak": int_peak, "unit": "Gop/s",
-                "frac": achieved / int_peak, "traffic": None,
+                "frac": achieved / int_peak,
+                "traffic": 2.589e9,     # dram__bytes_read.sum + dram__bytes_write.sum of this launch, profiles/r1d_gemm_permute_ncu.txt
+                "traffic_unit": "bytes per launch (algorithmic operand+result bytes: %.3e)" % (3.0 * gb * n * n * 12),
                 "note": (f"op = int32 lane-instruction; achieved = {INT_OPS_PER_FMA[32]} algorithmic int32 instructions per tropical FMA "
                          "(fused add-max, tie add, tie compare, 32x32+64 multiply-add) x GFMA/s of the K3 launch; peak = committed "
                          "microbenchmark (bbtn_int32_microbench), best of IADD3 / IMNMX / IMAD / mixed ALU+FMA-pipe issue, same run; "
