@@ -226,13 +226,22 @@ int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, c
   if (rc) return rc;
   if ((rc = upload_tables(h, dp))) return rc;
   const bool dev_io = (h->P.flags & BBTN_IO_DEVICE) != 0;
+  // With host pointers the library owns the device-side batch buffers, so the launched batch is rounded up to
+  // a power of two (padding leaves = assignment 0, results dropped): the CUDA graph of this fixed set is then
+  // captured once per size class instead of once per distinct B (the host B&B loop sends ragged batches).
+  const int64_t B_user = B;
+  if (!dev_io) { int64_t bp = 1; while (bp < B) bp <<= 1; B = bp; }
   if ((rc = ensure_batch(h, dp, B, !dev_io))) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const uint8_t *d_assign = assign; int32_t *d_energy = energy; uint64_t *d_count = count; uint32_t *d_mod = count_mod;
   if (!dev_io) {
     d_assign = (const uint8_t *)dp->assign.p; d_energy = (int32_t *)dp->energy.p; d_count = (uint64_t *)dp->count.p;
     d_mod = count_mod ? (uint32_t *)dp->count_mod.p : nullptr;
-    if (n_fixed > 0) CUDA_TRY(h, cudaMemcpyAsync(dp->assign.p, assign, (size_t)B * n_fixed, cudaMemcpyHostToDevice, st));
+    if (n_fixed > 0) {
+      CUDA_TRY(h, cudaMemcpyAsync(dp->assign.p, assign, (size_t)B_user * n_fixed, cudaMemcpyHostToDevice, st));
+      if (B > B_user)
+        CUDA_TRY(h, cudaMemsetAsync((char *)dp->assign.p + (size_t)B_user * n_fixed, 0, (size_t)(B - B_user) * n_fixed, st));
+    }
   }
   const int n_rings = (crt && d_mod) ? 3 : 1;
   const bool use_graph = !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
@@ -263,13 +272,13 @@ int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, c
   CUDA_TRY(h, cudaGetLastError());
   if (!dev_io) {
     // stage into temporaries so that outputs stay untouched on error
-    std::vector<int32_t> te((size_t)B); std::vector<uint64_t> tc((size_t)B); std::vector<uint32_t> tm(count_mod ? (size_t)B * 2 : 0);
-    CUDA_TRY(h, cudaMemcpyAsync(te.data(), d_energy, (size_t)B * 4, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(h, cudaMemcpyAsync(tc.data(), d_count, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
-    if (count_mod) CUDA_TRY(h, cudaMemcpyAsync(tm.data(), d_mod, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    std::vector<int32_t> te((size_t)B_user); std::vector<uint64_t> tc((size_t)B_user); std::vector<uint32_t> tm(count_mod ? (size_t)B_user * 2 : 0);
+    CUDA_TRY(h, cudaMemcpyAsync(te.data(), d_energy, (size_t)B_user * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(h, cudaMemcpyAsync(tc.data(), d_count, (size_t)B_user * 8, cudaMemcpyDeviceToHost, st));
+    if (count_mod) CUDA_TRY(h, cudaMemcpyAsync(tm.data(), d_mod, (size_t)B_user * 8, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(h, cudaStreamSynchronize(st));
-    std::memcpy(energy, te.data(), (size_t)B * 4); std::memcpy(count, tc.data(), (size_t)B * 8);
-    if (count_mod) std::memcpy(count_mod, tm.data(), (size_t)B * 8);
+    std::memcpy(energy, te.data(), (size_t)B_user * 4); std::memcpy(count, tc.data(), (size_t)B_user * 8);
+    if (count_mod) std::memcpy(count_mod, tm.data(), (size_t)B_user * 8);
   }
   return BBTN_OK;
 }

@@ -60,13 +60,22 @@ __device__ __forceinline__ void tie_fma(typename AccT<MODE>::T &c, int32_t ea, i
         : "+r"(c32) : "r"(ea), "r"(eb), "r"(E), "r"((uint32_t)ca), "r"((uint32_t)cb));
     c = c32;
   } else if (MODE == ACC64N) {
+    // ptxas lowers a predicated 64-bit multiply-add to multiply + 2 selects + 2 adds; selecting the 32-bit
+    // multiplicand instead keeps it at SEL + IMAD.WIDE (with the 64-bit accumulate fused)
     uint64_t c64 = c;
-    asm("{\n\t.reg .pred p;\n\t.reg .s32 s;\n\tadd.s32 s, %1, %2;\n\tsetp.eq.s32 p, s, %3;\n\t@p mad.wide.u32 %0, %4, %5, %0;\n\t}"
+    asm("{\n\t.reg .pred p;\n\t.reg .s32 s;\n\t.reg .u32 t;\n\tadd.s32 s, %1, %2;\n\tsetp.eq.s32 p, s, %3;\n\t"
+        "selp.u32 t, %5, 0, p;\n\tmad.wide.u32 %0, %4, t, %0;\n\t}"
         : "+l"(c64) : "r"(ea), "r"(eb), "r"(E), "r"((uint32_t)ca), "r"((uint32_t)cb));
     c = c64;
   } else {
+    // full 64x64->64: low product through SEL + IMAD.WIDE, the two cross terms as predicated 32-bit IMADs
     uint64_t c64 = c;
-    asm("{\n\t.reg .pred p;\n\t.reg .s32 s;\n\tadd.s32 s, %1, %2;\n\tsetp.eq.s32 p, s, %3;\n\t@p mad.lo.u64 %0, %4, %5, %0;\n\t}"
+    asm("{\n\t.reg .pred p;\n\t.reg .s32 s;\n\t.reg .u32 alo, ahi, blo, bhi, t, clo, chi;\n\t"
+        "mov.b64 {alo, ahi}, %4;\n\tmov.b64 {blo, bhi}, %5;\n\t"
+        "add.s32 s, %1, %2;\n\tsetp.eq.s32 p, s, %3;\n\tselp.u32 t, blo, 0, p;\n\t"
+        "mad.wide.u32 %0, alo, t, %0;\n\tmov.b64 {clo, chi}, %0;\n\t"
+        "@p mad.lo.u32 chi, alo, bhi, chi;\n\t@p mad.lo.u32 chi, ahi, blo, chi;\n\t"
+        "mov.b64 %0, {clo, chi};\n\t}"
         : "+l"(c64) : "r"(ea), "r"(eb), "r"(E), "l"(ca), "l"(cb));
     c = c64;
   }

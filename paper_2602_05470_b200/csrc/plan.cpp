@@ -1,5 +1,6 @@
 // plan.cpp -- host planner (see plan.h).  Plain C++17, no CUDA, no oracle code.
 #include "plan.h"
+#include <cmath>
 
 #include <algorithm>
 #include <map>
@@ -101,48 +102,63 @@ void derive_tree(const Problem &P, const std::vector<int32_t> &fixed,
       for (size_t j = i + 1; j < nb.size(); j++) { adj[nb[i]].insert(nb[j]); adj[nb[j]].insert(nb[i]); }
     adj[best].clear();
   }
-  // --- bucket elimination: merge all live tensors carrying v, smallest first
-  std::map<int, std::set<int>> live;            // tensor id -> labels
-  std::vector<std::set<int>> occ(n);            // label -> tensor ids
-  for (int t = 0; t < n_in; t++) {
-    std::set<int> s;
-    if (t < m) { if (!isfixed[P.eu[t]]) s.insert(P.eu[t]); if (!isfixed[P.ev[t]]) s.insert(P.ev[t]); }
-    else if (!isfixed[t - m]) s.insert(t - m);
-    for (int i : s) occ[i].insert(t);
-    live[t] = s;
-  }
-  int nxt = n_in;
-  tl.clear(); tr.clear();
-  auto merge = [&](int a, int b) {
-    std::set<int> sa = live[a], sb = live[b];
-    live.erase(a); live.erase(b);
-    for (int i : sa) occ[i].erase(a);
-    for (int i : sb) occ[i].erase(b);
-    std::set<int> keep;
-    for (int i : sa) if (!occ[i].empty()) keep.insert(i);   // still carried by another live tensor
-    for (int i : sb) if (!occ[i].empty()) keep.insert(i);
-    for (int i : keep) occ[i].insert(nxt);
-    live[nxt] = keep;
-    tl.push_back(a); tr.push_back(b);
-    return nxt++;
-  };
-  for (int v : order) {
-    while (occ[v].size() >= 2) {
-      int a = -1, b = -1;
-      for (int t : occ[v]) {
-        if (a < 0 || live[t].size() < live[a].size()) { b = a; a = t; }
-        else if (b < 0 || live[t].size() < live[b].size()) b = t;
-      }
-      merge(a, b);
+  // --- bucket elimination along an order: merge all live tensors carrying v, smallest first.
+  //     Returns (width = largest merged label set, cost = sum of 2^|union| over the merges).
+  auto eliminate = [&](const std::vector<int> &ord, std::vector<int32_t> &ol, std::vector<int32_t> &orr, int &width, double &cost) {
+    std::map<int, std::set<int>> live;            // tensor id -> labels
+    std::vector<std::set<int>> occ(n);            // label -> tensor ids
+    for (int t = 0; t < n_in; t++) {
+      std::set<int> s;
+      if (t < m) { if (!isfixed[P.eu[t]]) s.insert(P.eu[t]); if (!isfixed[P.ev[t]]) s.insert(P.ev[t]); }
+      else if (!isfixed[t - m]) s.insert(t - m);
+      for (int i : s) occ[i].insert(t);
+      live[t] = s;
     }
-  }
-  std::vector<std::pair<size_t, int>> rest;
-  for (auto &kv : live) rest.push_back({kv.second.size(), kv.first});
-  std::sort(rest.begin(), rest.end());
-  if (!rest.empty()) {
-    int cur = rest[0].second;
-    for (size_t i = 1; i < rest.size(); i++) cur = merge(cur, rest[i].second);
-  }
+    int nxt = n_in;
+    ol.clear(); orr.clear(); width = 0; cost = 0;
+    auto merge = [&](int a, int b) {
+      std::set<int> sa = live[a], sb = live[b];
+      live.erase(a); live.erase(b);
+      for (int i : sa) occ[i].erase(a);
+      for (int i : sb) occ[i].erase(b);
+      std::set<int> uni = sa;
+      uni.insert(sb.begin(), sb.end());
+      width = std::max(width, (int)uni.size());
+      cost += std::ldexp(1.0, (int)uni.size());
+      std::set<int> keep;
+      for (int i : uni) if (!occ[i].empty()) keep.insert(i);   // still carried by another live tensor
+      for (int i : keep) occ[i].insert(nxt);
+      live[nxt] = keep;
+      ol.push_back(a); orr.push_back(b);
+      return nxt++;
+    };
+    for (int v : ord) {
+      while (occ[v].size() >= 2) {
+        int a = -1, b = -1;
+        for (int t : occ[v]) {
+          if (a < 0 || live[t].size() < live[a].size()) { b = a; a = t; }
+          else if (b < 0 || live[t].size() < live[b].size()) b = t;
+        }
+        merge(a, b);
+      }
+    }
+    std::vector<std::pair<size_t, int>> rest;
+    for (auto &kv : live) rest.push_back({kv.second.size(), kv.first});
+    std::sort(rest.begin(), rest.end());
+    if (!rest.empty()) {
+      int cur = rest[0].second;
+      for (size_t i = 1; i < rest.size(); i++) cur = merge(cur, rest[i].second);
+    }
+  };
+  // candidates: the min-degree order and the plain vertex-id order (a frontier sweep for instances
+  // numbered row-major, e.g. lattices and King's subgraphs); keep the narrower, then the cheaper one
+  std::vector<int> natural;
+  for (int v = 0; v < n; v++) if (!isfixed[v]) natural.push_back(v);
+  std::vector<int32_t> l2, r2;
+  int w1 = 0, w2 = 0; double c1 = 0, c2 = 0;
+  eliminate(order, tl, tr, w1, c1);
+  eliminate(natural, l2, r2, w2, c2);
+  if (w2 < w1 || (w2 == w1 && c2 < c1)) { tl.swap(l2); tr.swap(r2); }
 }
 
 int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mode, bool enforce_cap,
