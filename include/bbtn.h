@@ -85,7 +85,7 @@ typedef struct {
   const int32_t *vertex_w;         /* Ising: integer h_i (NULL = no field). MIS: w_i (NULL = 1)  */
   int32_t n_steps;                 /* 0 with tree_l == NULL, else n_edges + n_vertices - 1       */
   const int32_t *tree_l, *tree_r;  /* [n_steps] or NULL                                          */
-  int64_t max_elements_per_leaf;   /* T_target of Eq. 4, in ELEMENTS; 0 = 2^28     */
+  int64_t max_elements_per_leaf;   /* T_target of Eq. 4, in ELEMENTS, <= 2^32; 0 = 2^28 */
   uint32_t flags;
 } bbtn_problem_desc;
 
@@ -161,6 +161,35 @@ int bbtn_solve_bb(bbtn_handle *h,
                   int64_t max_batch, int32_t incumbent_hint, int32_t use_pruning,
                   int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats,
                   void *cuda_stream);
+
+/* BBTN proper: non-uniform branching driven by the memory-overflow measure
+ *   rho(T) = sum over the tensors of the contraction tree of max(0, log2|T| - log2 T_target)   (Eq. 4)
+ * on the handle's contraction tree (the caller's, else the library's tree of the unsliced network).
+ * Each branching takes the free vertex v that minimises the branching factor gamma, the root of
+ * gamma^rho(T) = sum_i gamma^rho(T_i), over the rules
+ *   MIS:   { v = 0 } , { v = 1 and every free neighbour of v = 0 }        Ising: { s_v = 0 } , { s_v = 1 }
+ * (complete and orthogonal; the paper's rule search and inference rules are in its missing
+ * supplement, reading A23).  A branch with rho = 0 whose arena fits mem_budget_bytes is a leaf:
+ * its fixed indices are deleted from the tree, it is contracted by K1..K4 on the device (one plan per leaf,
+ * device buffers reused) and the leaf results are (+)-accumulated.  Leaves have DIFFERENT fixed sets
+ * ("different subsets of R are fixed across different branches").
+ *   log2_target       log2 T_target in ELEMENTS, 1..32 (the paper runs 2^31)
+ *   mem_budget_bytes  device bytes one leaf may use; 0 = 94 % of the free device memory
+ *   max_leaves        give up with BBTN_ESHAPE beyond this many leaves; 0 = unlimited
+ *   energy/count/count_mod  as bbtn_solve_bb;  stats[0..3] = branching nodes, leaves, largest |F|, rho of the root
+ *   work[0..1] = tropical FMAs, algorithmic bytes summed over the leaves (planner totals)
+ * Host pointers only.  Errors: EINVAL, ESHAPE, ENOMEM, ECUDA. */
+int bbtn_solve_branching(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t max_leaves,
+                         int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats, double *work,
+                         void *cuda_stream);
+
+/* The same branching without contracting anything (host only, no device needed): writes the leaves in CSR
+ * form -- leaf i fixes leaf_vertices[leaf_offsets[i] .. leaf_offsets[i+1]) to leaf_values[...] -- when the three
+ * arrays are non-NULL (capacities cap_leaves + 1 offsets, cap_entries vertices/values; EINVAL if too small),
+ * and stats/work as above.  mem_budget_bytes = 0 means no memory limit here. */
+int bbtn_branching_leaves(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t max_leaves,
+                          int64_t cap_leaves, int64_t cap_entries, int64_t *leaf_offsets, int32_t *leaf_vertices,
+                          uint8_t *leaf_values, int64_t *stats, double *work);
 
 /* Host-side (+) over leaf results in reported units (Eq. 3's outer sum; "the final
  * result is obtained by summing the contractions of each branch"): keeps the best

@@ -117,6 +117,25 @@ def frontier_dp(inst, order=None, fixed=None, assign=None, return_width=False):
     return out + (mf.value,) if return_width else out
 
 
+def frontier_dp_mis_sparse(inst, order=None, fixed=None, assign=None, return_stats=False):
+    """oracle-3 for MIS with only the independent frontier states stored (SURVEY.md 8(c));
+    reaches King's subgraphs whose dense frontier table would not fit.  Returns (size, count)."""
+    assert _kind(inst.kind) == 1
+    lib = _load()
+    eu, ev, _, vw = _common(inst)
+    fx, asg = _fixed(fixed, assign)
+    od = np.arange(inst.n_vertices, dtype=np.int32) if order is None else _i32(order)
+    assert len(od) == inst.n_vertices
+    e = C.c_int64(); f = C.c_int32(); c4 = (C.c_uint64 * 4)(); mf = C.c_int32(); ms = C.c_int64()
+    rc = lib.oracle_frontier_dp_mis_sparse(inst.n_vertices, inst.n_edges, _p(eu), _p(ev), _p(vw), _p(od),
+                                           len(fx), _p(fx), _p(asg), C.byref(e), C.byref(f), c4,
+                                           C.byref(mf), C.byref(ms))
+    if rc:
+        raise RuntimeError(f"oracle_frontier_dp_mis_sparse rc={rc}")
+    out = ((e.value if f.value else None), _count(c4))
+    return out + (mf.value, ms.value) if return_stats else out
+
+
 def gemm(Ae, Az, Ac, Be, Bz, Bc, full_counts=False):
     """C[b,m,n] = (+)_k A[b,m,k] (.) B[b,k,n].  A* are [B][M][K], B* are [B][K][N].
     Energies int64, zero flags uint8, counts uint64.  Returns (Ce, Cz, Cc mod 2^64[, Cc4])."""

@@ -21,6 +21,8 @@
  *                          loop nests, sliced per Eq. 3 (:61).
  *   oracle_frontier_dp     independent exact method: vertex-by-vertex transfer
  *                          (frontier) dynamic programme in the same algebra.
+ *   oracle_frontier_dp_mis_sparse  the same programme for MIS with only the
+ *                          independent frontier states stored (large King's subgraphs).
  *   oracle_gemm            C[b,m,n] = (+)_k A[b,m,k] (.) B[b,k,n], triple loop.
  *   oracle_permute         dst[pi(i)] = src[i] for a bit permutation pi.
  *   oracle_region_bound    DESIGN.md reading A15 of the pruning bound
@@ -334,6 +336,118 @@ int oracle_frontier_dp(int kind, int n, int m, const int32_t *eu, const int32_t 
     }
     if (!rc) { if (sz != 1) rc = 6; else write_out(tab[0], kind, energy, feasible, count4); }
     free(tab); free(val); free(visited); free(remaining);
+    return rc;
+}
+
+/* ---- oracle-3, sparse form for MIS ("for MIS only independent frontier
+ * states are stored") --------------------------------------------------------------------
+ * Same vertex-by-vertex transfer as oracle_frontier_dp, but the table holds only the
+ * frontier states that are independent sets (every other state is the zero element,
+ * PAPER.md:55), as a list sorted by key.  key bit p = 1 <=> the frontier vertex in slot p
+ * is in the set.  Visiting v: every state survives with v out; a state with no chosen
+ * frontier neighbour of v also spawns (key | bit_v, e + w_v, c).  A frontier vertex whose
+ * neighbours are all visited is summed out: its bit is cleared and equal keys are (+)-merged.
+ * Both operations are merges of two key-sorted lists.  Handles frontiers of up to 64 vertices. */
+typedef struct { uint64_t key; int64_t e; u256 c; } sstate;
+
+int oracle_frontier_dp_mis_sparse(int n, int m, const int32_t *eu, const int32_t *ev,
+                                  const int32_t *vertex_w, const int32_t *order,
+                                  int n_fixed, const int32_t *fixed, const uint8_t *assign,
+                                  int64_t *energy, int32_t *feasible, uint64_t *count4,
+                                  int32_t *max_frontier, int64_t *max_states)
+{
+    int *val = (int *)malloc(sizeof(int) * (size_t)(n + 1));
+    int *visited = (int *)calloc((size_t)(n + 1), sizeof(int));
+    int *remaining = (int *)calloc((size_t)(n + 1), sizeof(int));
+    int *slot = (int *)malloc(sizeof(int) * (size_t)(n + 1));
+    for (int i = 0; i < n; i++) { val[i] = -1; slot[i] = -1; }
+    for (int j = 0; j < n_fixed; j++) val[fixed[j]] = assign[j] ? 1 : 0;
+    for (int e = 0; e < m; e++) { remaining[eu[e]]++; remaining[ev[e]]++; }
+    uint64_t used = 0;            /* occupied slots */
+    int nfr = 0, rc = 0;
+    size_t sz = 1;
+    sstate *tab = (sstate *)malloc(sizeof(sstate));
+    tab[0].key = 0; tab[0].e = 0; tab[0].c = u256_from(1);
+    *max_frontier = 0; *max_states = 1;
+    for (int step = 0; step < n && !rc; step++) {
+        int v = order[step];
+        if (v < 0 || v >= n || visited[v]) { rc = 2; break; }
+        int64_t w = vw_of(1, vertex_w, v);
+        uint64_t nbmask = 0; int nb_fixed_in = 0;
+        for (int e = 0; e < m; e++) {
+            int u = -1;
+            if (eu[e] == v) u = ev[e]; else if (ev[e] == v) u = eu[e];
+            if (u < 0 || !visited[u]) continue;
+            if (val[u] == 1) nb_fixed_in = 1;
+            else if (val[u] < 0) nbmask |= 1ull << slot[u];
+        }
+        if (val[v] == 1) {
+            /* forced in: states with a chosen neighbour die, the rest gain w */
+            size_t k = 0;
+            for (size_t s = 0; s < sz; s++)
+                if (!nb_fixed_in && !(tab[s].key & nbmask)) { tab[k] = tab[s]; tab[k].e += w; k++; }
+            sz = k;
+        } else if (val[v] < 0) {
+            if (nfr >= 64) { rc = 4; break; }
+            int p = 0; while (used & (1ull << p)) p++;
+            slot[v] = p; used |= 1ull << p; nfr++;
+            if (!nb_fixed_in) {
+                uint64_t bit = 1ull << p;
+                sstate *nt = (sstate *)malloc(sizeof(sstate) * (2 * sz + 1));
+                if (!nt) { rc = 5; break; }
+                /* list "out" = tab as it is; list "in" = eligible states with the bit set; merge by key */
+                size_t i = 0, j = 0, k = 0;
+                while (j < sz && (tab[j].key & nbmask)) j++;
+                while (i < sz || j < sz) {
+                    if (j >= sz || (i < sz && tab[i].key < (tab[j].key | bit))) nt[k++] = tab[i++];
+                    else {
+                        nt[k] = tab[j]; nt[k].key |= bit; nt[k].e += w; k++;
+                        j++; while (j < sz && (tab[j].key & nbmask)) j++;
+                    }
+                }
+                free(tab); tab = nt; sz = k;
+            }
+        }
+        visited[v] = 1;
+        for (int e = 0; e < m; e++) { if (eu[e] == v) remaining[ev[e]]--; else if (ev[e] == v) remaining[eu[e]]--; }
+        if (nfr > *max_frontier) *max_frontier = nfr;
+        if ((int64_t)sz > *max_states) *max_states = (int64_t)sz;
+        /* sum out every frontier vertex whose neighbours have all been visited */
+        for (int u = 0; u < n && !rc; u++) {
+            if (slot[u] < 0 || remaining[u] > 0) continue;
+            uint64_t bit = 1ull << slot[u];
+            sstate *nt = (sstate *)malloc(sizeof(sstate) * (sz + 1));
+            if (!nt) { rc = 5; break; }
+            size_t i = 0, j = 0, k = 0;     /* i walks states with the bit clear, j those with it set */
+            while (i < sz && (tab[i].key & bit)) i++;
+            while (j < sz && !(tab[j].key & bit)) j++;
+            while (i < sz || j < sz) {
+                uint64_t ki = i < sz ? tab[i].key : ~0ull, kj = j < sz ? (tab[j].key & ~bit) : ~0ull;
+                if (i < sz && (j >= sz || ki < kj)) {
+                    nt[k++] = tab[i];
+                    i++; while (i < sz && (tab[i].key & bit)) i++;
+                } else if (j < sz && (i >= sz || kj < ki)) {
+                    nt[k] = tab[j]; nt[k].key = kj; k++;
+                    j++; while (j < sz && !(tab[j].key & bit)) j++;
+                } else {                    /* same key: (+) */
+                    elem a = el_make(tab[i].e, 0), b = el_make(tab[j].e, 0);
+                    a.c = tab[i].c; b.c = tab[j].c;
+                    elem r = el_add(a, b);
+                    nt[k].key = ki; nt[k].e = r.e; nt[k].c = r.c; k++;
+                    i++; while (i < sz && (tab[i].key & bit)) i++;
+                    j++; while (j < sz && !(tab[j].key & bit)) j++;
+                }
+            }
+            free(tab); tab = nt; sz = k;
+            used &= ~bit; slot[u] = -1; nfr--;
+        }
+    }
+    if (!rc) {
+        if (sz > 1) rc = 6;
+        else if (sz == 0) write_out(el_zero(), 1, energy, feasible, count4);
+        else { elem r = el_make(tab[0].e, 0); r.c = tab[0].c; write_out(r, 1, energy, feasible, count4); }
+    }
+    free(tab); free(val); free(visited); free(remaining); free(slot);
     return rc;
 }
 

@@ -23,7 +23,7 @@ BBTN_COUNT_CRT, BBTN_IO_DEVICE, BBTN_NO_GRAPH = 0x1, 0x2, 0x4
 BBTN_FORCE_STREAMING, BBTN_FORCE_TILED = 0x10, 0x20
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
-EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb",
+EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves",
            "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
            "bbtn_permute_batched", "bbtn_int32_microbench",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
@@ -65,6 +65,8 @@ def load():
     lib.bbtn_plan_query.argtypes = [vp, vp, i32, i64, C.POINTER(_PlanInfo)]
     lib.bbtn_region_bound.argtypes = [vp, vp, vp, i32, vp, i32, vp, i64, vp, vp]
     lib.bbtn_solve_bb.argtypes = [vp, vp, i32, i32, vp, vp, i32, i64, i32, i32, vp, vp, vp, vp, vp]
+    lib.bbtn_solve_branching.argtypes = [vp, i32, i64, i64, vp, vp, vp, vp, vp, vp]
+    lib.bbtn_branching_leaves.argtypes = [vp, i32, i64, i64, i64, i64, vp, vp, vp, vp, vp]
     lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
     lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
     lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
@@ -193,6 +195,37 @@ class Handle:
         if crt:
             out["count_mod"] = (cm[0], cm[1])
         return out
+
+
+    def solve_branching(self, log2_target: int, mem_budget_bytes: int = 0, max_leaves: int = 0, stream=None):
+        """bbtn_solve_branching: rho-driven non-uniform branching (Eq. 4), leaves contracted on the device."""
+        e = C.c_int32(); c = C.c_uint64(); cm = (C.c_uint32 * 2)(); stats = (C.c_int64 * 4)(); work = (C.c_double * 2)()
+        crt = bool(self.flags & BBTN_COUNT_CRT)
+        _check(load().bbtn_solve_branching(self._h, log2_target, mem_budget_bytes, max_leaves, C.addressof(e),
+                                           C.addressof(c), C.addressof(cm) if crt else None, C.addressof(stats),
+                                           C.addressof(work), _stream(stream)), self._h)
+        out = {"energy": e.value, "count": c.value, "branch_nodes": stats[0], "leaves": stats[1],
+               "max_fixed": stats[2], "rho_root": stats[3], "fma": work[0], "bytes": work[1]}
+        if crt:
+            out["count_mod"] = (cm[0], cm[1])
+        return out
+
+    def branching_leaves(self, log2_target: int, mem_budget_bytes: int = 0, max_leaves: int = 0, store: bool = True,
+                         cap_entries: int = 1 << 24):
+        """bbtn_branching_leaves (host only): the leaves [(fixed vertices, values)] and the stats."""
+        stats = (C.c_int64 * 4)(); work = (C.c_double * 2)()
+        if not store:
+            _check(load().bbtn_branching_leaves(self._h, log2_target, mem_budget_bytes, max_leaves, 0, 0, None, None,
+                                                None, C.addressof(stats), C.addressof(work)), self._h)
+            leaves = None
+        else:
+            cap_leaves = max(max_leaves, 1 << 16)
+            off = np.zeros(cap_leaves + 1, np.int64); lv = np.zeros(cap_entries, np.int32); lx = np.zeros(cap_entries, np.uint8)
+            _check(load().bbtn_branching_leaves(self._h, log2_target, mem_budget_bytes, max_leaves, cap_leaves, cap_entries,
+                                                _ptr(off), _ptr(lv), _ptr(lx), C.addressof(stats), C.addressof(work)), self._h)
+            leaves = [(lv[off[i]:off[i + 1]].copy(), lx[off[i]:off[i + 1]].copy()) for i in range(stats[1])]
+        return leaves, {"branch_nodes": stats[0], "leaves": stats[1], "max_fixed": stats[2], "rho_root": stats[3],
+                        "fma": work[0], "bytes": work[1]}
 
 
 def tropical_gemm_batched(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, stream=None):

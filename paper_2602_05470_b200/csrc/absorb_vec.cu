@@ -25,7 +25,7 @@ enum LowPattern : int { LP_FAR = 0, LP_K0 = 1, LP_K1 = 2 };
 
 struct AbsorbVecArgs {
   int rO, nK, tb;                 // output rank, summed bits, tile bits (<= 12)
-  uint32_t addA[28], addB[28];    // per output bit
+  uint32_t addA[32], addB[32];    // per output bit
   uint32_t kA[8], kB[8];          // per summed bit
   int64_t sA, sB, sC, n_tiles;    // batch strides (elements), tiles over all batch entries
 };
@@ -149,7 +149,7 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
 #endif
   AbsorbVecArgs p;
   p.rO = s.rO; p.nK = s.nK; p.tb = s.rO < 12 ? s.rO : 12;
-  for (int i = 0; i < 28; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
+  for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
   for (int i = 0; i < 8; i++) { p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
   // the 16-byte reads of A must stay 4-element aligned: every offset that can be added is a multiple of 4
   for (int q = 2; q < s.rO; q++) if (p.addA[q] & 3u) return false;

@@ -224,6 +224,18 @@ int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, c
   DevPlan *dp = nullptr;
   int rc = get_plan(h, fixed, n_fixed, true, &dp);
   if (rc) return rc;
+  return bbtn::run_plan(h, dp, assign, B, energy, count, count_mod, true, stream);
+}
+
+}  // extern "C"
+
+// Run one planned contraction (K1 -> K2/K3 -> K4) for B leaves; shared by bbtn_contract_batch (cached
+// plans, CUDA-graph replay) and the branching driver (one-leaf plans on the handle's scratch buffers).
+int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B, int32_t *energy, uint64_t *count,
+                   uint32_t *count_mod, bool allow_graph, void *stream) {
+  const bool crt = (h->P.flags & BBTN_COUNT_CRT) != 0;
+  const int32_t n_fixed = (int32_t)dp->plan.fixed.size();
+  int rc;
   if ((rc = upload_tables(h, dp))) return rc;
   const bool dev_io = (h->P.flags & BBTN_IO_DEVICE) != 0;
   // With host pointers the library owns the device-side batch buffers, so the launched batch is rounded up to
@@ -244,7 +256,7 @@ int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, c
     }
   }
   const int n_rings = (crt && d_mod) ? 3 : 1;
-  const bool use_graph = !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
+  const bool use_graph = allow_graph && !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
   if (!use_graph) {
     for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring, st);
   } else {
@@ -282,6 +294,8 @@ int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, c
   }
   return BBTN_OK;
 }
+
+extern "C" {
 
 int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac,
                                const int32_t *Be, const uint64_t *Bc, int32_t *Ce, uint64_t *Cc,

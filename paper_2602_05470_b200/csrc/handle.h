@@ -55,6 +55,8 @@ struct BoundPlan {
 
 int fail(bbtn_handle *h, int code, const std::string &msg);
 bool have_device();
+int run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B, int32_t *energy, uint64_t *count,
+             uint32_t *count_mod, bool allow_graph, void *stream);
 
 }  // namespace bbtn
 
@@ -64,6 +66,10 @@ struct bbtn_handle {
   int force_mode = 0;
   std::map<std::vector<int32_t>, std::unique_ptr<bbtn::DevPlan>> plans;
   std::map<std::vector<int32_t>, std::unique_ptr<bbtn::BoundPlan>> bounds;
+  // branching driver (branching.cu): the unsliced tree every leaf is planned on, and one scratch plan whose
+  // device buffers are reused by every leaf (leaves have different fixed sets, so they are not cached)
+  std::unique_ptr<bbtn::Problem> Pbr;
+  std::unique_ptr<bbtn::DevPlan> scratch;
 };
 
 #define CUDA_TRY(h, expr)                                                                       \

@@ -83,7 +83,7 @@ __global__ void construct_offset_kernel(int kind, const InputRec *__restrict__ i
 // ---------------------------------------------------------------------------------------------
 struct AbsorbArgs {
   int rO, nK;
-  uint32_t addA[28], addB[28], kA[12], kB[12];
+  uint32_t addA[32], addB[32], kA[12], kB[12];
   int64_t sA, sB, sC, total;
 };
 
@@ -91,10 +91,10 @@ template <class R>
 __global__ void absorb_kernel(AbsorbArgs p, const int32_t *__restrict__ Ae, const typename R::T *__restrict__ Ac,
                               const int32_t *__restrict__ Be, const typename R::T *__restrict__ Bc,
                               int32_t *__restrict__ Ce, typename R::T *__restrict__ Cc) {
-  const uint32_t omask = (1u << p.rO) - 1u;
+  const int64_t omask = ((int64_t)1 << p.rO) - 1;      // rO may be 32
   for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < p.total; t += (int64_t)gridDim.x * blockDim.x) {
     const int64_t b = t >> p.rO;
-    const uint32_t o = (uint32_t)t & omask;
+    const uint32_t o = (uint32_t)(t & omask);
     uint32_t a0 = 0, b0 = 0;
     for (int q = 0; q < p.rO; q++) if ((o >> q) & 1u) { a0 += p.addA[q]; b0 += p.addB[q]; }
     const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
@@ -116,7 +116,7 @@ __global__ void absorb_kernel(AbsorbArgs p, const int32_t *__restrict__ Ae, cons
 // long-reduction form: one CTA per output element, block-wide (+) over k (tree roots, traces)
 struct ReduceArgs {
   int rO, nK;
-  uint32_t addA[28], addB[28], kA[28], kB[28];
+  uint32_t addA[32], addB[32], kA[32], kB[32];
   int64_t sA, sB, sC;
 };
 
@@ -134,9 +134,9 @@ __global__ void reduce_kernel(ReduceArgs p, const int32_t *__restrict__ Ae, cons
   const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
   const int32_t *be = Be + b * p.sB; const typename R::T *bc = Bc + b * p.sB;
   int32_t acc_e = NEG_INF; typename R::T acc_c = 0;
-  for (uint32_t k = threadIdx.x; k < (1u << p.nK); k += blockDim.x) {
+  for (uint64_t k = threadIdx.x; k < (1ull << p.nK); k += blockDim.x) {      // nK may be 32
     uint32_t ia = a0, ib = b0;
-    for (int j = 0; j < p.nK; j++) if ((k >> j) & 1u) { ia += p.kA[j]; ib += p.kB[j]; }
+    for (int j = 0; j < p.nK; j++) if ((k >> j) & 1ull) { ia += p.kA[j]; ib += p.kB[j]; }
     oplus<R>(acc_e, acc_c, ae[ia] + be[ib], R::mul(ac[ia], bc[ib]));
   }
   // warp (+), then across warps
@@ -219,7 +219,7 @@ void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
   if (launch_absorb_vec(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st)) return;   // 16-byte form (absorb_vec.cu)
   AbsorbArgs p;
   p.rO = s.rO; p.nK = s.nK;
-  for (int i = 0; i < 28; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
+  for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
   for (int i = 0; i < 12; i++) { p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
   p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
   p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
@@ -235,7 +235,7 @@ void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
   ReduceArgs p;
   p.rO = s.rO; p.nK = s.nK;
-  for (int i = 0; i < 28; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
+  for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
   p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
   p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
   p.sC = (int64_t)1 << s.rO;

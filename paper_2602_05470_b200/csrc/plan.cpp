@@ -162,7 +162,7 @@ void derive_tree(const Problem &P, const std::vector<int32_t> &fixed,
 }
 
 int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mode, bool enforce_cap,
-              Plan &out, std::string &err) {
+              Plan &out, std::string &err, bool single_arena, bool want_labels) {
   const int n = P.n, m = P.m, n_in = n + m;
   out = Plan();
   out.fixed = fixed;
@@ -174,7 +174,7 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
     fpos[v] = (int)j;
   }
   int cap_rank = 0;
-  while (((int64_t)1 << (cap_rank + 1)) <= P.max_elements && cap_rank < 30) cap_rank++;
+  while (((int64_t)1 << (cap_rank + 1)) <= P.max_elements && cap_rank < 32) cap_rank++;
 
   // ---- inputs
   std::vector<int> occ_total(n, 0);
@@ -200,7 +200,7 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
     if (r.fu < 0 && !r.su) { r.bu = rank++; x.idx.push_back(r.u); x.sub[r.u] = 1; }
     if (r.v >= 0 && r.fv < 0 && !r.sv) { r.bv = rank++; x.idx.push_back(r.v); x.sub[r.v] = 1; }
     r.rank = rank;
-    r.variant = (r.fu >= 0 || r.fv >= 0) ? 1 : 0;
+    r.variant = (single_arena || r.fu >= 0 || r.fv >= 0) ? 1 : 0;
     r.offset = -1;
     if (rank == 0) { out.scalar_inputs.push_back(t); x.removed = true; continue; }
     x.removed = false;
@@ -261,6 +261,13 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
       return ST_ESHAPE;
     }
     out.max_rank = std::max(out.max_rank, std::max(rO, std::max(rA, rB)));
+    if (want_labels) {
+      std::vector<int32_t> labs;
+      for (int lab : gl) labs.push_back(lab);
+      for (int lab : ml) labs.push_back(lab);
+      for (int lab : nl) labs.push_back(lab);
+      out.node_labels.push_back(std::move(labs));
+    }
     const bool var = O.variant;
     Arena &ao = var ? av : ai;
     const double fma = (double)((int64_t)1 << (rO + lk));

@@ -75,13 +75,18 @@ struct Plan {
   double fma_variant = 0, fma_invariant = 0;
   double bytes_variant = 0, bytes_invariant = 0;
   int32_t n_nodes = 0, n_variant_nodes = 0;
+  // filled when make_plan is asked to (want_labels): the index labels of every launched node's
+  // output tensor, in step order -- the tensors Eq. 4 sums over (used by the branching driver)
+  std::vector<std::vector<int32_t>> node_labels;
 };
 
 // Returns 0 or a bbtn_status value; err receives the message.
 // force_mode: 0 = automatic, 1 = never use the tiled GEMM path, 2 = use it wherever |K| >= 1.
 // enforce_cap: fail with ESHAPE when a tensor exceeds P.max_elements (otherwise only rho records it).
+// single_arena: place every tensor in the leaf-variant arena (one-leaf plans of the branching driver,
+// which reuse one device buffer across different fixed sets).  want_labels: fill Plan::node_labels.
 int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mode, bool enforce_cap,
-              Plan &out, std::string &err);
+              Plan &out, std::string &err, bool single_arena = false, bool want_labels = false);
 
 // Elimination-order tree for the network with `fixed` sliced out (used when the caller gave no tree).
 void derive_tree(const Problem &P, const std::vector<int32_t> &fixed,

@@ -87,10 +87,29 @@ def solve_king_bb(L, seed=1, block=4, chunk=4, max_batch=1024):
             "contract_calls": out["calls"]}
 
 
+def solve_king_bbtn(L, seed=1, log2_target=31, crt=True):
+    """BBTN proper (bbtn_solve_branching): rho-driven non-uniform branching, T_target = 2^log2_target elements."""
+    k = I.kings_subgraph(L, L, 0.8, seed)
+    h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT if crt else 0)
+    t0 = time.perf_counter()
+    out = h.solve_branching(log2_target)
+    dt = time.perf_counter() - t0
+    h.close()
+    cnt = bb.crt_combine(out["count"], *out["count_mod"]) if crt else out["count"]
+    rings = 3 if crt else 1
+    return {"instance": f"king {L}x{L} p0.8 seed {seed}", "mode": f"BBTN branching on rho (Eq. 4), T_target = 2^{log2_target}"
+            + (", counts mod 2^64, p1, p2 (3 passes) CRT-combined" if crt else ""),
+            "n_vertices": k.n_vertices, "n_edges": k.n_edges, "seconds": dt, "energy": out["energy"],
+            "count_mod_2_64": out["count"], "count": str(cnt), "rho_root": out["rho_root"], "branch_nodes": out["branch_nodes"],
+            "leaves": out["leaves"], "max_fixed": out["max_fixed"], "fma": out["fma"] * rings, "bytes": out["bytes"] * rings,
+            "algorithmic_gb_per_s": out["bytes"] * rings / dt / 1e9}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", nargs="*", default=["1", "2", "3", "4b", "5"])
     ap.add_argument("--king-sizes", nargs="*", type=int, default=[16, 20, 24])
+    ap.add_argument("--bbtn", nargs="*", default=[], help="L:seed:log2_target[:crt] runs of bbtn_solve_branching, e.g. 32:1:31:1")
     ap.add_argument("--repeat", type=int, default=5)
     a = ap.parse_args()
     bb.load()
@@ -116,6 +135,9 @@ def main():
     if "5" in a.configs:
         for L in a.king_sizes:
             emit(solve_king_bb(L))
+    for spec in a.bbtn:
+        f = [int(x) for x in spec.split(":")]
+        emit(solve_king_bbtn(f[0], f[1], f[2], crt=bool(f[3]) if len(f) > 3 else False))
 
 
 if __name__ == "__main__":

@@ -1,7 +1,7 @@
 """Writes tests/golden/config_goldens.json: exact (energy, count) of the BASELINE.json configs at FULL size,
 computed by the oracle alone (oracle.frontier_dp, the tree-free transfer-matrix method; SURVEY.md 8(c) Oracle-3).
 
-    python tests/golden/make_config_goldens.py [out.json]   # minutes of CPU (OpenMP over the host cores)
+    python tests/golden/make_config_goldens.py [out.json] [--missing-only]   # minutes of CPU (OpenMP over the host cores)
 
 Nothing here touches the CUDA path: the GPU parity tests read the file this script writes.
 Instances come from the seeded generators (paper_2602_05470_b200/instances.py holds no arithmetic of the method).
@@ -26,24 +26,40 @@ CASES = [
     ("config5-shape king 20x20 p0.8 seed 1", lambda: I.kings_subgraph(20, 20, 0.8, 1)),
     ("config5-shape king 24x24 p0.8 seed 1", lambda: I.kings_subgraph(24, 24, 0.8, 1)),
 ]
+# King's subgraphs whose dense frontier table would not fit: oracle.frontier_dp_mis_sparse (independent
+# frontier states only); 28x28 6 s, 32x32 ~1.5 min, 36x36 ~8 min, 40x40 longer (one core each)
+SPARSE_CASES = [
+    ("config5-shape king 28x28 p0.8 seed 1", lambda: I.kings_subgraph(28, 28, 0.8, 1)),
+    ("config5-shape king 32x32 p0.8 seed 1", lambda: I.kings_subgraph(32, 32, 0.8, 1)),
+    ("config5-shape king 32x32 p0.8 seed 2", lambda: I.kings_subgraph(32, 32, 0.8, 2)),
+    ("config5-shape king 36x36 p0.8 seed 1", lambda: I.kings_subgraph(36, 36, 0.8, 1)),
+    ("config5 king 40x40 p0.8 seed 1", lambda: I.kings_subgraph(40, 40, 0.8, 1)),
+]
 
 
 def main():
     oracle.build()
-    out = {"_about": "exact results of oracle.frontier_dp on the seeded full-size instances; written by "
+    out = {"_about": "exact results of oracle.frontier_dp (King's subgraphs of 28x28 and more: oracle.frontier_dp_mis_sparse) on the seeded full-size instances; written by "
                      "tests/golden/make_config_goldens.py (calls only oracle/). energy: Ising min H (Eq. 1, PAPER.md:47), "
                      "MIS max set size (PAPER.md:55); count as a decimal string (may exceed 2^64).", "cases": {}}
-    for name, make in CASES:
+    dst = [a for a in sys.argv[1:] if not a.startswith("--")]
+    dst = dst[0] if dst else os.path.join(os.path.dirname(os.path.abspath(__file__)), "config_goldens.json")
+    if "--missing-only" in sys.argv and os.path.exists(dst):      # keep what is there, add the cases not yet in the file
+        with open(dst) as f:
+            out["cases"] = json.load(f)["cases"]
+    todo = [(n, m, oracle.frontier_dp) for n, m in CASES] + [(n, m, oracle.frontier_dp_mis_sparse) for n, m in SPARSE_CASES]
+    for name, make, method in todo:
+        if name in out["cases"]:
+            continue
         inst = make()
         t0 = time.perf_counter()
-        e, c = oracle.frontier_dp(inst)[:2]
+        e, c = method(inst)[:2]
         dt = time.perf_counter() - t0
         out["cases"][name] = {"energy": int(e), "count": str(int(c)), "n_vertices": int(inst.n_vertices),
                               "n_edges": int(inst.n_edges), "oracle_seconds": round(dt, 2)}
         print(name, e, c, f"{dt:.1f}s", flush=True)
-    dst = sys.argv[1] if len(sys.argv) > 1 else os.path.join(os.path.dirname(os.path.abspath(__file__)), "config_goldens.json")
-    with open(dst, "w") as f:
-        json.dump(out, f, indent=1)
+        with open(dst, "w") as f:                                   # after every case: the long ones can be interrupted
+            json.dump(out, f, indent=1)
 
 
 if __name__ == "__main__":

@@ -130,3 +130,46 @@ def test_crt_combine_host():
     for x in (0, 1, 2 ** 64 - 1, 2 ** 64 + 12345, 3 ** 70, 2 ** 125 + 7):
         got = bb.crt_combine(x % 2 ** 64, x % bb.BBTN_P1, x % bb.BBTN_P2)
         assert got == x
+
+
+# ---- branching driver (host side of BBTN proper): rho-driven non-uniform leaves ----
+@pytest.mark.parametrize("name,make,t", [
+    ("king8", lambda: I.kings_subgraph(8, 8, 0.8, 1), 5),
+    ("king10", lambda: I.kings_subgraph(10, 10, 0.8, 2), 6),
+    ("king7w", lambda: I.kings_subgraph(7, 6, 0.9, 3), 6),
+    ("ising5", lambda: I.ising_lattice_2d(5, 5, 3), 3),
+    ("cube3", lambda: I.ising_lattice_3d(3, 3, 3, 2), 5),
+])
+def test_branching_leaves_are_complete_and_orthogonal(lib, oracle, name, make, t):
+    """the decomposition must be complete and orthogonal, so the (+) over the leaves -- each
+    evaluated by the ORACLE here -- reproduces the unbranched result; every leaf obeys rho = 0 (Eq. 4)."""
+    inst = make()
+    h = bb.Handle(inst)
+    leaves, st = h.branching_leaves(t)
+    assert st["rho_root"] > 0 and st["leaves"] == len(leaves) == st["branch_nodes"] + 1
+    res = []
+    for f, x in leaves:
+        assert len(set(f.tolist())) == len(f)
+        res.append(oracle.frontier_dp(inst, fixed=f, assign=x))
+    if inst.kind == "mis":                                     # MIS rules fix different subsets in different branches
+        assert len({tuple(sorted(f.tolist())) for f, _ in leaves}) > 1
+    tot = (oracle.oplus_max if inst.kind == "mis" else oracle.oplus_min)(res)
+    assert tuple(tot) == tuple(oracle.frontier_dp(inst))
+    # orthogonality stated directly: any two leaves disagree on a vertex both fix
+    for i in range(len(leaves)):
+        for j in range(i + 1, len(leaves)):
+            a = dict(zip(leaves[i][0].tolist(), leaves[i][1].tolist()))
+            assert any(v in a and a[v] != x for v, x in zip(leaves[j][0].tolist(), leaves[j][1].tolist()))
+    h.close()
+
+
+def test_branching_target_above_width_is_one_leaf_and_guards(lib):
+    inst = I.kings_subgraph(8, 8, 0.8, 1)
+    h = bb.Handle(inst)
+    leaves, st = h.branching_leaves(20)
+    assert st["leaves"] == 1 and st["rho_root"] == 0 and len(leaves[0][0]) == 0
+    with pytest.raises(bb.BbtnError):
+        h.branching_leaves(3, max_leaves=2)            # needs more leaves than allowed -> ESHAPE
+    with pytest.raises(bb.BbtnError):
+        h.branching_leaves(0)                          # log2_target out of range
+    h.close()

@@ -409,3 +409,49 @@ def test_config1_config2_full_size_goldens(bb):
         assert (int(e[0]), int(c[0])) == _expect(f"config1 ising 6x6 seed {seed}")
     e, c = bb.Handle(I.kings_subgraph(12, 12, 0.8, 1)).contract_batch()
     assert (int(e[0]), int(c[0])) == _expect("config2 king 12x12 p0.8 seed 1")
+
+
+# ---- BBTN proper: rho-driven non-uniform branching (bbtn_solve_branching), leaves of different fixed sets ----
+@pytest.mark.parametrize("name,make,t,flags", [
+    ("king10", lambda: I.kings_subgraph(10, 10, 0.8, 2), 6, 0),
+    ("king12", lambda: I.kings_subgraph(12, 12, 0.8, 3), 7, 0),
+    ("king9-crt", lambda: I.kings_subgraph(9, 9, 1.0, 0), 5, 1),
+    ("ising6", lambda: I.ising_lattice_2d(6, 6, 4), 3, 0),
+    ("cube3-crt", lambda: I.ising_lattice_3d(3, 3, 3, 2), 5, 1),
+])
+def test_solve_branching_matches_oracle(bb, oracle, name, make, t, flags):
+    inst = make()
+    ref_e, ref_c = oracle.frontier_dp(inst)
+    h = bb.Handle(inst, flags=flags)
+    out = h.solve_branching(t)
+    assert out["rho_root"] > 0 and out["leaves"] > 1
+    assert (out["energy"], out["count"]) == (ref_e, ref_c & MASK64)
+    if flags:
+        assert out["count_mod"] == (ref_c % 2147483647, ref_c % 2147483629)
+    one = h.solve_branching(24)                    # target above the width: a single unbranched leaf
+    assert one["leaves"] == 1 and (one["energy"], one["count"]) == (ref_e, ref_c & MASK64)
+    h.close()
+
+
+def test_solve_branching_king28_rank30_leaf(bb):
+    # one rank-30 leaf (12.9 GB tensors, 0.46 TB streamed): element offsets beyond 2^30
+    h = bb.Handle(I.kings_subgraph(28, 28, 0.8, 1))
+    out = h.solve_branching(30)
+    assert out["leaves"] == 1
+    assert (out["energy"], out["count"]) == _expect("config5-shape king 28x28 p0.8 seed 1")
+    out = h.solve_branching(28)                    # two leaves of different fixed sets
+    assert out["leaves"] == 2
+    assert (out["energy"], out["count"]) == _expect("config5-shape king 28x28 p0.8 seed 1")
+    h.close()
+
+
+def test_solve_branching_king32_seed2_rank31_crt(bb):
+    # T_target = 2^31 as in the paper: one unbranched rank-31 leaf, count 5.3e24 > 2^64 via CRT
+    g = _goldens()["config5-shape king 32x32 p0.8 seed 2"]
+    h = bb.Handle(I.kings_subgraph(32, 32, 0.8, 2), flags=1)
+    out = h.solve_branching(31)
+    c = int(g["count"])
+    assert out["leaves"] == 1 and out["energy"] == int(g["energy"]) and out["count"] == c & MASK64
+    assert out["count_mod"] == (c % 2147483647, c % 2147483629)
+    assert bb.crt_combine(out["count"], *out["count_mod"]) == c
+    h.close()

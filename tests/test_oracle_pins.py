@@ -390,3 +390,43 @@ def test_rho_eq4(oracle):
     # Eq. 4: rho = sum_T max(0, log2|T| - log2 T_target)
     assert oracle.rho([10, 31, 33, 35, 2], 31) == 2 + 4
     assert oracle.rho([5, 6], 31) == 0
+
+
+# ---- oracle-3, sparse MIS form (only independent frontier states stored) ------------------------
+@pytest.mark.parametrize("L,p,seed", [(3, 1.0, 1), (4, 1.0, 1), (5, 0.8, 1), (4, 0.7, 2), (3, 0.5, 3)])
+def test_sparse_mis_dp_equals_exhaustive(oracle, L, p, seed):
+    inst = I.kings_subgraph(L, L + 1, p, seed)          # <= 24 vertices: the definition itself
+    assert oracle.frontier_dp_mis_sparse(inst) == oracle.exhaustive(inst)
+
+
+@pytest.mark.parametrize("case", GOLD["kings_full"], ids=lambda c: f"L{c['L']}")
+def test_sparse_mis_dp_full_kings_closed_form(oracle, case):
+    # north_star: a full odd-L King's grid has MIS size ((L+1)/2)^2 and count 1; 4x4 -> (4, 79)
+    inst = I.kings_subgraph(case["L"], case["L"], 1.0, 0)
+    assert oracle.frontier_dp_mis_sparse(inst) == (case["size"], case["count"])
+
+
+@pytest.mark.parametrize("L", [9, 11, 13])
+def test_sparse_mis_dp_odd_full_grid(oracle, L):
+    inst = I.kings_subgraph(L, L, 1.0, 0)
+    assert oracle.frontier_dp_mis_sparse(inst) == (((L + 1) // 2) ** 2, 1)
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_sparse_mis_dp_equals_dense_dp_orders_weights_and_slices(oracle, seed):
+    inst = I.kings_subgraph(7 + seed, 9, 0.8, seed)
+    inst.vertex_w = (1 + (I.splitmix64(seed, inst.n_vertices, 7) % 3)).astype(np.int32)   # MWIS weights 1..3
+    order = np.arange(inst.n_vertices, dtype=np.int32)[::-1].copy() if seed % 2 else None     # a second sweep direction
+    assert oracle.frontier_dp_mis_sparse(inst, order=order) == oracle.frontier_dp(inst)
+    fixed = I.random_order(inst.n_vertices, 100 + seed)[:5]
+    for x in I.all_assignments(5)[:: 7]:
+        assert oracle.frontier_dp_mis_sparse(inst, fixed=fixed, assign=x) == oracle.frontier_dp(inst, fixed=fixed, assign=x)
+
+
+def test_sparse_mis_dp_path_and_cycle(oracle):
+    # P_n: size ceil(n/2), count 1 (n odd) or n/2+1 (n even);  C_n: (n/2, 2) n even, ((n-1)/2, n) n odd
+    for n in (7, 10, 31, 40):
+        path = _inst("mis", n, [(i, i + 1) for i in range(n - 1)], None, None)
+        assert oracle.frontier_dp_mis_sparse(path) == ((n + 1) // 2, 1 if n % 2 else n // 2 + 1)
+        cyc = _inst("mis", n, [(i, (i + 1) % n) for i in range(n)], None, None)
+        assert oracle.frontier_dp_mis_sparse(cyc) == ((n // 2, 2) if n % 2 == 0 else ((n - 1) // 2, n))
