@@ -11,11 +11,15 @@ namespace {
 
 enum { ST_EINVAL = 1, ST_ESHAPE = 4 };
 
-// First-fit free-list allocator over element offsets (sizes are powers of two).
+// First-fit free-list allocator over element offsets (sizes are powers of two).  Every block is a
+// multiple of 4 elements, so every tensor starts 16-byte aligned in both planes (the vectorised kernels
+// need that; a 2-element bond tensor in front of a 2^31-element one must not push it off alignment).
 struct Arena {
   std::map<int64_t, int64_t> free_;   // offset -> size
   int64_t top = 0;                    // high-water mark
+  static int64_t round4(int64_t n) { return (n + 3) & ~(int64_t)3; }
   int64_t alloc(int64_t n) {
+    n = round4(n);
     for (auto it = free_.begin(); it != free_.end(); ++it) {
       if (it->second >= n) {
         int64_t off = it->first, rest = it->second - n;
@@ -39,6 +43,7 @@ struct Arena {
     return off;
   }
   void release(int64_t off, int64_t n) {
+    n = round4(n);
     auto it = free_.emplace(off, n).first;
     auto nx = std::next(it);
     if (nx != free_.end() && it->first + it->second == nx->first) { it->second += nx->second; free_.erase(nx); }
