@@ -24,7 +24,8 @@ namespace {
 enum LowPattern : int { LP_FAR = 0, LP_K0 = 1, LP_K1 = 2 };
 
 struct AbsorbVecArgs {
-  int rO, nK, tb;                 // output rank, summed bits, tile bits (<= 12)
+  int rO, nK, tb;                 // rank of the output WITHOUT its folded top bits, summed bits, tile bits (<= 12)
+  uint32_t foldB[4];              // offset into B of each combination of the folded (new, B-only) top output bits
   uint32_t addA[32], addB[32];    // per output bit
   uint32_t kA[8], kB[8];          // per summed bit
   int64_t sA, sB, sC, n_tiles;    // batch strides (elements), tiles over all batch entries
@@ -56,13 +57,18 @@ __device__ __forceinline__ void load_e4(const int32_t *p, int32_t *d) {
   d[0] = a.x; d[1] = a.y; d[2] = a.z; d[3] = a.w;
 }
 
-template <class R, int LP>
+// NF = number of FOLDED output bits: the planner puts the indices that only B carries (the new legs) at the
+// top of the output, where A's address does not depend on them.  One thread produces all 2^NF outputs that
+// share an element of A from a single read of A -- otherwise a node that grows the tensor reads A 2^NF times
+// from DRAM (the re-reads lie 2^(rO-NF) elements apart, far beyond any cache).
+template <class R, int LP, int NF>
 __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const int32_t *__restrict__ Ae,
                                                          const typename R::T *__restrict__ Ac,
                                                          const int32_t *__restrict__ Be, const typename R::T *__restrict__ Bc,
                                                          int32_t *__restrict__ Ce, typename R::T *__restrict__ Cc) {
   using CT = typename R::T;
   constexpr int VPT = 4;                                    // vectors per thread in a full 4096-output tile
+  constexpr int NFV = 1 << NF;
   const int nvec = 1 << (p.tb - 2);
   // per-thread part of the addresses: output bits 2 .. tb-1
   uint32_t ta[VPT], tbo[VPT];
@@ -76,6 +82,9 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
   const uint32_t ub1 = p.addB[0], ub2 = p.addB[1];
   const int tiles_per_entry_lg = p.rO - p.tb;
   const int n_k = 1 << p.nK;
+  uint32_t fb[NFV];
+#pragma unroll
+  for (int f = 0; f < NFV; f++) fb[f] = p.foldB[f];
 
   for (int64_t t = blockIdx.x; t < p.n_tiles; t += gridDim.x) {
     const int64_t b = t >> tiles_per_entry_lg;
@@ -89,9 +98,11 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
     for (int j = 0; j < VPT; j++) {
       const int v = threadIdx.x + 256 * j;
       if (v >= nvec) break;
-      int32_t acc_e[4]; CT acc_c[4];
+      int32_t acc_e[NFV][4]; CT acc_c[NFV][4];
 #pragma unroll
-      for (int u = 0; u < 4; u++) { acc_e[u] = NEG_INF; acc_c[u] = 0; }
+      for (int f = 0; f < NFV; f++)
+#pragma unroll
+        for (int u = 0; u < 4; u++) { acc_e[f][u] = NEG_INF; acc_c[f][u] = 0; }
       if (LP == LP_FAR) {
         for (int k = 0; k < n_k; k++) {
           uint32_t ka = 0, kb = 0;
@@ -99,10 +110,12 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
           int32_t e4[4]; V4<CT> c4;
           load_e4(ae + ta[j] + ka, e4); c4.load(ac + ta[j] + ka);
 #pragma unroll
-          for (int u = 0; u < 4; u++) {
-            const uint32_t ib = tbo[j] + kb + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-            oplus<R>(acc_e[u], acc_c[u], e4[u] + be[ib], R::mul(c4.v[u], bc[ib]));
-          }
+          for (int f = 0; f < NFV; f++)
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+              const uint32_t ib = tbo[j] + kb + fb[f] + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+              oplus<R>(acc_e[f][u], acc_c[f][u], e4[u] + be[ib], R::mul(c4.v[u], bc[ib]));
+            }
         }
       } else {
         // nK == 1 and the summed index is A's bit 0 (K0) or bit 1 (K1): 8 consecutive elements of A
@@ -110,20 +123,26 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
         load_e4(ae + ta[j], e8); load_e4(ae + ta[j] + 4, e8 + 4);
         c8[0].load(ac + ta[j]); c8[1].load(ac + ta[j] + 4);
 #pragma unroll
-        for (int u = 0; u < 4; u++)
+        for (int f = 0; f < NFV; f++)
 #pragma unroll
-          for (int k = 0; k < 2; k++) {
-            // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
-            const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
-            const uint32_t ib = tbo[j] + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-            oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], bc[ib]));
-          }
+          for (int u = 0; u < 4; u++)
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+              // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
+              const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
+              const uint32_t ib = tbo[j] + fb[f] + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+              oplus<R>(acc_e[f][u], acc_c[f][u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], bc[ib]));
+            }
       }
-      V4<CT> oc;
 #pragma unroll
-      for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[u], acc_c[u]); oc.v[u] = acc_c[u]; }
-      *reinterpret_cast<int4 *>(ce + 4 * v) = make_int4(acc_e[0], acc_e[1], acc_e[2], acc_e[3]);
-      oc.store(cc + 4 * v);
+      for (int f = 0; f < NFV; f++) {
+        V4<CT> oc;
+#pragma unroll
+        for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[f][u], acc_c[f][u]); oc.v[u] = acc_c[f][u]; }
+        const int64_t fo = ((int64_t)f << p.rO) + 4 * v;
+        *reinterpret_cast<int4 *>(ce + fo) = make_int4(acc_e[f][0], acc_e[f][1], acc_e[f][2], acc_e[f][3]);
+        oc.store(cc + fo);
+      }
     }
   }
 }
@@ -147,27 +166,38 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
 #ifdef BBTN_TRACE_LP
   fprintf(stderr, "LP %d ring %d nK %d rO %d\n", lp, ring, s.nK, s.rO);
 #endif
+  // fold the top output bits that only B carries (see the kernel comment); keep >= 4 unfolded bits
+  int nF = 0;
+  while (nF < 2 && s.rO - nF > 4 && s.addA[s.rO - 1 - nF] == 0u) nF++;
+  const int rOe = s.rO - nF;
   AbsorbVecArgs p;
-  p.rO = s.rO; p.nK = s.nK; p.tb = s.rO < 12 ? s.rO : 12;
+  p.rO = rOe; p.nK = s.nK; p.tb = rOe < 12 ? rOe : 12;
   for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
   for (int i = 0; i < 8; i++) { p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
+  for (int f = 0; f < 4; f++) {
+    p.foldB[f] = 0;
+    for (int i = 0; i < nF; i++) if ((f >> i) & 1) p.foldB[f] += s.addB[rOe + i];
+  }
   // the 16-byte reads of A must stay 4-element aligned: every offset that can be added is a multiple of 4
   for (int q = 2; q < s.rO; q++) if (p.addA[q] & 3u) return false;
   p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
   p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
   p.sC = (int64_t)1 << s.rO;
-  p.n_tiles = nb << (s.rO - p.tb);
+  p.n_tiles = nb << (rOe - p.tb);
   const int64_t cap = 148 * 8;
   const int grid = (int)(p.n_tiles < cap ? p.n_tiles : cap);
+#define BBTN_ABSORB_LAUNCH(LPV, NFV_)                                                                               \
+  absorb_vec_kernel<R, LPV, NFV_><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc)
+#define BBTN_ABSORB_NF(LPV)                                                                                         \
+  do { if (nF == 0) BBTN_ABSORB_LAUNCH(LPV, 0); else if (nF == 1) BBTN_ABSORB_LAUNCH(LPV, 1); else BBTN_ABSORB_LAUNCH(LPV, 2); } while (0)
   BBTN_RING_DISPATCH(ring, {
     using CT = typename R::T;
-    if (lp == LP_FAR)
-      absorb_vec_kernel<R, LP_FAR><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
-    else if (lp == LP_K0)
-      absorb_vec_kernel<R, LP_K0><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
-    else
-      absorb_vec_kernel<R, LP_K1><<<grid, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
+    if (lp == LP_FAR) BBTN_ABSORB_NF(LP_FAR);
+    else if (lp == LP_K0) BBTN_ABSORB_NF(LP_K0);
+    else BBTN_ABSORB_NF(LP_K1);
   });
+#undef BBTN_ABSORB_NF
+#undef BBTN_ABSORB_LAUNCH
   return true;
 }
 
