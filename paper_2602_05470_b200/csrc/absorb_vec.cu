@@ -34,13 +34,13 @@ struct AbsorbVecArgs {
 template <class CT> struct V4;
 template <> struct V4<uint64_t> {
   uint64_t v[4];
+  // 32-byte global accesses (LDG.E.256 / STG.E.256, new on sm_100): one full 32-byte sector per thread instead
+  // of two half-filled ones per instruction
   __device__ __forceinline__ void load(const uint64_t *p) {
-    const ulonglong2 a = *reinterpret_cast<const ulonglong2 *>(p), b = *reinterpret_cast<const ulonglong2 *>(p + 2);
-    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+    asm("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(v[0]), "=l"(v[1]), "=l"(v[2]), "=l"(v[3]) : "l"(p));
   }
   __device__ __forceinline__ void store(uint64_t *p) const {
-    *reinterpret_cast<ulonglong2 *>(p) = make_ulonglong2(v[0], v[1]);
-    *reinterpret_cast<ulonglong2 *>(p + 2) = make_ulonglong2(v[2], v[3]);
+    asm volatile("st.global.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(v[0]), "l"(v[1]), "l"(v[2]), "l"(v[3]));
   }
 };
 template <> struct V4<uint32_t> {
@@ -148,6 +148,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
 }
 
 inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+inline bool al32(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 31) == 0; }
 
 }  // namespace
 
@@ -156,6 +157,7 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
                        int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
   if (s.rO < 4 || s.nK > 3 || s.rA < 3) return false;
   if (!al16(Ae) || !al16(Ac) || !al16(Ce) || !al16(Cc)) return false;
+  if (ring == RING_U64 && (!al32(Ac) || !al32(Cc))) return false;       // 32-byte count vectors
   int lp;
   if (s.addA[0] == 1u && s.addA[1] == 2u) {
     lp = LP_FAR;

@@ -455,3 +455,13 @@ def test_solve_branching_king32_seed2_rank31_crt(bb):
     assert out["count_mod"] == (c % 2147483647, c % 2147483629)
     assert bb.crt_combine(out["count"], *out["count_mod"]) == c
     h.close()
+
+
+def test_solve_branching_king32_seed1_rank32_leaves(bb):
+    # T_target = 2^32: four leaves of different fixed sets, rank-32 tensors (51.5 GB each, 129 GB arena --
+    # if less device memory is free the driver keeps branching, the result is the same)
+    h = bb.Handle(I.kings_subgraph(32, 32, 0.8, 1))
+    out = h.solve_branching(32)
+    assert out["leaves"] >= 4 and out["rho_root"] == 5
+    assert (out["energy"], out["count"]) == _expect("config5-shape king 32x32 p0.8 seed 1")
+    h.close()
