@@ -19,7 +19,16 @@ struct RingU64 {
 template <uint32_t P>
 struct RingMod {
   using T = uint32_t;
-  static __device__ __forceinline__ T mul(T a, T b) { return (T)(((uint64_t)a * b) % P); }
+  // P = 2^31 - C with a small C (1 and 19 for the two primes), so 2^31 == C (mod P): fold the high part of the
+  // 62-bit product down twice instead of dividing.  x = hi*2^31 + lo  ->  hi*C + lo < (C+1)*2^31  ->  < 2^31 + C*(C+1).
+  static constexpr uint32_t C = 0x80000000u - P;
+  static_assert(C >= 1 && C <= 64, "RingMod expects a prime just below 2^31");
+  static __device__ __forceinline__ T mul(T a, T b) {
+    const uint64_t x = (uint64_t)a * b;                                   // a, b < P  =>  x < 2^62
+    const uint64_t y = (uint64_t)(uint32_t)(x >> 31) * C + ((uint32_t)x & 0x7fffffffu);
+    const uint32_t z = (uint32_t)(y >> 31) * C + ((uint32_t)y & 0x7fffffffu);   // < 2^31 + C*(C+1) < 2P
+    return z >= P ? z - P : z;
+  }
   static __device__ __forceinline__ T add(T a, T b) { uint32_t s = a + b; return s >= P ? s - P : s; }   // a,b < 2^31
   static __device__ __forceinline__ T from_small(uint32_t x) { return x % P; }
 };
