@@ -218,8 +218,9 @@ int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,
                                int32_t count_bits, void *cuda_stream);
 
 /* Same operation with HOST pointers (the end-to-end form of the config-4 sweep): the operands are
- * copied to library-owned device staging buffers on `cuda_stream` (pass pinned memory for full
- * PCIe speed), K3 runs, C is copied back and the call returns after the results landed.
+ * copied to library-owned device staging buffers, K3 runs, C is copied back and the call returns after
+ * the results landed.  The batch flows in chunks through three internal streams ordered after
+ * `cuda_stream`, so with PINNED host memory the PCIe copies of one chunk overlap the GEMM of another.
  * On BBTN_ECUDA during the copy-back the contents of Ce/Cc are unspecified. */
 int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t K,
                                     const int32_t *Ae, const uint64_t *Ac,

@@ -326,15 +326,61 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
   const size_t nC = (size_t)(batch - 1) * strideC + (size_t)M * N;
   const size_t n[3] = {nA, nB, nC};
   for (int i = 0; i < 3; i++) { CUDA_TRY(nullptr, st_e[i].ensure(n[i] * 4)); CUDA_TRY(nullptr, st_c[i].ensure(n[i] * 8)); }
-  CUDA_TRY(nullptr, cudaMemcpyAsync(st_e[0].p, Ae, nA * 4, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(nullptr, cudaMemcpyAsync(st_c[0].p, Ac, nA * 8, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(nullptr, cudaMemcpyAsync(st_e[1].p, Be, nB * 4, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(nullptr, cudaMemcpyAsync(st_c[1].p, Bc, nB * 8, cudaMemcpyHostToDevice, st));
-  launch_gemm_tiled(batch, 1, M, N, K, 0, (const int32_t *)st_e[0].p, st_c[0].p, (const int32_t *)st_e[1].p, st_c[1].p,
-                    (int32_t *)st_e[2].p, st_c[2].p, strideA, strideB, strideC, RING_U64, count_bits, st);
-  CUDA_TRY(nullptr, cudaGetLastError());
-  CUDA_TRY(nullptr, cudaMemcpyAsync(Ce, st_e[2].p, nC * 4, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(nullptr, cudaMemcpyAsync(Cc, st_c[2].p, nC * 8, cudaMemcpyDeviceToHost, st));
+  // The batch is cut into chunks that flow through three internal streams -- host->device copies, K3, device->host
+  // copies -- so the PCIe transfers of chunk c+1 / c-1 overlap the GEMM of chunk c (pinned host memory needed for
+  // the overlap; pageable memory still works, serialised by the driver).  Shared operands (stride 0) go up once.
+  static thread_local cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
+  static thread_local cudaEvent_t ev_start = nullptr, ev_in[8], ev_k[8], ev_done = nullptr;
+  if (!s_in) {
+    CUDA_TRY(nullptr, cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    CUDA_TRY(nullptr, cudaStreamCreateWithFlags(&s_k, cudaStreamNonBlocking));
+    CUDA_TRY(nullptr, cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+    CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
+    for (int i = 0; i < 8; i++) {
+      CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming));
+      CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming));
+    }
+  }
+  const int n_chunks = (int)std::min<int64_t>(8, std::max<int64_t>(1, batch / 4));   // >= 4 entries per chunk
+  int32_t *dAe = (int32_t *)st_e[0].p, *dBe = (int32_t *)st_e[1].p, *dCe = (int32_t *)st_e[2].p;
+  uint64_t *dAc = (uint64_t *)st_c[0].p, *dBc = (uint64_t *)st_c[1].p, *dCc = (uint64_t *)st_c[2].p;
+  CUDA_TRY(nullptr, cudaEventRecord(ev_start, st));
+  CUDA_TRY(nullptr, cudaStreamWaitEvent(s_in, ev_start, 0));
+  CUDA_TRY(nullptr, cudaStreamWaitEvent(s_out, ev_start, 0));   // earlier work on st may still read the staging buffers
+  if (!strideA) {
+    CUDA_TRY(nullptr, cudaMemcpyAsync(dAe, Ae, (size_t)M * K * 4, cudaMemcpyHostToDevice, s_in));
+    CUDA_TRY(nullptr, cudaMemcpyAsync(dAc, Ac, (size_t)M * K * 8, cudaMemcpyHostToDevice, s_in));
+  }
+  if (!strideB) {
+    CUDA_TRY(nullptr, cudaMemcpyAsync(dBe, Be, (size_t)K * N * 4, cudaMemcpyHostToDevice, s_in));
+    CUDA_TRY(nullptr, cudaMemcpyAsync(dBc, Bc, (size_t)K * N * 8, cudaMemcpyHostToDevice, s_in));
+  }
+  for (int c = 0; c < n_chunks; c++) {
+    const int64_t b0 = batch * c / n_chunks, b1 = batch * (c + 1) / n_chunks, nb = b1 - b0;
+    if (strideA) {
+      const size_t off = (size_t)b0 * strideA, len = (size_t)(nb - 1) * strideA + (size_t)M * K;
+      CUDA_TRY(nullptr, cudaMemcpyAsync(dAe + off, Ae + off, len * 4, cudaMemcpyHostToDevice, s_in));
+      CUDA_TRY(nullptr, cudaMemcpyAsync(dAc + off, Ac + off, len * 8, cudaMemcpyHostToDevice, s_in));
+    }
+    if (strideB) {
+      const size_t off = (size_t)b0 * strideB, len = (size_t)(nb - 1) * strideB + (size_t)K * N;
+      CUDA_TRY(nullptr, cudaMemcpyAsync(dBe + off, Be + off, len * 4, cudaMemcpyHostToDevice, s_in));
+      CUDA_TRY(nullptr, cudaMemcpyAsync(dBc + off, Bc + off, len * 8, cudaMemcpyHostToDevice, s_in));
+    }
+    CUDA_TRY(nullptr, cudaEventRecord(ev_in[c], s_in));
+    CUDA_TRY(nullptr, cudaStreamWaitEvent(s_k, ev_in[c], 0));
+    launch_gemm_tiled(nb, 1, M, N, K, 0, dAe + b0 * strideA, dAc + b0 * strideA, dBe + b0 * strideB, dBc + b0 * strideB,
+                      dCe + b0 * strideC, dCc + b0 * strideC, strideA, strideB, strideC, RING_U64, count_bits, s_k);
+    CUDA_TRY(nullptr, cudaGetLastError());
+    CUDA_TRY(nullptr, cudaEventRecord(ev_k[c], s_k));
+    CUDA_TRY(nullptr, cudaStreamWaitEvent(s_out, ev_k[c], 0));
+    const size_t off = (size_t)b0 * strideC, len = (size_t)(nb - 1) * strideC + (size_t)M * N;
+    CUDA_TRY(nullptr, cudaMemcpyAsync(Ce + off, dCe + off, len * 4, cudaMemcpyDeviceToHost, s_out));
+    CUDA_TRY(nullptr, cudaMemcpyAsync(Cc + off, dCc + off, len * 8, cudaMemcpyDeviceToHost, s_out));
+  }
+  CUDA_TRY(nullptr, cudaEventRecord(ev_done, s_out));
+  CUDA_TRY(nullptr, cudaStreamWaitEvent(st, ev_done, 0));
   CUDA_TRY(nullptr, cudaStreamSynchronize(st));
   return BBTN_OK;
 }

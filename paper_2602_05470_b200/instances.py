@@ -93,6 +93,15 @@ def ising_lattice_2d(rows: int, cols: int, seed: int, field_h: int = 0,
                     {"shape": (rows, cols), "seed": seed})
 
 
+def ising_lattice_2d_half_field(rows: int, cols: int, seed: int) -> Instance:
+    """The paper's spin-glass setting (J = +-1 at random, external field 0.5) in integers
+    (reading A6): every coupling doubled, h = 1, energies come out in HALF units."""
+    inst = ising_lattice_2d(rows, cols, seed, field_h=1)
+    inst.edge_w = (2 * inst.edge_w).astype(np.int32)
+    inst.meta["energy_unit"] = 0.5
+    return inst
+
+
 def ising_lattice_3d(lx: int, ly: int, lz: int, seed: int) -> Instance:
     """Open-boundary cubic +-J lattice, id = (z*ly + y)*lx + x, bonds +x, +y, +z per site."""
     eu, ev = [], []

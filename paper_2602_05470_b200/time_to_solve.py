@@ -105,11 +105,26 @@ def solve_king_bbtn(L, seed=1, log2_target=31, crt=True):
             "algorithmic_gb_per_s": out["bytes"] * rings / dt / 1e9}
 
 
+def solve_e1(L, seed=1, log2_target=32):
+    """The paper's spin-glass setting (+-J, field 0.5 -> 2J, h = 1, half units) unbranched: one leaf of width L+1."""
+    inst = I.ising_lattice_2d_half_field(L, L, seed)
+    h = bb.Handle(inst)
+    t0 = time.perf_counter()
+    out = h.solve_branching(log2_target)
+    dt = time.perf_counter() - t0
+    h.close()
+    return {"instance": f"paper-E1 ising {L}x{L} seed {seed} h=0.5 (2J, h=1)", "mode": f"bbtn_solve_branching, T_target = 2^{log2_target}",
+            "n_vertices": inst.n_vertices, "n_edges": inst.n_edges, "seconds": dt, "energy_half_units": out["energy"],
+            "energy": out["energy"] / 2, "count_mod_2_64": out["count"], "leaves": out["leaves"], "rho_root": out["rho_root"],
+            "fma": out["fma"], "bytes": out["bytes"], "algorithmic_gb_per_s": out["bytes"] / dt / 1e9}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--configs", nargs="*", default=["1", "2", "3", "4b", "5"])
     ap.add_argument("--king-sizes", nargs="*", type=int, default=[16, 20, 24])
     ap.add_argument("--bbtn", nargs="*", default=[], help="L:seed:log2_target[:crt] runs of bbtn_solve_branching, e.g. 32:1:31:1")
+    ap.add_argument("--e1", nargs="*", type=int, default=[], help="lattice sizes L for the paper's +-J, h = 0.5 setting, unbranched")
     ap.add_argument("--repeat", type=int, default=5)
     a = ap.parse_args()
     bb.load()
@@ -135,6 +150,8 @@ def main():
     if "5" in a.configs:
         for L in a.king_sizes:
             emit(solve_king_bb(L))
+    for L in a.e1:
+        emit(solve_e1(L))
     for spec in a.bbtn:
         f = [int(x) for x in spec.split(":")]
         emit(solve_king_bbtn(f[0], f[1], f[2], crt=bool(f[3]) if len(f) > 3 else False))

@@ -25,6 +25,10 @@ CASES = [
     ("config5-shape king 16x16 p0.8 seed 1", lambda: I.kings_subgraph(16, 16, 0.8, 1)),
     ("config5-shape king 20x20 p0.8 seed 1", lambda: I.kings_subgraph(20, 20, 0.8, 1)),
     ("config5-shape king 24x24 p0.8 seed 1", lambda: I.kings_subgraph(24, 24, 0.8, 1)),
+    # the paper's own spin-glass setting (+-J with field 0.5), in integers: J -> 2J, h -> 1, half units
+    ("paper-E1 ising 16x16 seed 1 h=0.5 (2J, h=1, half units)", lambda: I.ising_lattice_2d_half_field(16, 16, 1)),
+    ("paper-E1 ising 20x20 seed 1 h=0.5 (2J, h=1, half units)", lambda: I.ising_lattice_2d_half_field(20, 20, 1)),
+    ("paper-E1 ising 24x24 seed 1 h=0.5 (2J, h=1, half units)", lambda: I.ising_lattice_2d_half_field(24, 24, 1)),
 ]
 # King's subgraphs whose dense frontier table would not fit: oracle.frontier_dp_mis_sparse (independent
 # frontier states only); 28x28 6 s, 32x32 ~1.5 min, 36x36 ~8 min, 40x40 longer (one core each)

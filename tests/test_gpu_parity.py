@@ -465,3 +465,18 @@ def test_solve_branching_king32_seed1_rank32_leaves(bb):
     assert out["leaves"] >= 4 and out["rho_root"] == 5
     assert (out["energy"], out["count"]) == _expect("config5-shape king 32x32 p0.8 seed 1")
     h.close()
+
+
+@pytest.mark.parametrize("L", [16, 20, 24])
+def test_paper_e1_spin_glass_with_half_field(bb, L):
+    # +-J with external field 0.5, in integers (J -> 2J, h -> 1, half units; reading A6): one unbranched
+    # leaf through bbtn_solve_branching, and all 2^8 leaves of a slit through bbtn_contract_batch
+    inst = I.ising_lattice_2d_half_field(L, L, 1)
+    want = _expect(f"paper-E1 ising {L}x{L} seed 1 h=0.5 (2J, h=1, half units)")
+    h = bb.Handle(inst)
+    out = h.solve_branching(31)
+    assert out["leaves"] == 1 and (out["energy"], out["count"]) == want
+    fixed = I.slit_fixed_set_2d(L, L, 8)
+    e, c = h.contract_batch(fixed, I.all_assignments(8))
+    assert bb.oplus_combine("ising", e, c)[:2] == want
+    h.close()
