@@ -98,12 +98,12 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
     for (int j = 0; j < VPT; j++) {
       const int v = threadIdx.x + 256 * j;
       if (v >= nvec) break;
-      int32_t acc_e[NFV][4]; CT acc_c[NFV][4];
-#pragma unroll
-      for (int f = 0; f < NFV; f++)
-#pragma unroll
-        for (int u = 0; u < 4; u++) { acc_e[f][u] = NEG_INF; acc_c[f][u] = 0; }
       if (LP == LP_FAR) {
+        int32_t acc_e[NFV][4]; CT acc_c[NFV][4];
+#pragma unroll
+        for (int f = 0; f < NFV; f++)
+#pragma unroll
+          for (int u = 0; u < 4; u++) { acc_e[f][u] = NEG_INF; acc_c[f][u] = 0; }
         for (int k = 0; k < n_k; k++) {
           uint32_t ka = 0, kb = 0;
           for (int q = 0; q < p.nK; q++) if ((k >> q) & 1) { ka += p.kA[q]; kb += p.kB[q]; }
@@ -117,31 +117,44 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
               oplus<R>(acc_e[f][u], acc_c[f][u], e4[u] + be[ib], R::mul(c4.v[u], bc[ib]));
             }
         }
+#pragma unroll
+        for (int f = 0; f < NFV; f++) {
+          V4<CT> oc;
+#pragma unroll
+          for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[f][u], acc_c[f][u]); oc.v[u] = acc_c[f][u]; }
+          const int64_t fo = ((int64_t)f << p.rO) + 4 * v;
+          *reinterpret_cast<int4 *>(ce + fo) = make_int4(acc_e[f][0], acc_e[f][1], acc_e[f][2], acc_e[f][3]);
+          oc.store(cc + fo);
+        }
       } else {
-        // nK == 1 and the summed index is A's bit 0 (K0) or bit 1 (K1): 8 consecutive elements of A
+        // nK == 1 and the summed index is A's bit 0 (K0) or bit 1 (K1): 8 consecutive elements of A hold both k of
+        // all 4 outputs.  One folded combination at a time (not unrolled: unrolling hoists the 16 B-operand loads
+        // of every combination and costs 178 registers, one CTA per SM)
         int32_t e8[8]; V4<CT> c8[2];
         load_e4(ae + ta[j], e8); load_e4(ae + ta[j] + 4, e8 + 4);
         c8[0].load(ac + ta[j]); c8[1].load(ac + ta[j] + 4);
+#pragma unroll 1
+        for (int f = 0; f < NFV; f++) {
+          int32_t acc_e[4]; CT acc_c[4];
+          const uint32_t fbf = p.foldB[f];
 #pragma unroll
-        for (int f = 0; f < NFV; f++)
-#pragma unroll
-          for (int u = 0; u < 4; u++)
+          for (int u = 0; u < 4; u++) {
+            acc_e[u] = NEG_INF; acc_c[u] = 0;
 #pragma unroll
             for (int k = 0; k < 2; k++) {
               // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
               const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
-              const uint32_t ib = tbo[j] + fb[f] + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-              oplus<R>(acc_e[f][u], acc_c[f][u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], bc[ib]));
+              const uint32_t ib = tbo[j] + fbf + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+              oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], bc[ib]));
             }
-      }
+          }
+          V4<CT> oc;
 #pragma unroll
-      for (int f = 0; f < NFV; f++) {
-        V4<CT> oc;
-#pragma unroll
-        for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[f][u], acc_c[f][u]); oc.v[u] = acc_c[f][u]; }
-        const int64_t fo = ((int64_t)f << p.rO) + 4 * v;
-        *reinterpret_cast<int4 *>(ce + fo) = make_int4(acc_e[f][0], acc_e[f][1], acc_e[f][2], acc_e[f][3]);
-        oc.store(cc + fo);
+          for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[u], acc_c[u]); oc.v[u] = acc_c[u]; }
+          const int64_t fo = ((int64_t)f << p.rO) + 4 * v;
+          *reinterpret_cast<int4 *>(ce + fo) = make_int4(acc_e[0], acc_e[1], acc_e[2], acc_e[3]);
+          oc.store(cc + fo);
+        }
       }
     }
   }
