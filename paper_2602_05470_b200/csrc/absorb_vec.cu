@@ -99,31 +99,50 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
       const int v = threadIdx.x + 256 * j;
       if (v >= nvec) break;
       if (LP == LP_FAR) {
-        int32_t acc_e[NFV][4]; CT acc_c[NFV][4];
-#pragma unroll
-        for (int f = 0; f < NFV; f++)
-#pragma unroll
-          for (int u = 0; u < 4; u++) { acc_e[f][u] = NEG_INF; acc_c[f][u] = 0; }
-        for (int k = 0; k < n_k; k++) {
-          uint32_t ka = 0, kb = 0;
-          for (int q = 0; q < p.nK; q++) if ((k >> q) & 1) { ka += p.kA[q]; kb += p.kB[q]; }
-          int32_t e4[4]; V4<CT> c4;
-          load_e4(ae + ta[j] + ka, e4); c4.load(ac + ta[j] + ka);
-#pragma unroll
-          for (int f = 0; f < NFV; f++)
-#pragma unroll
-            for (int u = 0; u < 4; u++) {
-              const uint32_t ib = tbo[j] + kb + fb[f] + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-              oplus<R>(acc_e[f][u], acc_c[f][u], e4[u] + be[ib], R::mul(c4.v[u], bc[ib]));
-            }
+        // A's vector(s) stay in registers for nK <= 1 (the common case); the folded combinations run one at a time.
+        // With more summed bits and folded bits (rare) A is simply re-read per combination (L1/L2 hits, no DRAM traffic).
+        const bool in_regs = NF > 0 && p.nK <= 1;      // nothing folded: stream A per k, fewest registers
+        int32_t e4[2][4]; V4<CT> c4[2];
+        if (in_regs) {
+          load_e4(ae + ta[j], e4[0]); c4[0].load(ac + ta[j]);
+          if (p.nK == 1) { load_e4(ae + ta[j] + p.kA[0], e4[1]); c4[1].load(ac + ta[j] + p.kA[0]); }
         }
-#pragma unroll
+#pragma unroll 1
         for (int f = 0; f < NFV; f++) {
+          int32_t acc_e[4]; CT acc_c[4];
+          const uint32_t fbf = p.foldB[f];
+#pragma unroll
+          for (int u = 0; u < 4; u++) { acc_e[u] = NEG_INF; acc_c[u] = 0; }
+          if (in_regs) {
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+              if (k < n_k) {
+                const uint32_t kb = k ? p.kB[0] : 0u;
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                  const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+                  oplus<R>(acc_e[u], acc_c[u], e4[k][u] + be[ib], R::mul(c4[k].v[u], bc[ib]));
+                }
+              }
+            }
+          } else {
+            for (int k = 0; k < n_k; k++) {
+              uint32_t ka = 0, kb = 0;
+              for (int q = 0; q < p.nK; q++) if ((k >> q) & 1) { ka += p.kA[q]; kb += p.kB[q]; }
+              int32_t ex[4]; V4<CT> cx;
+              load_e4(ae + ta[j] + ka, ex); cx.load(ac + ta[j] + ka);
+#pragma unroll
+              for (int u = 0; u < 4; u++) {
+                const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
+                oplus<R>(acc_e[u], acc_c[u], ex[u] + be[ib], R::mul(cx.v[u], bc[ib]));
+              }
+            }
+          }
           V4<CT> oc;
 #pragma unroll
-          for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[f][u], acc_c[f][u]); oc.v[u] = acc_c[f][u]; }
+          for (int u = 0; u < 4; u++) { canonicalise<R>(acc_e[u], acc_c[u]); oc.v[u] = acc_c[u]; }
           const int64_t fo = ((int64_t)f << p.rO) + 4 * v;
-          *reinterpret_cast<int4 *>(ce + fo) = make_int4(acc_e[f][0], acc_e[f][1], acc_e[f][2], acc_e[f][3]);
+          *reinterpret_cast<int4 *>(ce + fo) = make_int4(acc_e[0], acc_e[1], acc_e[2], acc_e[3]);
           oc.store(cc + fo);
         }
       } else {
