@@ -13,7 +13,9 @@ namespace {
 
 constexpr int BM = 64, BN = 64, BK = 16, TM = 4, TN = 4, NT = 256;
 
-template <class R, bool A_KMAJOR>
+// NARROW: both operands' counts are < 2^32 (caller's count_bits <= 32, RING_U64 only), so the
+// product is one 32x32->64 multiply instead of a 64x64->64 one; the result is the same number.
+template <class R, bool A_KMAJOR, bool NARROW = false>
 __global__ void __launch_bounds__(NT) gemm_tiled_kernel(int64_t G, int M, int N, int K,
                                                         const int32_t *__restrict__ Ae, const typename R::T *__restrict__ Ac,
                                                         const int32_t *__restrict__ Be, const typename R::T *__restrict__ Bc,
@@ -72,7 +74,8 @@ __global__ void __launch_bounds__(NT) gemm_tiled_kernel(int64_t G, int M, int N,
 #pragma unroll
       for (int i = 0; i < TM; i++)
 #pragma unroll
-        for (int j = 0; j < TN; j++) oplus<R>(acc_e[i][j], acc_c[i][j], a_e[i] + b_e[j], R::mul(a_c[i], b_c[j]));
+        for (int j = 0; j < TN; j++) oplus<R>(acc_e[i][j], acc_c[i][j], a_e[i] + b_e[j],
+                   NARROW ? (CT)((uint64_t)(uint32_t)a_c[i] * (uint32_t)b_c[j]) : R::mul(a_c[i], b_c[j]));
     }
     __syncthreads();
   }
@@ -103,6 +106,13 @@ void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmaj
   }
   const int64_t n_cta = (int64_t)((N + BN - 1) / BN) * ((M + BM - 1) / BM) * batch * G;
   dim3 grid((unsigned)n_cta);
+  if (ring == RING_U64 && count_bits <= 32) {
+    using R = RingU64;
+    const uint64_t *ac = (const uint64_t *)Ac, *bc = (const uint64_t *)Bc; uint64_t *cc = (uint64_t *)Cc;
+    if (a_kmajor) gemm_tiled_kernel<R, true, true><<<grid, NT, 0, st>>>(G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
+    else gemm_tiled_kernel<R, false, true><<<grid, NT, 0, st>>>(G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
+    return;
+  }
   BBTN_RING_DISPATCH(ring, {
     using CT = typename R::T;
     if (a_kmajor)

@@ -46,6 +46,8 @@ def _oracle_gemm(oracle, Ae, Ac, Be, Bc):
     (4, 17, 200, 3, 6, 0.5, True),
     (1, 1, 300, 1000, 7, 0.0, False),
     (2, 333, 1, 129, 8, 0.3, False),
+    (7, 48, 64, 33, 9, 0.2, False),        # M, N <= 64: the 64x64-tile kernel, ragged, batched
+    (3, 64, 37, 70, 10, 0.0, True),
 ])
 def test_gemm_matches_oracle(bb, oracle, B, M, N, K, seed, frac, wide):
     Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed, neg_inf_frac=frac, wide_counts=wide)
