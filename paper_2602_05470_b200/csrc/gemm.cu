@@ -13,6 +13,18 @@ namespace {
 
 constexpr int BM = 64, BN = 64, BK = 16, TM = 4, TN = 4, NT = 256;
 
+template <class CT> struct Stage {
+  static constexpr int AE = 0, AC = AE + BK * (BM + 4) * 4, BE = AC + BK * (BM + 2) * (int)sizeof(CT),
+                       BC = BE + BK * (BN + 4) * 4, BYTES = BC + BK * (BN + 2) * (int)sizeof(CT);
+  static_assert(AC % 8 == 0 && BE % 8 == 0 && BC % 8 == 0 && BYTES % 16 == 0, "stage alignment");
+};
+
+// 4- or 8-byte asynchronous global -> shared copy (element-wise: the A tile is transposed on the way in)
+template <int BYTES> __device__ __forceinline__ void cp_async_small(void *smem, const void *gmem) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(d), "l"(gmem), "n"(BYTES) : "memory");
+}
+
 // c += (ea + eb == E) ? lo32(ca) * lo32(cb) : 0, as SEL + IMAD.WIDE with the 64-bit accumulate fused
 template <class CT>
 __device__ __forceinline__ void tie_fma_narrow(CT &c, int32_t ea, int32_t eb, int32_t E, CT ca, CT cb) {
@@ -32,10 +44,10 @@ __global__ void __launch_bounds__(NT, NARROW ? 2 : 1) gemm_tiled_kernel(int64_t 
                                                         int32_t *__restrict__ Ce, typename R::T *__restrict__ Cc,
                                                         int64_t sA, int64_t sB, int64_t sC) {
   using CT = typename R::T;
-  __shared__ int32_t As_e[BK][BM + 4];
-  __shared__ CT As_c[BK][BM + 2];
-  __shared__ int32_t Bs_e[BK][BN + 4];
-  __shared__ CT Bs_c[BK][BN + 2];
+  // two stages, each [k][m] A energies / counts and [k][n] B energies / counts; the next chunk is
+  // brought in by cp.async while the current one is consumed (no staging registers)
+  using S = Stage<CT>;
+  extern __shared__ __align__(16) unsigned char dsm[];
 
   const int tiles_n = (N + BN - 1) / BN, tiles_m = (M + BM - 1) / BM;
   const int64_t bg = blockIdx.x / (tiles_n * tiles_m);
@@ -53,26 +65,39 @@ __global__ void __launch_bounds__(NT, NARROW ? 2 : 1) gemm_tiled_kernel(int64_t 
 #pragma unroll
     for (int j = 0; j < TN; j++) { acc_e[i][j] = NEG_INF; acc_c[i][j] = 0; }
 
-  for (int k0 = 0; k0 < K; k0 += BK) {
-    // stage A tile as [k][m] and B tile as [k][n]; out-of-range entries are the zero element
+  // stage A tile as [k][m] and B tile as [k][n]; out-of-range entries are the zero element
+  auto fill = [&](int st, int k0) {
+    unsigned char *base = dsm + st * S::BYTES;
+    auto Ase = reinterpret_cast<int32_t (*)[BM + 4]>(base + S::AE); auto Asc = reinterpret_cast<CT (*)[BM + 2]>(base + S::AC);
+    auto Bse = reinterpret_cast<int32_t (*)[BN + 4]>(base + S::BE); auto Bsc = reinterpret_cast<CT (*)[BN + 2]>(base + S::BC);
     for (int i = threadIdx.x; i < BM * BK; i += NT) {
       int kk, mm;
       if (A_KMAJOR) { kk = i / BM; mm = i % BM; } else { mm = i / BK; kk = i % BK; }
       const int gm = m0 + mm, gk = k0 + kk;
-      int32_t e = NEG_INF; CT c = 0;
       if (gm < M && gk < K) {
         const int64_t idx = A_KMAJOR ? (int64_t)gk * M + gm : (int64_t)gm * K + gk;
-        e = ae[idx]; c = ac[idx];
-      }
-      As_e[kk][mm] = e; As_c[kk][mm] = c;
+        cp_async_small<4>(&Ase[kk][mm], ae + idx); cp_async_small<(int)sizeof(CT)>(&Asc[kk][mm], ac + idx);
+      } else { Ase[kk][mm] = NEG_INF; Asc[kk][mm] = 0; }
     }
     for (int i = threadIdx.x; i < BN * BK; i += NT) {
       const int kk = i / BN, nn = i % BN;
       const int gn = n0 + nn, gk = k0 + kk;
-      int32_t e = NEG_INF; CT c = 0;
-      if (gn < N && gk < K) { e = be[(int64_t)gk * N + gn]; c = bc[(int64_t)gk * N + gn]; }
-      Bs_e[kk][nn] = e; Bs_c[kk][nn] = c;
+      if (gn < N && gk < K) {
+        const int64_t idx = (int64_t)gk * N + gn;
+        cp_async_small<4>(&Bse[kk][nn], be + idx); cp_async_small<(int)sizeof(CT)>(&Bsc[kk][nn], bc + idx);
+      } else { Bse[kk][nn] = NEG_INF; Bsc[kk][nn] = 0; }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+
+  fill(0, 0);
+  for (int k0 = 0, chunk = 0; k0 < K; k0 += BK, chunk++) {
+    const int cur = chunk & 1;
+    if (k0 + BK < K) { fill(cur ^ 1, k0 + BK); asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+    else asm volatile("cp.async.wait_group 0;" ::: "memory");
+    unsigned char *base = dsm + cur * S::BYTES;
+    auto As_e = reinterpret_cast<int32_t (*)[BM + 4]>(base + S::AE); auto As_c = reinterpret_cast<CT (*)[BM + 2]>(base + S::AC);
+    auto Bs_e = reinterpret_cast<int32_t (*)[BN + 4]>(base + S::BE); auto Bs_c = reinterpret_cast<CT (*)[BN + 2]>(base + S::BC);
     __syncthreads();
     if (NARROW) {
       // two passes over the chunk, as in gemm_tiled.cu: (1) the running maximum, one fused add-max per term;
@@ -142,6 +167,18 @@ __global__ void __launch_bounds__(NT, NARROW ? 2 : 1) gemm_tiled_kernel(int64_t 
     }
 }
 
+template <class R, bool A_KMAJOR, bool NARROW>
+void launch_v1(dim3 grid, cudaStream_t st, int64_t G, int M, int N, int K, const int32_t *Ae, const typename R::T *Ac,
+               const int32_t *Be, const typename R::T *Bc, int32_t *Ce, typename R::T *Cc, int64_t sA, int64_t sB, int64_t sC) {
+  constexpr int SMEM = 2 * Stage<typename R::T>::BYTES;
+  static bool configured = false;                      // per instantiation; the attribute is per function
+  if (!configured) {
+    cudaFuncSetAttribute(gemm_tiled_kernel<R, A_KMAJOR, NARROW>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+    configured = true;
+  }
+  gemm_tiled_kernel<R, A_KMAJOR, NARROW><<<grid, NT, SMEM, st>>>(G, M, N, K, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC);
+}
+
 }  // namespace
 
 void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
@@ -159,16 +196,16 @@ void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmaj
   if (ring == RING_U64 && count_bits <= 32) {
     using R = RingU64;
     const uint64_t *ac = (const uint64_t *)Ac, *bc = (const uint64_t *)Bc; uint64_t *cc = (uint64_t *)Cc;
-    if (a_kmajor) gemm_tiled_kernel<R, true, true><<<grid, NT, 0, st>>>(G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
-    else gemm_tiled_kernel<R, false, true><<<grid, NT, 0, st>>>(G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
+    if (a_kmajor) launch_v1<R, true, true>(grid, st, G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
+    else launch_v1<R, false, true>(grid, st, G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
     return;
   }
   BBTN_RING_DISPATCH(ring, {
     using CT = typename R::T;
     if (a_kmajor)
-      gemm_tiled_kernel<R, true><<<grid, NT, 0, st>>>(G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
+      launch_v1<R, true, false>(grid, st, G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
     else
-      gemm_tiled_kernel<R, false><<<grid, NT, 0, st>>>(G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
+      launch_v1<R, false, false>(grid, st, G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
   });
 }
 
