@@ -4,7 +4,8 @@
 //   (ea,ca) (.) (eb,cb) = (ea+eb, ca*cb);  (+) keeps the max energy, adds counts on ties.
 //
 // Tensor cores cannot evaluate max-plus, so this runs on the integer CUDA cores (north_star).
-// v1: single pass, 64x64 CTA tile, BK = 16, 256 threads, 4x4 outputs per thread.
+// 64x64 CTA tile, BK = 16, 256 threads, 4x4 outputs per thread, two cp.async-fed shared-memory stages.
+// Used by the mod-p rings and by RING_U64 shapes with M, N <= 64 (gemm_tiled.cu has the 128-row tile).
 #include "kernels.h"
 #include "ring.cuh"
 
