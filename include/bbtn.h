@@ -202,14 +202,31 @@ int bbtn_oplus_combine(int32_t kind, int64_t n, const int32_t *energy, const uin
                        const uint32_t *count_mod, int32_t *out_energy, uint64_t *out_count,
                        uint32_t *out_count_mod);
 
+/* CRT recombination of the three count residues of BBTN_COUNT_CRT mode (reading A9): 2^64, BBTN_P1 and
+ * BBTN_P2 are pairwise coprime, so (count mod 2^64, count mod P1, count mod P2) determine the count modulo
+ * 2^64 * P1 * P2 (about 2^126).  out[0] = low 64 bits, out[1] = high 64 bits of that value; it IS the exact count
+ * whenever the count is below 2^126.  Host only, no device.  Errors: EINVAL (null out, residue >= its prime). */
+int bbtn_crt_combine(uint64_t count_mod_2_64, uint32_t count_mod_p1, uint32_t count_mod_p2, uint64_t out[2]);
+
+/* Debug checks of caller promises (process-wide switch, default off; also switched on by the environment
+ * variable BBTN_DEBUG_CHECKS=1 at load time).  When on, the raw GEMM entry points first verify ON THE DEVICE
+ * that every operand count is below 2^count_bits (for count_bits < 64) and that every operand energy is either
+ * exactly BBTN_NEG_INF or within +-BBTN_ENERGY_LIMIT, synchronise, and return BBTN_EINVAL without launching K3
+ * if a promise is broken.  Returns the previous setting. */
+int bbtn_set_debug_checks(int32_t on);
+
 /* Raw batched counting-tropical GEMM (K3 alone; the config-4 sweep):
  *   C[b,m,n] = (+)_k A[b,m,k] (.) B[b,k,n]
  * ALL pointers are DEVICE pointers.  Row-major: A [batch][M][K], B [batch][K][N], C [batch][M][N];
  * stride* are the ELEMENT distances between consecutive batch entries (0 = operand shared by the
- * whole batch).  Energies int32 (<= -2^29 means the zero element; outputs are canonical),
- * counts uint64 mod 2^64.  M, N, K >= 1, any size (ragged tiles are handled).
- * count_bits: upper bound on log2(count+1) of BOTH operands that the caller guarantees
- * (64 = no promise; <= 32 selects the 32x32->64 multiply fast path).  Asynchronous on cuda_stream. */
+ * whole batch).  Energies int32: the zero element must be passed in its canonical form (BBTN_NEG_INF, count 0),
+ * finite energies obey |e| <= BBTN_ENERGY_LIMIT; outputs are canonical, so results can be fed back in.  Other
+ * energies are a broken promise (sums could wrap): undefined results, caught by bbtn_set_debug_checks.
+ * Counts uint64 mod 2^64.  M, N, K >= 1, any size (ragged tiles are handled); the launch is refused with
+ * BBTN_ESHAPE if it would need more than 2^31-1 thread blocks.
+ * count_bits in 1..64: upper bound on log2(count+1) of BOTH operands that the caller guarantees (64 = no
+ * promise; <= 32 selects the 32x32->64 multiply path, small values 32-bit accumulators).  A broken promise gives
+ * wrong counts silently unless bbtn_set_debug_checks is on.  Asynchronous on cuda_stream. */
 int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,
                                const int32_t *Ae, const uint64_t *Ac,
                                const int32_t *Be, const uint64_t *Bc,

@@ -25,7 +25,7 @@ BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
 EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves",
            "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
-           "bbtn_permute_batched", "bbtn_int32_microbench",
+           "bbtn_permute_batched", "bbtn_int32_microbench", "bbtn_crt_combine", "bbtn_set_debug_checks",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
 
 
@@ -72,6 +72,8 @@ def load():
     lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
     lib.bbtn_permute_batched.argtypes = [i32, vp, i64, vp, vp, vp, vp, vp]
     lib.bbtn_int32_microbench.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+    lib.bbtn_crt_combine.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, vp]
+    lib.bbtn_set_debug_checks.argtypes = [i32]
     lib.bbtn_destroy.argtypes = [vp]
     lib.bbtn_destroy.restype = None
     lib.bbtn_last_error.argtypes = [vp]
@@ -293,11 +295,13 @@ def int32_microbench(which: int, iters: int = 2000, stream=None):
 
 
 def crt_combine(c64: int, r1: int, r2: int) -> int:
-    """Host-side CRT of (count mod 2^64, mod P1, mod P2) -> count mod 2^64*P1*P2 (reading A9)."""
-    mods = [1 << 64, BBTN_P1, BBTN_P2]
-    x, m = int(c64), mods[0]
-    for r, p in ((int(r1), BBTN_P1), (int(r2), BBTN_P2)):
-        t = ((r - x) * pow(m, -1, p)) % p
-        x += m * t
-        m *= p
-    return x
+    """bbtn_crt_combine: (count mod 2^64, mod P1, mod P2) -> count mod 2^64*P1*P2 (reading A9), as a Python int
+    assembled from the two 64-bit limbs the library returns."""
+    out = (C.c_uint64 * 2)()
+    _check(load().bbtn_crt_combine(int(c64), int(r1), int(r2), C.addressof(out)))
+    return int(out[0]) | (int(out[1]) << 64)
+
+
+def set_debug_checks(on: bool) -> bool:
+    """bbtn_set_debug_checks: verify the raw GEMM's count_bits / energy-range promises on the device."""
+    return bool(load().bbtn_set_debug_checks(1 if on else 0))

@@ -16,7 +16,6 @@
 // Anything else (rank < 4, several summed low bits, unaligned arena offsets) takes the scalar kernel.
 #include "kernels.h"
 #include "ring.cuh"
-#include <cstdio>
 
 namespace bbtn {
 namespace {
@@ -197,9 +196,6 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
   } else if (s.nK == 1 && s.kA[0] == 1u && s.addA[0] == 2u && s.addA[1] == 4u) lp = LP_K0;
   else if (s.nK == 1 && s.kA[0] == 2u && s.addA[0] == 1u && s.addA[1] == 4u) lp = LP_K1;
   else return false;
-#ifdef BBTN_TRACE_LP
-  fprintf(stderr, "LP %d ring %d nK %d rO %d\n", lp, ring, s.nK, s.rO);
-#endif
   // fold the top output bits that only B carries (see the kernel comment); keep >= 4 unfolded bits
   int nF = 0;
   while (nF < 2 && s.rO - nF > 4 && s.addA[s.rO - 1 - nF] == 0u) nF++;

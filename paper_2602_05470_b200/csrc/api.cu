@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <memory>
@@ -28,6 +29,47 @@ bool have_device() {
 }  // namespace bbtn
 
 namespace {
+
+// ---- debug checks of the raw-GEMM promises (include/bbtn.h: bbtn_set_debug_checks) ----
+bool g_debug_checks = [] { const char *e = std::getenv("BBTN_DEBUG_CHECKS"); return e && e[0] == '1'; }();
+
+// flags |= 1: a count >= 2^count_bits;  |= 2: an energy that is neither BBTN_NEG_INF nor within +-BBTN_ENERGY_LIMIT
+__global__ void check_operand_kernel(const int32_t *__restrict__ e, const uint64_t *__restrict__ c, int64_t rows, int64_t row_len,
+                                     int64_t row_stride, int count_bits, int *flags) {
+  const int64_t total = rows * row_len;
+  int bad = 0;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = t / row_len, i = r * row_stride + (t - r * row_len);
+    const int32_t ee = e[i];
+    if (count_bits < 64 && (c[i] >> count_bits) != 0) bad |= 1;
+    if (ee != BBTN_NEG_INF && (ee > BBTN_ENERGY_LIMIT || ee < -BBTN_ENERGY_LIMIT)) bad |= 2;
+  }
+  if (bad) atomicOr(flags, bad);
+}
+
+int check_gemm_operands(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac, const int32_t *Be,
+                        const uint64_t *Bc, int64_t sA, int64_t sB, int32_t count_bits, cudaStream_t st) {
+  int *d_flags = nullptr, h_flags = 0;
+  CUDA_TRY(nullptr, cudaMalloc(&d_flags, sizeof(int)));
+  cudaMemsetAsync(d_flags, 0, sizeof(int), st);
+  check_operand_kernel<<<148 * 4, 256, 0, st>>>(Ae, Ac, sA ? batch : 1, (int64_t)M * K, sA, count_bits, d_flags);
+  check_operand_kernel<<<148 * 4, 256, 0, st>>>(Be, Bc, sB ? batch : 1, (int64_t)K * N, sB, count_bits, d_flags);
+  cudaError_t e = cudaMemcpyAsync(&h_flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_flags);
+  CUDA_TRY(nullptr, e);
+  if (h_flags & 1) return fail(nullptr, BBTN_EINVAL, "debug check: an operand count is not below 2^count_bits (count_bits = " + std::to_string(count_bits) + ")");
+  if (h_flags & 2) return fail(nullptr, BBTN_EINVAL, "debug check: an operand energy is neither BBTN_NEG_INF nor within +-BBTN_ENERGY_LIMIT");
+  return BBTN_OK;
+}
+
+int check_gemm_shape(int64_t batch, int32_t M, int32_t N, int32_t count_bits) {
+  if (count_bits < 1 || count_bits > 64) return fail(nullptr, BBTN_EINVAL, "count_bits must be in 1..64");
+  // the smallest tile any K3 form uses is 64x64: one thread block per tile and batch entry
+  const double n_cta = (double)((M + 63) / 64) * (double)((N + 63) / 64) * (double)batch;
+  if (n_cta > 2147483647.0) return fail(nullptr, BBTN_ESHAPE, "GEMM launch would need more than 2^31-1 thread blocks; split the batch");
+  return BBTN_OK;
+}
 
 int get_plan(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, bool enforce, DevPlan **out) {
   if (n_fixed < 0 || (n_fixed > 0 && !fixed)) return fail(h, BBTN_EINVAL, "bad fixed set");
@@ -126,7 +168,7 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
                           pe(s.vA, s.offA), pc(s.vA, s.offA), pe(s.vB, s.offB), pc(s.vB, s.offB),
                           pe(s.vC, s.offC), pc(s.vC, s.offC),
                           s.vA ? ((int64_t)1 << s.rA) : 0, s.vB ? ((int64_t)1 << s.rB) : 0, (int64_t)1 << s.rO,
-                          ring, 64, st);
+                          ring, s.count_bits, st);
         break;
     }
   }
@@ -242,7 +284,14 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
   // a power of two (padding leaves = assignment 0, results dropped): the CUDA graph of this fixed set is then
   // captured once per size class instead of once per distinct B (the host B&B loop sends ragged batches).
   const int64_t B_user = B;
-  if (!dev_io) { int64_t bp = 1; while (bp < B) bp <<= 1; B = bp; }
+  if (!dev_io) {
+    int64_t bp = 1; while (bp < B) bp <<= 1;
+    // pad only when the padded arena fits; a ragged B just above a power of two must not turn into ENOMEM
+    size_t free_b = 0, total_b = 0;
+    if (bp <= dp->B_cap || (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess &&
+                            (double)dp->plan.arena_variant_elems * (double)bp * 12.0 <= (double)free_b + (double)dp->var_e.bytes + (double)dp->var_c.bytes))
+      B = bp;
+  }
   if ((rc = ensure_batch(h, dp, B, !dev_io))) return rc;
   cudaStream_t st = (cudaStream_t)stream;
   const uint8_t *d_assign = assign; int32_t *d_energy = energy; uint64_t *d_count = count; uint32_t *d_mod = count_mod;
@@ -267,16 +316,22 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
       dp->graphs.clear();
       cudaStream_t cs;
       CUDA_TRY(h, cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
-      for (int ring = 0; ring < n_rings; ring++) {
+      cudaError_t ce = cudaSuccess;
+      for (int ring = 0; ring < n_rings && ce == cudaSuccess; ring++) {
         cudaGraph_t g = nullptr; cudaGraphExec_t ge = nullptr;
-        CUDA_TRY(h, cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+        if ((ce = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal)) != cudaSuccess) break;
         enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring, cs);
-        CUDA_TRY(h, cudaStreamEndCapture(cs, &g));
-        CUDA_TRY(h, cudaGraphInstantiate(&ge, g, 0));
-        cudaGraphDestroy(g);
-        dp->graphs.push_back(ge);
+        ce = cudaStreamEndCapture(cs, &g);          // always ends the capture, also after a failed launch
+        if (ce == cudaSuccess) ce = cudaGraphInstantiate(&ge, g, 0);
+        if (g) cudaGraphDestroy(g);
+        if (ce == cudaSuccess) dp->graphs.push_back(ge);
       }
       cudaStreamDestroy(cs);
+      if (ce != cudaSuccess) {
+        for (auto g : dp->graphs) if (g) cudaGraphExecDestroy(g);
+        dp->graphs.clear(); dp->graph_B = -1;
+        CUDA_TRY(h, ce);
+      }
       dp->graph_B = B; std::memcpy(dp->graph_io, io, sizeof(io));
     }
     for (auto ge : dp->graphs) CUDA_TRY(h, cudaGraphLaunch(ge, st));
@@ -303,7 +358,10 @@ int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, c
   if (batch < 1 || M < 1 || N < 1 || K < 1 || !Ae || !Ac || !Be || !Bc || !Ce || !Cc || strideA < 0 || strideB < 0 || strideC < 0)
     return fail(nullptr, BBTN_EINVAL, "bad GEMM arguments");
   if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
+  int rc = check_gemm_shape(batch, M, N, count_bits);
+  if (rc) return rc;
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  if (g_debug_checks && (rc = check_gemm_operands(batch, M, N, K, Ae, Ac, Be, Bc, strideA, strideB, count_bits, (cudaStream_t)stream))) return rc;
   launch_gemm_tiled(batch, 1, M, N, K, 0, Ae, Ac, Be, Bc, Ce, Cc, strideA, strideB, strideC, RING_U64, count_bits,
                     (cudaStream_t)stream);
   CUDA_TRY(nullptr, cudaGetLastError());
@@ -318,6 +376,7 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
   if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
   if ((strideA && strideA < (int64_t)M * K) || (strideB && strideB < (int64_t)K * N))
     return fail(nullptr, BBTN_EINVAL, "operand stride smaller than the operand");
+  { int rc = check_gemm_shape(batch, M, N, count_bits); if (rc) return rc; }
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
   static thread_local DevBuf st_e[3], st_c[3];
   cudaStream_t st = (cudaStream_t)stream;
@@ -370,6 +429,11 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
     }
     CUDA_TRY(nullptr, cudaEventRecord(ev_in[c], s_in));
     CUDA_TRY(nullptr, cudaStreamWaitEvent(s_k, ev_in[c], 0));
+    if (g_debug_checks) {
+      int rc = check_gemm_operands(nb, M, N, K, dAe + b0 * strideA, dAc + b0 * strideA, dBe + b0 * strideB, dBc + b0 * strideB,
+                                   strideA, strideB, count_bits, s_k);
+      if (rc) { cudaStreamSynchronize(s_in); cudaStreamSynchronize(s_out); return rc; }
+    }
     launch_gemm_tiled(nb, 1, M, N, K, 0, dAe + b0 * strideA, dAc + b0 * strideA, dBe + b0 * strideB, dBc + b0 * strideB,
                       dCe + b0 * strideC, dCc + b0 * strideC, strideA, strideB, strideC, RING_U64, count_bits, s_k);
     CUDA_TRY(nullptr, cudaGetLastError());
@@ -397,6 +461,30 @@ int bbtn_permute_batched(int32_t rank, const int32_t *perm, int64_t batch, const
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
   launch_permute(rank, perm, batch, src_e, src_c, dst_e, dst_c, RING_U64, (cudaStream_t)stream);
   CUDA_TRY(nullptr, cudaGetLastError());
+  return BBTN_OK;
+}
+
+int bbtn_set_debug_checks(int32_t on) {
+  const int prev = g_debug_checks ? 1 : 0;
+  g_debug_checks = on != 0;
+  return prev;
+}
+
+// CRT over the pairwise coprime moduli 2^64, P1, P2 (Garner's form): x = c64 + 2^64 * (t1 + P1 * t2).
+int bbtn_crt_combine(uint64_t c64, uint32_t r1, uint32_t r2, uint64_t out[2]) {
+  if (!out || r1 >= BBTN_P1 || r2 >= BBTN_P2) return fail(nullptr, BBTN_EINVAL, "bad crt_combine arguments");
+  auto powmod = [](uint64_t b, uint64_t e, uint64_t p) { uint64_t r = 1; b %= p; for (; e; e >>= 1, b = b * b % p) if (e & 1) r = r * b % p; return r; };
+  const uint64_t p1 = BBTN_P1, p2 = BBTN_P2;
+  const uint64_t two64_p1 = (((uint64_t)1 << 32) % p1) * (((uint64_t)1 << 32) % p1) % p1;
+  const uint64_t two64_p2 = (((uint64_t)1 << 32) % p2) * (((uint64_t)1 << 32) % p2) % p2;
+  // t1 = (r1 - c64) / 2^64 mod P1     (inverse by Fermat: P1 is prime)
+  const uint64_t t1 = (r1 + p1 - c64 % p1) % p1 * powmod(two64_p1, p1 - 2, p1) % p1;
+  // x1 = c64 + 2^64 t1;  t2 = (r2 - x1) / (2^64 P1) mod P2
+  const uint64_t x1_p2 = (c64 % p2 + two64_p2 * (t1 % p2)) % p2;
+  const uint64_t m_p2 = two64_p2 * (p1 % p2) % p2;
+  const uint64_t t2 = (r2 + p2 - x1_p2) % p2 * powmod(m_p2, p2 - 2, p2) % p2;
+  out[0] = c64;
+  out[1] = t1 + p1 * t2;            // < P1 * P2 < 2^62
   return BBTN_OK;
 }
 

@@ -15,9 +15,7 @@
 // contracted by K1..K4 (run_plan), and the leaf results are (+)-accumulated ("summing the
 // contractions of each branch").  Plain C++; every arithmetic step on tensors runs in the kernels.
 #include <algorithm>
-#include <chrono>
 #include <cmath>
-#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 
@@ -48,8 +46,7 @@ struct Brancher {
   bool contract = false; void *stream = nullptr; bool want_mod = false;
   bool have_best = false; int32_t best = BBTN_NEG_INF; uint64_t c64 = 0, m1 = 0, m2 = 0;
   int64_t n_leaves = 0;
-  double leaf_bytes = 0, leaf_fma = 0, plan_seconds = 0;
-  const bool trace = std::getenv("BBTN_TRACE_BRANCHING") != nullptr;   // per-leaf progress on stderr
+  double leaf_bytes = 0, leaf_fma = 0;
 
   int init(std::string &err) {
     Plan pl;
@@ -132,14 +129,8 @@ struct Brancher {
     for (int v : trail) a.push_back((uint8_t)val[v]);
     int32_t e; uint64_t c; uint32_t cm[2] = {0, 0};
     DevPlan *dp = h->scratch.get();
-    const auto t0 = std::chrono::steady_clock::now();
     int rc = run_plan(h, dp, a.data(), 1, &e, &c, want_mod ? cm : nullptr, false, stream);
     if (rc) return rc;
-    if (trace)
-      fprintf(stderr, "[bbtn branching] leaf %lld: |F| = %zu, width %d, %.3g GB arena, %.3g TB moved, run %.3f s (plan %.3f s)\n",
-              (long long)n_leaves, trail.size(), pl->max_rank, pl->arena_variant_elems * 12e-9,
-              (pl->bytes_variant + pl->bytes_invariant) * 1e-12,
-              std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count(), plan_seconds);
     if (e == BBTN_NEG_INF) return BBTN_OK;
     const bool better = !have_best || (P->kind == BBTN_ISING ? e < best : e > best);
     if (better) { best = e; c64 = 0; m1 = m2 = 0; have_best = true; }
@@ -155,9 +146,7 @@ struct Brancher {
       // against a tighter threshold
       DevPlan *dp = h->scratch.get();
       std::string err;
-      const auto t0 = std::chrono::steady_clock::now();
       int rc = make_plan(*P, trail, h->force_mode, false, dp->plan, err, true, false);
-      plan_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
       if (rc) return fail(h, rc, err);
       dp->tables_ready = false; dp->B_cap = 0; dp->graph_B = -1;
       const int64_t bytes = dp->plan.arena_variant_elems * 12;

@@ -172,11 +172,8 @@ template <class R, bool A_KMAJOR, bool NARROW>
 void launch_v1(dim3 grid, cudaStream_t st, int64_t G, int M, int N, int K, const int32_t *Ae, const typename R::T *Ac,
                const int32_t *Be, const typename R::T *Bc, int32_t *Ce, typename R::T *Cc, int64_t sA, int64_t sB, int64_t sC) {
   constexpr int SMEM = 2 * Stage<typename R::T>::BYTES;
-  static bool configured = false;                      // per instantiation; the attribute is per function
-  if (!configured) {
-    cudaFuncSetAttribute(gemm_tiled_kernel<R, A_KMAJOR, NARROW>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
-    configured = true;
-  }
+  // per function AND per device, so set it on every launch (a cheap host-side call)
+  cudaFuncSetAttribute(gemm_tiled_kernel<R, A_KMAJOR, NARROW>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
   gemm_tiled_kernel<R, A_KMAJOR, NARROW><<<grid, NT, SMEM, st>>>(G, M, N, K, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC);
 }
 

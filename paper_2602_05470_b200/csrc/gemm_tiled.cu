@@ -415,11 +415,8 @@ void launch_one(const GemmArgs &a, int64_t batch, cudaStream_t st) {
   using CT = typename std::conditional<MODE == WIDE, uint64_t, uint32_t>::type;
   using T = Tile<NCB, CT>;
   static_assert(T::SMEM <= 227 * 1024, "shared memory budget");
-  static bool configured = false;                      // per instantiation; the attribute is per function
-  if (!configured) {
-    cudaFuncSetAttribute(gemm_tiled3_kernel<MODE, A_KMAJOR, NCB>, cudaFuncAttributeMaxDynamicSharedMemorySize, T::SMEM);
-    configured = true;
-  }
+  // per function AND per device, so set it on every launch (a cheap host-side call)
+  cudaFuncSetAttribute(gemm_tiled3_kernel<MODE, A_KMAJOR, NCB>, cudaFuncAttributeMaxDynamicSharedMemorySize, T::SMEM);
   const int64_t n_cta = (int64_t)((a.N + T::BNt - 1) / T::BNt) * ((a.M + BM - 1) / BM) * batch * a.G;
   gemm_tiled3_kernel<MODE, A_KMAJOR, NCB><<<dim3((unsigned)n_cta), NT, T::SMEM, st>>>(a);
 }

@@ -83,7 +83,7 @@ __global__ void construct_offset_kernel(int kind, const InputRec *__restrict__ i
 // ---------------------------------------------------------------------------------------------
 struct AbsorbArgs {
   int rO, nK;
-  uint32_t addA[32], addB[32], kA[12], kB[12];
+  uint32_t addA[32], addB[32], kA[32], kB[32];
   int64_t sA, sB, sC, total;
 };
 
@@ -100,9 +100,9 @@ __global__ void absorb_kernel(AbsorbArgs p, const int32_t *__restrict__ Ae, cons
     const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
     const int32_t *be = Be + b * p.sB; const typename R::T *bc = Bc + b * p.sB;
     int32_t acc_e = NEG_INF; typename R::T acc_c = 0;
-    for (uint32_t k = 0; k < (1u << p.nK); k++) {
+    for (uint64_t k = 0; k < (1ull << p.nK); k++) {        // nK may be 32
       uint32_t ia = a0, ib = b0;
-      for (int j = 0; j < p.nK; j++) if ((k >> j) & 1u) { ia += p.kA[j]; ib += p.kB[j]; }
+      for (int j = 0; j < p.nK; j++) if ((k >> j) & 1ull) { ia += p.kA[j]; ib += p.kB[j]; }
       const int32_t e = ae[ia] + be[ib];
       const typename R::T c = R::mul(ac[ia], bc[ib]);
       oplus<R>(acc_e, acc_c, e, c);
@@ -219,8 +219,7 @@ void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
   if (launch_absorb_vec(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st)) return;   // 16-byte form (absorb_vec.cu)
   AbsorbArgs p;
   p.rO = s.rO; p.nK = s.nK;
-  for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; }
-  for (int i = 0; i < 12; i++) { p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
+  for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
   p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
   p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
   p.sC = (int64_t)1 << s.rO;

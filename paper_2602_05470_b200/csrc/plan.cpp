@@ -60,6 +60,7 @@ struct TRef {
   std::vector<int> idx;           // idx[p] = index label at bit p
   int64_t off = 0;
   std::map<int, int> sub;         // unfinished indices -> number of input tensors in the subtree carrying them
+  int lc = 0;                     // every count of this tensor is <= 2^lc (inputs: 1; (.) adds, (+) over 2^k terms adds k)
 };
 
 int pos_of(const std::vector<int> &v, int x) {
@@ -205,6 +206,7 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
     if (r.fu < 0 && !r.su) { r.bu = rank++; x.idx.push_back(r.u); x.sub[r.u] = 1; }
     if (r.v >= 0 && r.fv < 0 && !r.sv) { r.bv = rank++; x.idx.push_back(r.v); x.sub[r.v] = 1; }
     r.rank = rank;
+    x.lc = r.su + r.sv;             // K1 pre-sums single-owner indices: up to 2 (4) unit counts added
     r.variant = (single_arena || r.fu >= 0 || r.fv >= 0) ? 1 : 0;
     r.offset = -1;
     if (rank == 0) { out.scalar_inputs.push_back(t); x.removed = true; continue; }
@@ -235,6 +237,7 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
     // merged occurrence counts -> I_O = labels still carried by an input outside this subtree
     O.removed = false;
     O.variant = L.variant || R.variant;
+    const int lc_in = std::max(L.lc, R.lc), lc_sum = L.lc + R.lc;
     O.sub = L.sub;
     for (auto &kv : R.sub) O.sub[kv.first] += kv.second;
     for (auto it = O.sub.begin(); it != O.sub.end();) {
@@ -279,13 +282,15 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
     bool tiled = false;
     if (force_mode == 2) tiled = lk >= 1;
     else if (force_mode == 0) tiled = lk >= 4 && lm >= 5 && ln >= 5;
+    O.lc = std::min(lc_sum + lk, 1 << 20);
     out.n_nodes++;
     if (var) out.n_variant_nodes++;
     (var ? out.fma_variant : out.fma_invariant) += fma;
 
     if (!tiled) {
       Step st;
-      st.kind = (rO <= 6 && lk >= 8) ? STEP_REDUCE : STEP_ABSORB;
+      // few outputs and a long sum: one CTA per output ((+)-reduction across the block); everything else streams
+      st.kind = (lk >= 8 && rO <= 10) ? STEP_REDUCE : STEP_ABSORB;
       st.variant = var;
       st.rO = rO; st.nK = lk;
       // output layout: A's surviving bits in A's order, then B's new bits
@@ -335,6 +340,7 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
       if (tmpB) release(B);
       Step st;
       st.kind = STEP_GEMM; st.variant = var;
+      st.count_bits = std::min(lc_in + 1, 64);
       st.lg = lg; st.lm = lm; st.ln = ln; st.lk = lk; st.rO = rO; st.nK = lk;
       O.idx = nl;
       O.idx.insert(O.idx.end(), ml.begin(), ml.end());

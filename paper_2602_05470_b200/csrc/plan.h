@@ -57,6 +57,9 @@ struct Step {
   int32_t perm[32] = {0};
   // GEMM: A [g][k][m], B [g][k][n] -> C [g][m][n]   (log2 sizes)
   int32_t lg = 0, lm = 0, ln = 0, lk = 0;
+  // upper bound on log2(count + 1) of BOTH operands (inputs hold counts 0/1, each (.) adds the operands' bounds,
+  // each (+) over 2^k terms adds k): lets K3 pick its narrow count modes inside a tree; 64 = no useful bound
+  int32_t count_bits = 64;
   double fma = 0;               // tropical FMAs of this launch per batch entry
   double bytes = 0;             // algorithmic bytes per batch entry (12 B per element moved)
 };

@@ -273,6 +273,91 @@ def elimination_tree(index_sets: list[list[int]], order) -> tuple[np.ndarray, np
     return np.array(tl, np.int32), np.array(tr, np.int32)
 
 
+def grouped_elimination_tree(index_sets: list[list[int]], parts) -> tuple[np.ndarray, np.ndarray]:
+    """SSA tree that contracts the network PART BY PART and then joins the parts (a divide-and-conquer
+    tree, as opposed to the frontier sweep of elimination_tree).
+
+    parts = [(vertex_set, order), ...]: input tensor t belongs to the first part whose vertex_set holds
+    every index of t.  Inside a part, bucket elimination along `order` (vertices of the part that occur in
+    no other part), then the part's leftover tensors are merged, smallest first, into ONE boundary tensor
+    over the vertices the part shares with others.  The part results are then joined left to right in a
+    balanced binary fashion: ((P0 P1) (P2 P3)) ...  Pure structure; which index is summed where follows
+    from the occurrence rule of the engine and the oracle alike (reading A11)."""
+    n_in = len(index_sets)
+    owner = [-1] * n_in
+    vsets = [set(int(v) for v in vs) for vs, _ in parts]
+    for t, s in enumerate(index_sets):
+        for p, vs in enumerate(vsets):
+            if all(int(i) in vs for i in s):
+                owner[t] = p
+                break
+        assert owner[t] >= 0, f"input tensor {t} fits no part"
+    occ_all: dict[int, int] = {}
+    for s in index_sets:
+        for i in s:
+            occ_all[int(i)] = occ_all.get(int(i), 0) + 1
+    tl, tr = [], []
+    nxt = n_in
+    # live[t] = (labels, merged-occurrence counts)
+    def merge(live, a, b):
+        nonlocal nxt
+        (sa, ca), (sb, cb) = live.pop(a), live.pop(b)
+        cnt = dict(ca)
+        for i, c in cb.items():
+            cnt[i] = cnt.get(i, 0) + c
+        cnt = {i: c for i, c in cnt.items() if c < occ_all[i]}
+        live[nxt] = (frozenset(i for i in (sa | sb) if i in cnt), cnt)
+        tl.append(a); tr.append(b)
+        nxt += 1
+        return nxt - 1
+    results = []
+    for p, (_, order) in enumerate(parts):
+        live = {t: (frozenset(int(i) for i in s), {int(i): 1 for i in s}) for t, s in enumerate(index_sets) if owner[t] == p}
+        for v in order:
+            v = int(v)
+            while True:
+                ts = sorted((t for t, (s, _) in live.items() if v in s), key=lambda t: (len(live[t][0]), t))
+                if len(ts) < 2:
+                    break
+                merge(live, ts[0], ts[1])
+        while len(live) > 1:
+            ts = sorted(live.keys(), key=lambda t: (len(live[t][0]), t))
+            merge(live, ts[0], ts[1])
+        results.append(live)
+    while len(results) > 1:
+        nxt_round = []
+        for i in range(0, len(results) - 1, 2):
+            live = {**results[i], **results[i + 1]}
+            a, b = list(results[i].keys())[0], list(results[i + 1].keys())[0]
+            merge(live, a, b)
+            nxt_round.append(live)
+        if len(results) % 2:
+            nxt_round.append(results[-1])
+        results = nxt_round
+    return np.array(tl, np.int32), np.array(tr, np.int32)
+
+
+def lattice_block_parts(rows: int, cols: int, row_cuts, col_cuts, ids=None, exclude=()):
+    """Parts for grouped_elimination_tree on a rows x cols lattice (vertex id r*cols + c, or ids[r][c] with
+    -1 for a missing site): rectangular blocks delimited by the separator rows / columns in row_cuts /
+    col_cuts; neighbouring blocks SHARE their separator line.  Inside a block the private vertices are
+    eliminated row-major.  Vertices in `exclude` (a fixed set) are left out."""
+    rb = [0] + list(row_cuts) + [rows - 1]
+    cb = [0] + list(col_cuts) + [cols - 1]
+    ex = set(int(v) for v in exclude)
+    vid = (lambda r, c: r * cols + c) if ids is None else (lambda r, c: int(ids[r][c]))
+    blocks = []
+    for i in range(len(rb) - 1):
+        for j in range(len(cb) - 1):
+            blocks.append([vid(r, c) for r in range(rb[i], rb[i + 1] + 1) for c in range(cb[j], cb[j + 1] + 1)
+                           if vid(r, c) >= 0 and vid(r, c) not in ex])
+    count: dict[int, int] = {}
+    for b in blocks:
+        for v in b:
+            count[v] = count.get(v, 0) + 1
+    return [(b, [v for v in b if count[v] == 1]) for b in blocks]
+
+
 def min_degree_order(inst: "Instance", fixed=()) -> np.ndarray:
     """Greedy min-degree elimination order of the free vertices (ties: fewest fill edges, then lowest
     id) on the graph with `fixed` removed.  Graph structure only."""

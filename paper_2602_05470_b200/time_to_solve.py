@@ -35,8 +35,8 @@ def _timed(fn, repeat):
 
 
 def _leaf_sum(kind, e, c):
-    best = int(e.min()) if kind == "ising" else int(e.max())
-    return best, sum(int(x) for x in c[e == best]) & MASK64
+    """Eq. 3's outer (+) over the leaf results, by the library (bbtn_oplus_combine)."""
+    return bb.oplus_combine(kind, e, c)[:2]
 
 
 def solve_unbranched(name, inst, tree=None, repeat=5, cap=1 << 28):

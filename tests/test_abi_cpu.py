@@ -173,3 +173,39 @@ def test_branching_target_above_width_is_one_leaf_and_guards(lib):
     with pytest.raises(bb.BbtnError):
         h.branching_leaves(0)                          # log2_target out of range
     h.close()
+
+
+def test_crt_combine_matches_big_integers(lib):
+    # bbtn_crt_combine is host arithmetic behind the ABI (reading A9): compare with Python's big integers
+    P1, P2 = bb.BBTN_P1, bb.BBTN_P2
+    M = (1 << 64) * P1 * P2
+    vals = [0, 1, (1 << 64) - 1, 1 << 64, 6 ** 30, 2 ** 100, 4 ** 40 * 3, M - 1, 113847283001211021991799704166400]
+    x = 0x9E3779B97F4A7C15
+    for _ in range(200):
+        x = (x * 6364136223846793005 + 1442695040888963407) % (1 << 128)
+        vals.append(x % M)
+    for v in vals:
+        assert bb.crt_combine(v % (1 << 64), v % P1, v % P2) == v
+    with pytest.raises(bb.BbtnError) as e:
+        bb.crt_combine(0, P1, 0)                 # residue not below its prime
+    assert e.value.status == bb.BBTN_EINVAL
+
+
+def test_raw_gemm_argument_checks_need_no_device(lib):
+    # count_bits outside 1..64 and launches beyond 2^31-1 thread blocks are refused before any CUDA call
+    z = C.c_void_p(16)
+    rc = lib.bbtn_tropical_gemm_batched(1, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 0, None)
+    assert rc == bb.BBTN_EINVAL
+    rc = lib.bbtn_tropical_gemm_batched(1 << 40, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 64, None)
+    assert rc == bb.BBTN_ESHAPE
+    assert bb.set_debug_checks(False) in (False, True)
+
+
+def test_block_tree_plans_use_tiled_gemm_and_trace(lib):
+    # a divide-and-conquer tree makes the planner pick permute + tiled GEMM and the long-reduction kernel in
+    # AUTOMATIC mode (the frontier sweeps of the lattice configs never do)
+    inst = I.ising_lattice_2d(12, 12, 3)
+    tree = I.grouped_elimination_tree(inst.input_index_sets(), I.lattice_block_parts(12, 12, [6], [6]))
+    info = bb.Handle(inst, tree=tree).plan_query()
+    assert info["n_gemm_tiled"] == 2 and info["n_permute"] >= 2 and info["n_trace"] == 1
+    assert info["n_nodes"] == inst.n_edges + inst.n_vertices - 1

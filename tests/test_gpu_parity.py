@@ -69,6 +69,43 @@ def test_gemm_shared_operand_stride0(bb, oracle):
     assert (Ce.cpu().numpy() == want_e).all() and (Cc.cpu().numpy().view(np.uint64) == want_c).all()
 
 
+def test_gemm_4096_sampled_rows_all_count_modes(bb, oracle):
+    # BASELINE config 4a's largest size: 64 sampled full rows (SURVEY 8(c) pin vi) in the three count modes
+    n = 4096
+    Ae, Ac, Be, Bc = I.gemm_operands(1, n, n, n, seed=31)
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    rows = np.unique((I.splitmix64(7, 64, 20) % np.uint64(n)).astype(np.int64))
+    we, wc = _oracle_gemm(oracle, Ae[:, rows], Ac[:, rows], Be, Bc)
+    for bits in (64, 32, 3):
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+        got_e = Ce[0].cpu().numpy(); got_c = Cc[0].cpu().numpy().view(np.uint64)
+        assert (got_e[rows] == we[0]).all() and (got_c[rows] == wc[0]).all(), bits
+        # cheap whole-matrix property: every output energy is attainable (<= 128) and every count is in [1, 16 n]
+        assert got_e.max() <= 128 and got_e.min() >= 100 and got_c.min() >= 1 and got_c.max() <= 16 * n
+
+
+def test_debug_checks_catch_a_broken_promise(bb):
+    # count_bits is a caller promise (include/bbtn.h); with bbtn_set_debug_checks the device verifies it
+    Ae, Ac, Be, Bc = I.gemm_operands(2, 96, 80, 72, seed=12)
+    Ac = Ac.copy(); Ac[1, 5, 7] = 70000
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    prev = bb.set_debug_checks(True)
+    try:
+        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=17)            # 70000 < 2^17: fine
+        with pytest.raises(bb.BbtnError) as e:
+            bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=3)
+        assert e.value.status == bb.BBTN_EINVAL and "count" in str(e.value)
+        Be2 = Be.copy(); Be2[0, 3, 3] = -(1 << 29) - 1                         # a non-canonical zero element
+        dBe2, _ = _to_dev(Be2, Bc)
+        with pytest.raises(bb.BbtnError) as e:
+            bb.tropical_gemm_batched(dAe, dAc, dBe2, dBc, count_bits=64)
+        assert e.value.status == bb.BBTN_EINVAL and "energy" in str(e.value)
+        with pytest.raises(bb.BbtnError):
+            bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=0)
+    finally:
+        bb.set_debug_checks(prev)
+
+
 def test_gemm_large_sampled_rows(bb, oracle):
     # BASELINE config 4a size n = 1024: full oracle is 1e9 FMAs; check 16 sampled rows of one batch entry
     n, B = 1024, 2
@@ -275,6 +312,64 @@ def test_config3_shape_branched_lattice_sampled(bb, oracle):
     assert (best, sum(int(x) for x in c[e == best]) & MASK64) == (whole[0], whole[1] & MASK64)
 
 
+# ---- divide-and-conquer trees: the joins run K2 + tiled K3 (automatic mode) and the long-reduction kernel ----
+def _king_ids(k, rows, cols):
+    ids = -np.ones((rows, cols), int)
+    ids[k.meta["keep"]] = np.arange(k.n_vertices)
+    return ids
+
+
+@pytest.mark.parametrize("case", ["ising12", "ising16", "king12", "ising12-sliced", "king12-sliced"])
+def test_block_tree_runs_tiled_gemm_and_trace_kernels(bb, oracle, case):
+    # four blocks contracted to boundary tensors, then joined: (TL x TR) and (BL x BR) are permute + tiled GEMM
+    # nodes in AUTOMATIC mode (>= 4 summed, >= 5 free indices on both sides), the last join is a 2^k-term trace
+    if case.startswith("ising"):
+        L = 16 if "16" in case else 12
+        inst = I.ising_lattice_2d(L, L, 3 if L == 12 else 4)
+        ids = None
+    else:
+        L = 12
+        inst = I.kings_subgraph(L, L, 1.0, 6, weights="rand")
+        ids = _king_ids(inst, L, L)
+    fixed, assign = None, None
+    if case.endswith("sliced"):
+        v = lambda r, c: r * L + c if ids is None else int(ids[r][c])
+        fixed = np.array([v(2, 2), v(2, L - 3), v(L - 3, 3)], np.int32)        # one private vertex in three of the blocks
+        assign = I.all_assignments(3)
+    parts = I.lattice_block_parts(L, L, [L // 2], [L // 2], ids, exclude=() if fixed is None else fixed)
+    tree = I.grouped_elimination_tree(inst.input_index_sets(() if fixed is None else fixed), parts)
+    h = bb.Handle(inst, tree=tree, flags=bb.BBTN_COUNT_CRT)
+    info = h.plan_query(fixed, 1 if assign is None else len(assign))
+    assert info["n_gemm_tiled"] > 0 and info["n_permute"] > 0 and info["n_trace"] > 0, info
+    energy, count, cmod = h.contract_batch(fixed, assign)
+    for b in range(len(energy)):
+        we, wc = oracle.contract_tree(inst, tree[0], tree[1], fixed, None if assign is None else assign[b])
+        assert (int(energy[b]), int(count[b])) == (we, wc & MASK64), (case, b)
+        assert (int(cmod[b, 0]), int(cmod[b, 1])) == (wc % bb.BBTN_P1, wc % bb.BBTN_P2), (case, b)
+    h.close()
+    if fixed is None:
+        assert (we, wc) == oracle.frontier_dp(inst)
+
+
+@pytest.mark.parametrize("mode", ["auto", "streaming"])
+def test_join_over_13_summed_indices(bb, oracle, mode):
+    # three column blocks of a 13-row lattice: the first join sums the 13 spins of a separator column into a
+    # rank-13 output (streaming K3 with a 2^13-term sum per output: more than 12 summed indices), the last join
+    # is a 13-index trace
+    inst = I.ising_lattice_2d(13, 7, 5)
+    parts = I.lattice_block_parts(13, 7, [], [2, 4])
+    tree = I.grouped_elimination_tree(inst.input_index_sets(), parts)
+    want = oracle.contract_tree(inst, *tree)
+    assert want == oracle.frontier_dp(inst)
+    h = bb.Handle(inst, tree=tree, flags=MODES[mode] | bb.BBTN_COUNT_CRT)
+    info = h.plan_query()
+    assert info["n_trace"] >= 1 and info["max_rank"] == 26
+    e, c, cm = h.contract_batch()
+    assert (int(e[0]), int(c[0])) == (want[0], want[1] & MASK64)
+    assert (int(cm[0, 0]), int(cm[0, 1])) == (want[1] % bb.BBTN_P1, want[1] % bb.BBTN_P2)
+    h.close()
+
+
 def test_batch_size_and_order_independence(bb):
     inst = I.ising_lattice_2d(8, 8, 3)
     fixed = I.slit_fixed_set_2d(8, 8, 4)
@@ -376,11 +471,47 @@ def _expect(name):
     return int(g["energy"]), int(g["count"]) & MASK64
 
 
+def _sampled_leaves(B, n, seed):
+    return sorted(set(int(x) for x in (I.splitmix64(seed, n, 21) % np.uint64(B))) | {0, B - 1})
+
+
+@pytest.mark.parametrize("f", [8, 10, 12])
+def test_config3_full_size_leaf_by_leaf(bb, oracle, f):
+    # BASELINE config 3 at full size in the launch configuration that is timed (all 2^f leaves, one call):
+    # 16 seeded leaves + the first and the last compared ONE BY ONE with the oracle's naive contraction of the same tree
+    inst = I.ising_lattice_2d(24, 24, 1)
+    fixed = I.slit_fixed_set_2d(24, 24, f)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(24, 24, f))
+    assign = I.all_assignments(f)
+    h = bb.Handle(inst, tree=tree, max_elements_per_leaf=1 << 26)
+    energy, count = h.contract_batch(fixed, assign)
+    h.close()
+    for b in _sampled_leaves(1 << f, 16, 100 + f):
+        we, wc = oracle.contract_tree(inst, tree[0], tree[1], fixed, assign[b])
+        assert (int(energy[b]), int(count[b])) == (we, wc & MASK64), (f, b)
+    assert bb.oplus_combine("ising", energy, count)[:2] == _expect("config3 ising 24x24 seed 1")
+
+
+@pytest.mark.parametrize("f", [6, 8, 10])
+def test_config4b_full_size_leaf_by_leaf(bb, oracle, f):
+    inst = I.ising_lattice_3d(5, 5, 5, 1)
+    fixed = I.layer_fixed_set_3d(5, 5, 5, f)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+    assign = I.all_assignments(f)
+    h = bb.Handle(inst, tree=tree, max_elements_per_leaf=1 << 26)
+    energy, count = h.contract_batch(fixed, assign)
+    h.close()
+    for b in _sampled_leaves(1 << f, 8 if f == 6 else 16, 200 + f):
+        we, wc = oracle.contract_tree(inst, tree[0], tree[1], fixed, assign[b])
+        assert (int(energy[b]), int(count[b])) == (we, wc & MASK64), (f, b)
+    assert bb.oplus_combine("ising", energy, count)[:2] == _expect("config4b ising 5x5x5 seed 1")
+
+
 def test_config3_full_size_24x24_all_leaves(bb):
     # the launch configuration time_to_solve.py times: slit of f spins, all 2^f leaves in one call
     from paper_2602_05470_b200 import time_to_solve as T
     inst = I.ising_lattice_2d(24, 24, 1)
-    for f in (8, 10):
+    for f in (8, 10, 12):
         fixed = I.slit_fixed_set_2d(24, 24, f)
         tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(24, 24, f))
         out = T.solve_branched("config3", inst, fixed, tree, repeat=1)

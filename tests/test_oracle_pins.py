@@ -430,3 +430,21 @@ def test_sparse_mis_dp_path_and_cycle(oracle):
         assert oracle.frontier_dp_mis_sparse(path) == ((n + 1) // 2, 1 if n % 2 else n // 2 + 1)
         cyc = _inst("mis", n, [(i, (i + 1) % n) for i in range(n)], None, None)
         assert oracle.frontier_dp_mis_sparse(cyc) == ((n // 2, 2) if n % 2 == 0 else ((n - 1) // 2, n))
+
+
+def test_block_trees_equal_exhaustive(oracle):
+    # divide-and-conquer trees (instances.grouped_elimination_tree: blocks contracted to boundary tensors, then
+    # joined) give the definition's result too: == exhaustive on <= 24 vertices, with and without a sliced leaf
+    for rows, cols, rc, cc in ((4, 6, [2], [3]), (5, 4, [2], [2]), (3, 8, [], [3, 5])):
+        inst = I.ising_lattice_2d(rows, cols, rows + cols, field_h=1)
+        tree = I.grouped_elimination_tree(inst.input_index_sets(), I.lattice_block_parts(rows, cols, rc, cc))
+        assert len(tree[0]) == inst.n_edges + inst.n_vertices - 1
+        assert oracle.contract_tree(inst, *tree) == oracle.exhaustive(inst)
+        fixed = np.array([1, cols + 1], np.int32)
+        parts = I.lattice_block_parts(rows, cols, rc, cc, exclude=fixed)
+        t2 = I.grouped_elimination_tree(inst.input_index_sets(fixed), parts)
+        for x in I.all_assignments(2):
+            assert oracle.contract_tree(inst, t2[0], t2[1], fixed, x) == oracle.exhaustive(inst, fixed, x)
+    k = I.kings_subgraph(4, 6, 1.0, 1, weights="rand")
+    tree = I.grouped_elimination_tree(k.input_index_sets(), I.lattice_block_parts(4, 6, [2], [3]))
+    assert oracle.contract_tree(k, *tree) == oracle.exhaustive(k)
