@@ -191,6 +191,34 @@ int bbtn_branching_leaves(bbtn_handle *h, int32_t log2_target, int64_t mem_budge
                           int64_t cap_leaves, int64_t cap_entries, int64_t *leaf_offsets, int32_t *leaf_vertices,
                           uint8_t *leaf_values, int64_t *stats, double *work);
 
+/* BBTN on sub-networks ("local branching"; PAPER.md:65-69, :67 boundary equivalence; readings A16, A25).
+ * The contraction tree (the caller's, else the library's tree of the unsliced network) is walked in order.  Where
+ * every tensor fits T_target = 2^log2_target elements the steps run once.  A stretch of the tree whose tensors
+ * overflow T_target is a sub-TN with open legs: it is decomposed by fixing a LOCAL set F of variables that are all
+ * summed inside it, chosen greedily to bring Eq. 4's overflow rho of the stretch to zero; every branch (assignment
+ * of F) is contracted by K1..K3 on slices of the stored tensors that enter the stretch, and the tensor that leaves
+ * it is the (+) over the branches -- per boundary state the (energy, count) of the interior.  Nothing
+ * outside a stretch is contracted more than once, so the cost is sum over stretches of 2^|F| x (its own cost)
+ * instead of 2^(sum |F|) x (the whole tree).  Branches are pruned before contraction: infeasible
+ * ones (MIS: two adjacent vertices of F set), and, when regions (as for bbtn_region_bound) and an incumbent are
+ * given, those whose K5 bound is strictly worse than the incumbent (ties kept, reading A14).
+ *   incumbent_hint  energy (reported units) of a feasible configuration known to the caller; BBTN_NEG_INF = none
+ *   mem_budget_bytes  0 = 94 % of the free device memory; the threshold is lowered until the arena fits
+ *   stats[0..9] = stretches, sliced stretches, branches planned (sum of 2^|F|), branches contracted, branches
+ *                 infeasible, branches pruned by bound, largest |F|, largest tensor rank, arena bytes, kernel launches
+ *   work[0..1]  = tropical FMAs, algorithmic bytes over all planned branches (12 B per element read or written)
+ * Host pointers only.  Errors: EINVAL, ESHAPE (a stretch needs more than 24 fixed variables, or the tree joins two
+ * overflowing parts so that no local set exists), ENOMEM, ECUDA. */
+int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes,
+                     const int32_t *region_offsets, const int32_t *region_vertices, int32_t n_regions,
+                     int32_t incumbent_hint,
+                     int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats, double *work,
+                     void *cuda_stream);
+
+/* The plan bbtn_solve_local would run, without running it (host only, no device): stats / work as above
+ * (the run-time entries 3, 4, 5, 9 are zero).  mem_budget_bytes = 0 means no memory limit here. */
+int bbtn_local_plan_query(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t *stats, double *work);
+
 /* Host-side (+) over leaf results in reported units (Eq. 3's outer sum; "the final
  * result is obtained by summing the contractions of each branch"): keeps the best
  * energy (Ising: lowest, MIS: highest), adds the counts of the leaves that attain it (mod 2^64,

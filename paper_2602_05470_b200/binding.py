@@ -23,7 +23,7 @@ BBTN_COUNT_CRT, BBTN_IO_DEVICE, BBTN_NO_GRAPH = 0x1, 0x2, 0x4
 BBTN_FORCE_STREAMING, BBTN_FORCE_TILED = 0x10, 0x20
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
-EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves",
+EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query",
            "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
            "bbtn_permute_batched", "bbtn_int32_microbench", "bbtn_crt_combine", "bbtn_set_debug_checks",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
@@ -67,6 +67,8 @@ def load():
     lib.bbtn_solve_bb.argtypes = [vp, vp, i32, i32, vp, vp, i32, i64, i32, i32, vp, vp, vp, vp, vp]
     lib.bbtn_solve_branching.argtypes = [vp, i32, i64, i64, vp, vp, vp, vp, vp, vp]
     lib.bbtn_branching_leaves.argtypes = [vp, i32, i64, i64, i64, i64, vp, vp, vp, vp, vp]
+    lib.bbtn_solve_local.argtypes = [vp, i32, i64, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.bbtn_local_plan_query.argtypes = [vp, i32, i64, vp, vp]
     lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
     lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
     lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
@@ -210,6 +212,33 @@ class Handle:
                "max_fixed": stats[2], "rho_root": stats[3], "fma": work[0], "bytes": work[1]}
         if crt:
             out["count_mod"] = (cm[0], cm[1])
+        return out
+
+    _LOCAL_STATS = ("stretches", "sliced_stretches", "branches_planned", "branches_contracted", "branches_infeasible",
+                    "branches_pruned", "max_fixed", "max_rank", "arena_bytes", "kernel_launches")
+
+    def solve_local(self, log2_target: int, mem_budget_bytes: int = 0, region_offsets=None, region_vertices=None,
+                    incumbent_hint=BBTN_NEG_INF, stream=None):
+        """bbtn_solve_local: BBTN on sub-networks (local fixed sets per overflowing stretch of the tree)."""
+        e = C.c_int32(); c = C.c_uint64(); cm = (C.c_uint32 * 2)(); stats = (C.c_int64 * 10)(); work = (C.c_double * 2)()
+        crt = bool(self.flags & BBTN_COUNT_CRT)
+        ro = None if region_offsets is None else _np(region_offsets, np.int32)
+        rv = None if region_vertices is None else _np(region_vertices, np.int32)
+        _check(load().bbtn_solve_local(self._h, log2_target, mem_budget_bytes, _ptr(ro), _ptr(rv), 0 if ro is None else len(ro) - 1,
+                                       incumbent_hint, C.addressof(e), C.addressof(c), C.addressof(cm) if crt else None,
+                                       C.addressof(stats), C.addressof(work), _stream(stream)), self._h)
+        out = {"energy": e.value, "count": c.value, "fma": work[0], "bytes": work[1]}
+        out.update({k: stats[i] for i, k in enumerate(self._LOCAL_STATS)})
+        if crt:
+            out["count_mod"] = (cm[0], cm[1])
+        return out
+
+    def local_plan_query(self, log2_target: int, mem_budget_bytes: int = 0) -> dict:
+        """bbtn_local_plan_query (host only)."""
+        stats = (C.c_int64 * 10)(); work = (C.c_double * 2)()
+        _check(load().bbtn_local_plan_query(self._h, log2_target, mem_budget_bytes, C.addressof(stats), C.addressof(work)), self._h)
+        out = {"fma": work[0], "bytes": work[1]}
+        out.update({k: stats[i] for i, k in enumerate(self._LOCAL_STATS)})
         return out
 
     def branching_leaves(self, log2_target: int, mem_budget_bytes: int = 0, max_leaves: int = 0, store: bool = True,

@@ -188,6 +188,24 @@ __global__ void finalize_kernel(int kind, int64_t B, const int32_t *__restrict__
   }
 }
 
+// acc (+)= offset (.) slice   (local slicing: the (+) over the slices of a segment)
+template <class R>
+__global__ void accumulate_kernel(int64_t n, const int32_t *__restrict__ slice_e, const typename R::T *__restrict__ slice_c,
+                                  const int32_t *__restrict__ off_e, const typename R::T *__restrict__ off_c,
+                                  int32_t *__restrict__ acc_e, typename R::T *__restrict__ acc_c, int first) {
+  int32_t oe = 0; typename R::T oc = R::from_small(1);
+  if (slice_e) { oe = off_e[0]; oc = off_c[0]; }
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    int32_t e = NEG_INF; typename R::T c = 0;
+    if (slice_e) {
+      e = slice_e[i] + oe; c = R::mul(slice_c[i], oc);
+      canonicalise<R>(e, c);
+      if (!first) { int32_t ae = acc_e[i]; typename R::T ac = acc_c[i]; oplus<R>(ae, ac, e, c); e = ae; c = ac; }
+    }
+    acc_e[i] = e; acc_c[i] = c;
+  }
+}
+
 inline int grid_for(int64_t total, int block) {
   int64_t g = (total + block - 1) / block;
   const int64_t cap = 148 * 16;          // grid-stride beyond 16 CTAs per SM
@@ -242,6 +260,15 @@ void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
   BBTN_RING_DISPATCH(ring, {
     using CT = typename R::T;
     reduce_kernel<R><<<(unsigned)total, 256, 0, st>>>(p, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc);
+  });
+}
+
+void launch_accumulate(int64_t n, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
+                       int32_t *acc_e, void *acc_c, int first, int ring, cudaStream_t st) {
+  BBTN_RING_DISPATCH(ring, {
+    using CT = typename R::T;
+    accumulate_kernel<R><<<grid_for(n, 256), 256, 0, st>>>(n, slice_e, (const CT *)slice_c, off_e, (const CT *)off_c, acc_e,
+                                                           (CT *)acc_c, first);
   });
 }
 

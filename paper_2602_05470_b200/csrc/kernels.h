@@ -46,6 +46,12 @@ void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_
                            const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
                            int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, cudaStream_t st);
 
+// Local slicing: acc (+)= offset (.) slice, element-wise over n elements (first = 1: acc = offset (.) slice); the
+// zero tensor when slice_e == nullptr.  offset is one element on the device.  (+) over the assignments of a segment's
+// locally fixed indices (Eq. 3, on a sub-network; plan.h "local slicing").
+void launch_accumulate(int64_t n, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
+                       int32_t *acc_e, void *acc_c, int first, int ring, cudaStream_t st);
+
 // K4: (E[b], c[b]) = offset[b] (.) root[b]; canonicalise; convert to reported units.
 //   root_e == nullptr: the network is all scalars.  root_stride 0: root is leaf-invariant.
 void launch_finalize(int kind, int64_t B, const int32_t *root_e, const void *root_c, int64_t root_stride,

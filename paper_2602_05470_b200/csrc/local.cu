@@ -1,0 +1,251 @@
+// local.cu -- BBTN on sub-networks: bbtn_solve_local / bbtn_local_plan_query (include/bbtn.h).
+//
+// The contraction tree is walked in SSA order.  Where every tensor fits T_target the steps run once.  A
+// segment whose tensors overflow T_target is a sub-TN with open legs; it is decomposed by fixing a LOCAL set F
+// of variables that are summed inside it ("decomposes a tensor network into multiple smaller
+// sub-TNs by fixing a subset of variables"), one contraction per assignment x of F (Eq. 3), and
+// its boundary tensor is the (+) over the branches ("summing the contractions of each branch";
+// per boundary state the (energy, count) of the interior: the counting form of the boundary-equivalence
+// principle, reading A16).  F is chosen to bring Eq. 4's overflow of the segment to
+// zero (plan.cpp make_local_plan).  Branches are pruned before they are contracted: infeasible
+// ones (MIS: two adjacent variables of F set) and, when the caller supplies regions and an incumbent, those
+// whose K5 region bound is strictly worse than the incumbent (reading A14).
+// Host logic only: tensors are built, contracted and (+)-accumulated by the kernels (kernels.h).
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "handle.h"
+
+using namespace bbtn;
+
+namespace {
+
+struct LocalRun {
+  bbtn_handle *h; const Problem *P; LocalPlan *lp; cudaStream_t st;
+  DevBuf inputs, lists, assign, arena_e, arena_c, off_e, off_c, res_e, res_c, res_m;
+  std::vector<int32_t> list_host; std::vector<int64_t> var_at, sc_at;   // per segment: position of its lists in `lists`
+  int64_t gsc_at = 0; int n_gsc = 0;                                    // scalars of the run-once segments, all together
+  int64_t n_contracted = 0, n_infeasible = 0, n_pruned = 0, n_launches = 0;
+  // pruning inputs
+  const int32_t *roff = nullptr, *rv = nullptr; int n_regions = 0; bool have_inc = false; int32_t inc = 0;
+
+  int upload() {
+    const Plan &pl = lp->plan;
+    CUDA_TRY(h, inputs.ensure(pl.inputs.size() * sizeof(InputRec)));
+    CUDA_TRY(h, cudaMemcpy(inputs.p, pl.inputs.data(), pl.inputs.size() * sizeof(InputRec), cudaMemcpyHostToDevice));
+    for (const LocalSeg &s : lp->segs) {
+      var_at.push_back((int64_t)list_host.size()); list_host.insert(list_host.end(), s.list_var.begin(), s.list_var.end());
+      sc_at.push_back((int64_t)list_host.size());
+      if (!s.fixed.empty()) list_host.insert(list_host.end(), s.list_scalar.begin(), s.list_scalar.end());
+    }
+    gsc_at = (int64_t)list_host.size();
+    for (const LocalSeg &s : lp->segs) if (s.fixed.empty()) { list_host.insert(list_host.end(), s.list_scalar.begin(), s.list_scalar.end()); n_gsc += (int)s.list_scalar.size(); }
+    CUDA_TRY(h, lists.upload(list_host));
+    CUDA_TRY(h, arena_e.ensure((size_t)pl.arena_variant_elems * 4));
+    CUDA_TRY(h, arena_c.ensure((size_t)pl.arena_variant_elems * 8));
+    CUDA_TRY(h, off_e.ensure(4 * 4)); CUDA_TRY(h, off_c.ensure(4 * 8));
+    CUDA_TRY(h, res_e.ensure(4)); CUDA_TRY(h, res_c.ensure(8)); CUDA_TRY(h, res_m.ensure(8));
+    return BBTN_OK;
+  }
+
+  void launch_steps(const LocalSeg &s, uint32_t x, int ring) {
+    const Plan &pl = lp->plan;
+    int32_t *ve = (int32_t *)arena_e.p; char *vc = (char *)arena_c.p;
+    const size_t csz = ring == 0 ? 8 : 4;
+    auto pe = [&](int64_t off) { return ve + off; };
+    auto pc = [&](int64_t off) { return (void *)(vc + (size_t)off * csz); };
+    for (int q = s.step_begin; q < s.step_end; q++) {
+      const Step &sp = pl.steps[q];
+      int64_t oa = sp.offA, ob = sp.offB;
+      for (int j = 0; j < sp.n_slice; j++) if ((x >> j) & 1u) { oa += sp.sliceA[j]; ob += sp.sliceB[j]; }
+      if (sp.kind == STEP_ABSORB) launch_absorb(sp, 1, pe(oa), pc(oa), pe(ob), pc(ob), pe(sp.offC), pc(sp.offC), ring, st);
+      else launch_reduce(sp, 1, pe(oa), pc(oa), pe(ob), pc(ob), pe(sp.offC), pc(sp.offC), ring, st);
+      n_launches++;
+    }
+  }
+
+  int run_ring(int ring, int32_t *d_energy, uint64_t *d_count, uint32_t *d_mod) {
+    const Plan &pl = lp->plan;
+    const int kind = P->kind;
+    int32_t *ve = (int32_t *)arena_e.p; char *vc = (char *)arena_c.p;
+    const size_t csz = ring == 0 ? 8 : 4;
+    const InputRec *d_in = (const InputRec *)inputs.p;
+    const int32_t *d_l = (const int32_t *)lists.p;
+    int32_t *oe = (int32_t *)off_e.p; char *oc = (char *)off_c.p;
+    // slot 0: (.) of the scalar inputs of the run-once segments; slot 1: of the current slice; slot 2: scratch
+    launch_construct(kind, d_in, nullptr, 0, nullptr, 0, d_l + gsc_at, n_gsc, nullptr, 0, 1, ve, vc, nullptr, nullptr, oe, oc, ring, st);
+    n_launches++;
+    for (size_t si = 0; si < lp->segs.size(); si++) {
+      const LocalSeg &s = lp->segs[si];
+      const int f = (int)s.fixed.size();
+      if (f == 0) {
+        launch_construct(kind, d_in, d_l + var_at[si], (int)s.list_var.size(), nullptr, 0, nullptr, 0, nullptr, 0, 1, ve, vc,
+                         nullptr, nullptr, oe + 2, oc + 2 * csz, ring, st);
+        n_launches += 2;
+        launch_steps(s, 0, ring);
+        continue;
+      }
+      // ---- a sliced segment: enumerate the assignments of F, prune, contract, (+)-accumulate
+      std::vector<std::pair<int, int>> adj_pairs;            // MIS: positions in F of adjacent fixed vertices
+      if (kind == BBTN_MIS) {
+        std::vector<int> posF(P->n, -1);
+        for (int j = 0; j < f; j++) posF[s.fixed[j]] = j;
+        for (int e = 0; e < P->m; e++) if (posF[P->eu[e]] >= 0 && posF[P->ev[e]] >= 0) adj_pairs.push_back({posF[P->eu[e]], posF[P->ev[e]]});
+      }
+      const uint32_t n_x = 1u << f;
+      const uint32_t chunk = std::min<uint32_t>(n_x, 1u << 14);
+      bool first = true;
+      for (uint32_t x0 = 0; x0 < n_x; x0 += chunk) {
+        std::vector<uint8_t> rows((size_t)chunk * f);
+        for (uint32_t i = 0; i < chunk; i++) for (int j = 0; j < f; j++) rows[(size_t)i * f + j] = (uint8_t)(((x0 + i) >> j) & 1u);
+        std::vector<char> skip(chunk, 0);
+        for (uint32_t i = 0; i < chunk; i++)
+          for (auto &pr : adj_pairs) if ((((x0 + i) >> pr.first) & 1u) && (((x0 + i) >> pr.second) & 1u)) { skip[i] = 1; break; }
+        if (ring == 0) for (uint32_t i = 0; i < chunk; i++) n_infeasible += skip[i];
+        if (have_inc && n_regions > 0) {
+          // global pruning: a branch whose bound is strictly worse than the incumbent holds no optimum
+          std::vector<int32_t> bound(chunk);
+          int rc = bbtn_region_bound(h, roff, rv, n_regions, s.fixed.data(), f, rows.data(), chunk, bound.data(), st);
+          if (rc) return rc;
+          for (uint32_t i = 0; i < chunk; i++) {
+            if (skip[i]) continue;
+            const bool worse = kind == BBTN_ISING ? bound[i] > inc : bound[i] < inc;
+            if (bound[i] == BBTN_NEG_INF || worse) { skip[i] = 1; if (ring == 0) n_pruned++; }
+          }
+        }
+        CUDA_TRY(h, assign.ensure(rows.size()));
+        CUDA_TRY(h, cudaMemcpyAsync(assign.p, rows.data(), rows.size(), cudaMemcpyHostToDevice, st));
+        for (uint32_t i = 0; i < chunk; i++) {
+          if (skip[i]) continue;
+          launch_construct(kind, d_in, d_l + var_at[si], (int)s.list_var.size(), nullptr, 0, d_l + sc_at[si], (int)s.list_scalar.size(),
+                           (const uint8_t *)assign.p + (size_t)i * f, f, 1, ve, vc, nullptr, nullptr, oe + 1, oc + csz, ring, st);
+          launch_steps(s, x0 + i, ring);
+          launch_accumulate((int64_t)1 << s.acc_rank, ve + s.tmp_off, vc + (size_t)s.tmp_off * csz, oe + 1, oc + csz,
+                            ve + s.acc_off, vc + (size_t)s.acc_off * csz, first ? 1 : 0, ring, st);
+          n_launches += 3;
+          first = false;
+          if (ring == 0) n_contracted++;
+        }
+        CUDA_TRY(h, cudaStreamSynchronize(st));               // `rows` is about to go out of scope
+      }
+      if (first) {                                            // every branch pruned: the boundary tensor is the zero tensor
+        launch_accumulate((int64_t)1 << s.acc_rank, nullptr, nullptr, nullptr, nullptr, ve + s.acc_off, vc + (size_t)s.acc_off * csz, 1, ring, st);
+        n_launches++;
+      }
+    }
+    const bool has_root = pl.result_offset >= 0;
+    launch_finalize(kind, 1, has_root ? ve + pl.result_offset : nullptr, has_root ? vc + (size_t)pl.result_offset * csz : nullptr, 0,
+                    oe, oc, d_energy, d_count, d_mod, ring, st);
+    n_launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    return BBTN_OK;
+  }
+};
+
+// Candidate trees: the caller's tree if there is one; else elimination trees along the vertex-id order, the
+// min-degree order and nested-min-cut sweeps with several look-ahead windows (plan.cpp).  The driver plans
+// every candidate and keeps the cheapest one that fits.
+void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out) {
+  const Problem &P0 = h->P;
+  if (!P0.tree_l.empty() || P0.n + P0.m <= 1) { out.push_back(std::make_unique<Problem>(P0)); return; }
+  std::vector<std::vector<int>> orders;
+  std::vector<int> natural(P0.n);
+  for (int v = 0; v < P0.n; v++) natural[v] = v;
+  orders.push_back(natural);
+  orders.push_back(min_degree_order(P0, {}));
+  int w0 = 0; double c0 = 0;
+  { std::vector<int32_t> l, r; elimination_tree_for_order(P0, {}, natural, l, r, w0, c0); }
+  for (int mult : {2, 3, 4, 5, 6, 8}) orders.push_back(mincut_sweep_order(P0, 4, std::max(8, mult * w0)));
+  for (auto &o : orders) {
+    auto P = std::make_unique<Problem>(P0);
+    int w = 0; double c = 0;
+    elimination_tree_for_order(P0, {}, o, P->tree_l, P->tree_r, w, c);
+    out.push_back(std::move(P));
+  }
+}
+
+void write_plan_stats(const LocalPlan &lp, int64_t *stats, double *work) {
+  if (stats) {
+    std::memset(stats, 0, 10 * sizeof(int64_t));
+    stats[0] = (int64_t)lp.segs.size(); stats[1] = lp.n_sliced_segs;
+    stats[2] = lp.n_slices > 9e18 ? INT64_MAX : (int64_t)lp.n_slices;
+    stats[6] = lp.max_fixed; stats[7] = lp.plan.max_rank; stats[8] = lp.plan.arena_variant_elems * 12;
+  }
+  if (work) { work[0] = lp.fma_total; work[1] = lp.bytes_total; }
+}
+
+// plan at log2_target, lowering the threshold while no candidate's arena fits the memory budget; among the
+// candidates that fit, the one that moves the fewest bytes
+int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, LocalPlan &lp, std::unique_ptr<Problem> &P_out) {
+  std::vector<std::unique_ptr<Problem>> cands;
+  candidate_trees(h, cands);
+  std::string last_err; int last_rc = BBTN_ESHAPE;
+  for (int cap = log2_target; cap >= 1; cap--) {
+    int best = -1; LocalPlan best_lp;
+    for (size_t i = 0; i < cands.size(); i++) {
+      LocalPlan cur; std::string err;
+      int rc = make_local_plan(*cands[i], cap, cur, err);
+      if (rc) { last_rc = rc; last_err = err; continue; }
+      if (budget > 0 && cur.plan.arena_variant_elems * 12 > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
+      if (best < 0 || cur.bytes_total < best_lp.bytes_total) { best = (int)i; best_lp = std::move(cur); }
+    }
+    if (best >= 0) { lp = std::move(best_lp); P_out = std::move(cands[best]); return BBTN_OK; }
+  }
+  return fail(h, last_rc, last_err);
+}
+
+}  // namespace
+
+extern "C" {
+
+int bbtn_local_plan_query(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t *stats, double *work) {
+  if (!h) return fail(nullptr, BBTN_EINVAL, "null handle");
+  if (log2_target < 1 || log2_target > 32) return fail(h, BBTN_EINVAL, "log2_target must be in 1..32");
+  LocalPlan lp; std::unique_ptr<Problem> P;
+  int rc = plan_within_budget(h, log2_target, mem_budget_bytes, lp, P);
+  if (rc) return rc;
+  write_plan_stats(lp, stats, work);
+  return BBTN_OK;
+}
+
+int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes,
+                     const int32_t *region_offsets, const int32_t *region_vertices, int32_t n_regions, int32_t incumbent_hint,
+                     int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats, double *work, void *stream) {
+  if (!h) return fail(nullptr, BBTN_EINVAL, "null handle");
+  if (!energy || !count || n_regions < 0 || (n_regions > 0 && (!region_offsets || !region_vertices)))
+    return fail(h, BBTN_EINVAL, "bad solve_local arguments");
+  if (log2_target < 1 || log2_target > 32) return fail(h, BBTN_EINVAL, "log2_target must be in 1..32");
+  if (h->P.flags & BBTN_IO_DEVICE) return fail(h, BBTN_EINVAL, "bbtn_solve_local needs a host-pointer handle");
+  const bool crt = (h->P.flags & BBTN_COUNT_CRT) != 0;
+  if (count_mod && !crt) return fail(h, BBTN_EINVAL, "count_mod needs a handle built with BBTN_COUNT_CRT");
+  if (!have_device()) return fail(h, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  if (mem_budget_bytes <= 0) {
+    size_t free_b = 0, total_b = 0;
+    CUDA_TRY(h, cudaMemGetInfo(&free_b, &total_b));
+    mem_budget_bytes = (int64_t)((double)free_b * 0.94);
+  }
+  LocalPlan lp; std::unique_ptr<Problem> Pt;
+  int rc = plan_within_budget(h, log2_target, mem_budget_bytes, lp, Pt);
+  if (rc) return rc;
+  const Problem *P = Pt.get();
+  LocalRun run{h, P, &lp, (cudaStream_t)stream};
+  run.roff = region_offsets; run.rv = region_vertices; run.n_regions = n_regions;
+  run.have_inc = incumbent_hint != BBTN_NEG_INF; run.inc = incumbent_hint;
+  if ((rc = run.upload())) return rc;
+  const int n_rings = (crt && count_mod) ? 3 : 1;
+  for (int ring = 0; ring < n_rings; ring++)
+    if ((rc = run.run_ring(ring, (int32_t *)run.res_e.p, (uint64_t *)run.res_c.p, (uint32_t *)run.res_m.p))) return rc;
+  int32_t e; uint64_t c; uint32_t cm[2] = {0, 0};
+  CUDA_TRY(h, cudaMemcpyAsync(&e, run.res_e.p, 4, cudaMemcpyDeviceToHost, run.st));
+  CUDA_TRY(h, cudaMemcpyAsync(&c, run.res_c.p, 8, cudaMemcpyDeviceToHost, run.st));
+  if (n_rings == 3) CUDA_TRY(h, cudaMemcpyAsync(cm, run.res_m.p, 8, cudaMemcpyDeviceToHost, run.st));
+  CUDA_TRY(h, cudaStreamSynchronize(run.st));
+  *energy = e; *count = c;
+  if (count_mod) { count_mod[0] = cm[0]; count_mod[1] = cm[1]; }
+  write_plan_stats(lp, stats, work);
+  if (stats) { stats[3] = run.n_contracted; stats[4] = run.n_infeasible; stats[5] = run.n_pruned; stats[9] = run.n_launches; }
+  return BBTN_OK;
+}
+
+}  // extern "C"

@@ -60,6 +60,10 @@ struct Step {
   // upper bound on log2(count + 1) of BOTH operands (inputs hold counts 0/1, each (.) adds the operands' bounds,
   // each (+) over 2^k terms adds k): lets K3 pick its narrow count modes inside a tree; 64 = no useful bound
   int32_t count_bits = 64;
+  // local slicing (make_local_plan): an operand that is a view of a stored tensor starts at
+  // off + sum_j x_j * slice[j], x = the current assignment of the segment's fixed indices
+  int32_t n_slice = 0;
+  uint32_t sliceA[24] = {0}, sliceB[24] = {0};
   double fma = 0;               // tropical FMAs of this launch per batch entry
   double bytes = 0;             // algorithmic bytes per batch entry (12 B per element moved)
 };
@@ -83,6 +87,37 @@ struct Plan {
   std::vector<std::vector<int32_t>> node_labels;
 };
 
+// ---- local slicing (BBTN on sub-networks) -------------------------------------------------------
+// The tree is walked in SSA order and cut into SEGMENTS.  A segment whose tensors fit T_target runs once.
+// A segment that holds tensors above T_target gets a LOCAL fixed set F (indices that are summed inside the
+// segment): the segment is contracted once per assignment x of F (Eq. 3, applied to the sub-TN)
+// with every tensor carrying an index of F cut down to its x-slice, and the one tensor that leaves the
+// segment and depends on F is the (+) over x of the slices' results -- for every state of the segment's
+// boundary the (energy, count) of its interior (the counting form of the boundary-equivalence principle,
+// PAPER.md:67; reading A16).  Tensors that enter a sliced segment are stored in full and read
+// through strided views, so nothing outside the segment is ever contracted twice.
+struct LocalSeg {
+  std::vector<int32_t> fixed;            // F; empty = the segment runs once
+  int32_t step_begin = 0, step_end = 0;  // range in Plan::steps
+  std::vector<int32_t> list_var;         // inputs K1 builds at the start of every slice (rank > 0 under F)
+  std::vector<int32_t> list_scalar;      // inputs that are scalars under F: their product is the slice's offset
+  int32_t acc_rank = -1;                 // sliced segments: the F-dependent tensor leaving the segment ...
+  int64_t acc_off = 0, tmp_off = 0;      // ... is accumulated at acc_off from the per-slice result at tmp_off
+  int32_t max_rank = 0;
+  double fma = 0, bytes = 0;             // per slice (bytes include the accumulation pass)
+};
+struct LocalPlan {
+  Plan plan;                             // inputs (each under its segment's F), all steps, arena size, result offset
+  std::vector<LocalSeg> segs;
+  int32_t cap_rank = 0;
+  double fma_total = 0, bytes_total = 0; // over all slices of all segments (infeasible slices included)
+  double n_slices = 0;                   // sum over segments of 2^|F|
+  int32_t max_fixed = 0, n_sliced_segs = 0;
+};
+// P must carry a tree (tree_l/tree_r non-empty).  cap_rank = log2 T_target.  Returns 0 or a status; ESHAPE when a
+// segment cannot be brought under T_target (needs more than 24 fixed indices, or the tree joins two sliced parts).
+int make_local_plan(const Problem &P, int cap_rank, LocalPlan &out, std::string &err);
+
 // Returns 0 or a bbtn_status value; err receives the message.
 // force_mode: 0 = automatic, 1 = never use the tiled GEMM path, 2 = use it wherever |K| >= 1.
 // enforce_cap: fail with ESHAPE when a tensor exceeds P.max_elements (otherwise only rho records it).
@@ -94,5 +129,12 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
 // Elimination-order tree for the network with `fixed` sliced out (used when the caller gave no tree).
 void derive_tree(const Problem &P, const std::vector<int32_t> &fixed,
                  std::vector<int32_t> &tl, std::vector<int32_t> &tr);
+
+// Building blocks of derive_tree, also used by the local-branching driver to pick its tree: bucket elimination along a
+// vertex order, and two order heuristics (plan.cpp).
+void elimination_tree_for_order(const Problem &P, const std::vector<int32_t> &fixed, const std::vector<int> &order,
+                                std::vector<int32_t> &tl, std::vector<int32_t> &tr, int &width, double &cost);
+std::vector<int> min_degree_order(const Problem &P, const std::vector<int32_t> &fixed);
+std::vector<int> mincut_sweep_order(const Problem &P, int delta, int window);
 
 }  // namespace bbtn

@@ -105,6 +105,36 @@ def solve_king_bbtn(L, seed=1, log2_target=31, crt=True):
             "algorithmic_gb_per_s": out["bytes"] * rings / dt / 1e9}
 
 
+def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None):
+    """BBTN on sub-networks (bbtn_solve_local): local fixed sets per overflowing stretch of the tree, K5 region bounds
+    against the caller's incumbent (if any) on every branch."""
+    k = I.kings_subgraph(L, L, 0.8, seed)
+    ids = -np.ones((L, L), int)
+    ids[k.meta["keep"]] = np.arange(k.n_vertices)
+    offs, verts = [0], []
+    for r0 in range(0, L, block):
+        for c0 in range(0, L, block):
+            verts += [int(ids[r][c]) for r in range(r0, min(r0 + block, L)) for c in range(c0, min(c0 + block, L)) if ids[r][c] >= 0]
+            offs.append(len(verts))
+    h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT if crt else 0)
+    t0 = time.perf_counter()
+    plan = h.local_plan_query(log2_target)
+    t_plan = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    out = h.solve_local(log2_target, region_offsets=offs, region_vertices=verts,
+                        incumbent_hint=bb.BBTN_NEG_INF if hint is None else hint)
+    dt = time.perf_counter() - t0
+    h.close()
+    cnt = bb.crt_combine(out["count"], *out["count_mod"]) if crt else out["count"]
+    rings = 3 if crt else 1
+    return {"instance": f"king {L}x{L} p0.8 seed {seed}", "mode": f"BBTN on sub-networks (bbtn_solve_local), T_target = 2^{log2_target}"
+            + (", counts mod 2^64, p1, p2 (3 passes) CRT-combined" if crt else ""),
+            "n_vertices": k.n_vertices, "n_edges": k.n_edges, "seconds": dt, "plan_only_seconds": t_plan, "energy": out["energy"],
+            "count_mod_2_64": out["count"], "count": str(cnt), **{key: out[key] for key in bb.Handle._LOCAL_STATS},
+            "fma": out["fma"] * rings, "bytes": out["bytes"] * rings,
+            "algorithmic_gb_per_s": (out["bytes"] * 12 + out["bytes"] * 8 * (rings - 1)) / 12 / dt / 1e9}
+
+
 def solve_e1(L, seed=1, log2_target=32):
     """The paper's spin-glass setting (+-J, field 0.5 -> 2J, h = 1, half units) unbranched: one leaf of width L+1."""
     inst = I.ising_lattice_2d_half_field(L, L, seed)
@@ -124,6 +154,7 @@ def main():
     ap.add_argument("--configs", nargs="*", default=["1", "2", "3", "4b", "5"])
     ap.add_argument("--king-sizes", nargs="*", type=int, default=[16, 20, 24])
     ap.add_argument("--bbtn", nargs="*", default=[], help="L:seed:log2_target[:crt] runs of bbtn_solve_branching, e.g. 32:1:31:1")
+    ap.add_argument("--local", nargs="*", default=[], help="L:seed:log2_target[:crt] runs of bbtn_solve_local, e.g. 40:1:32:1")
     ap.add_argument("--e1", nargs="*", type=int, default=[], help="lattice sizes L for the paper's +-J, h = 0.5 setting, unbranched")
     ap.add_argument("--repeat", type=int, default=5)
     a = ap.parse_args()
@@ -152,6 +183,9 @@ def main():
             emit(solve_king_bb(L))
     for L in a.e1:
         emit(solve_e1(L))
+    for spec in a.local:
+        f = [int(x) for x in spec.split(":")]
+        emit(solve_king_local(f[0], f[1], f[2], crt=bool(f[3]) if len(f) > 3 else False))
     for spec in a.bbtn:
         f = [int(x) for x in spec.split(":")]
         emit(solve_king_bbtn(f[0], f[1], f[2], crt=bool(f[3]) if len(f) > 3 else False))

@@ -600,6 +600,93 @@ def test_solve_branching_king32_seed1_rank32_leaves(bb):
     h.close()
 
 
+# ---- BBTN on sub-networks: local fixed sets per overflowing stretch of the tree (bbtn_solve_local) ----
+@pytest.mark.parametrize("name,make,t,flags,own_tree", [
+    ("king10", lambda: I.kings_subgraph(10, 10, 0.8, 2), 6, 0, False),
+    ("king12-crt", lambda: I.kings_subgraph(12, 12, 0.8, 3), 7, 1, False),
+    ("king12-sweep", lambda: I.kings_subgraph(12, 12, 0.8, 4, weights="rand"), 8, 0, True),
+    ("king9-full-crt", lambda: I.kings_subgraph(9, 9, 1.0, 0), 5, 1, True),
+    ("ising8", lambda: I.ising_lattice_2d(8, 8, 4), 5, 0, True),
+    ("ising10-field-crt", lambda: I.ising_lattice_2d_half_field(10, 10, 7), 6, 1, False),
+    ("cube3-crt", lambda: I.ising_lattice_3d(3, 3, 3, 2), 6, 1, False),
+    ("cube4", lambda: I.ising_lattice_3d(4, 4, 3, 5), 9, 0, True),
+    ("random-mis", lambda: I.random_graph(26, 0.2, 9, "mis"), 4, 1, False),
+])
+def test_solve_local_matches_oracle(bb, oracle, name, make, t, flags, own_tree):
+    inst = make()
+    ref_e, ref_c = oracle.frontier_dp(inst)
+    tree = I.elimination_tree(inst.input_index_sets(), I.natural_order(inst.n_vertices)) if own_tree else None
+    h = bb.Handle(inst, tree=tree, flags=flags)
+    out = h.solve_local(t)
+    assert out["sliced_stretches"] >= 1 and out["max_fixed"] >= 1 and out["max_rank"] <= t, out
+    assert out["branches_contracted"] + out["branches_infeasible"] == out["branches_planned"]
+    assert (out["energy"], out["count"]) == (ref_e, ref_c & MASK64), (name, out)
+    if flags:
+        assert out["count_mod"] == (ref_c % bb.BBTN_P1, ref_c % bb.BBTN_P2)
+    one = h.solve_local(30)                        # threshold above the width: a single stretch that runs once
+    assert one["sliced_stretches"] == 0 and one["branches_contracted"] == 0
+    assert (one["energy"], one["count"]) == (ref_e, ref_c & MASK64)
+    # a smaller threshold means more, smaller branches and the same result
+    two = h.solve_local(max(t - 2, 2))
+    assert two["max_rank"] <= max(t - 2, 2) and (two["energy"], two["count"]) == (ref_e, ref_c & MASK64)
+    h.close()
+
+
+@pytest.mark.parametrize("kind", ["mis", "ising"])
+def test_solve_local_prunes_with_region_bounds(bb, oracle, kind):
+    # global pruning inside the local-branching driver: with K5 regions and an incumbent, branches whose
+    # bound is strictly worse are never contracted; ties are kept, so the count stays exact (reading A14)
+    if kind == "mis":
+        rows = cols = 12
+        inst = I.kings_subgraph(rows, cols, 0.8, 5)
+        ids = _king_ids(inst, rows, cols)
+    else:
+        rows = cols = 9
+        inst = I.ising_lattice_2d(rows, cols, 8, field_h=1)
+        ids = None
+    offs, verts = _grid_regions(rows, cols, 3, 3, ids)
+    ref_e, ref_c = oracle.frontier_dp(inst)
+    h = bb.Handle(inst, flags=bb.BBTN_COUNT_CRT)
+    plain = h.solve_local(6)
+    exact = h.solve_local(6, region_offsets=offs, region_vertices=verts, incumbent_hint=ref_e)
+    loose = h.solve_local(6, region_offsets=offs, region_vertices=verts, incumbent_hint=ref_e + (3 if kind == "ising" else -3))
+    for out in (plain, exact, loose):
+        assert (out["energy"], out["count"]) == (ref_e, ref_c & MASK64)
+        assert out["count_mod"] == (ref_c % bb.BBTN_P1, ref_c % bb.BBTN_P2)
+        assert out["branches_contracted"] + out["branches_infeasible"] + out["branches_pruned"] == out["branches_planned"]
+    assert plain["branches_pruned"] == 0 and exact["branches_pruned"] >= loose["branches_pruned"]
+    assert exact["branches_contracted"] <= plain["branches_contracted"]
+    h.close()
+
+
+@pytest.mark.parametrize("L,seed,t", [(28, 1, 29), (32, 1, 31), (32, 2, 30), (36, 1, 32)])
+def test_solve_local_kings_large(bb, L, seed, t):
+    # King's subgraphs at filling 0.8 beyond the reach of one dense contraction at the threshold: goldens by the
+    # oracle's sparse frontier DP (tests/golden/config_goldens.json)
+    g = _goldens()[f"config5-shape king {L}x{L} p0.8 seed {seed}"]
+    c = int(g["count"])
+    h = bb.Handle(I.kings_subgraph(L, L, 0.8, seed), flags=bb.BBTN_COUNT_CRT)
+    out = h.solve_local(t)
+    assert out["energy"] == int(g["energy"]) and out["count"] == c & MASK64, out
+    assert out["count_mod"] == (c % bb.BBTN_P1, c % bb.BBTN_P2)
+    assert bb.crt_combine(out["count"], *out["count_mod"]) == c
+    h.close()
+
+
+def test_config5_kings_40x40_exact_size_and_count(bb):
+    # BASELINE configs[4]: MIS on the King's subgraph 40x40, filling 0.8, unit weights: exact size and count (1.1e32,
+    # so all three residues are needed) by local branching, with K5 region bounds on every branch
+    g = _goldens()["config5 king 40x40 p0.8 seed 1"]
+    c = int(g["count"])
+    k = I.kings_subgraph(40, 40, 0.8, 1)
+    offs, verts = _grid_regions(40, 40, 4, 4, _king_ids(k, 40, 40))
+    h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT)
+    out = h.solve_local(32, region_offsets=offs, region_vertices=verts, incumbent_hint=int(g["energy"]))
+    assert out["energy"] == int(g["energy"]) and out["count"] == c & MASK64, out
+    assert bb.crt_combine(out["count"], *out["count_mod"]) == c
+    h.close()
+
+
 @pytest.mark.parametrize("L", [16, 20, 24])
 def test_paper_e1_spin_glass_with_half_field(bb, L):
     # +-J with external field 0.5, in integers (J -> 2J, h -> 1, half units; reading A6): one unbranched
