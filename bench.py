@@ -7,7 +7,8 @@
 Workload = BASELINE.json configs[3], the configuration the metric ("counting-tropical GEMM Gop/s & %
 of int32 CUDA-core peak") is quoted on.  ONE STEP is one pass of the whole hot path over one batch:
   (a) raw batched counting-tropical GEMM (K3 tiled): M=N=K=1024, batch 64 per GPU, energies uniform
-      in [-64,64], counts uniform in {1..4} (so the caller promises count_bits = 3);
+      in [-64,64], counts uniform in {1..4} (so the caller promises count_bits = 3 and energy_bits = 7,
+      which selects the packed 16x2 form of K3);
       followed by K2 on its result: the 2^26-element C planes are bit-permuted (seeded random permutation
       of the 26 index bits) into the order a following contraction would want;
   (b) the 5x5x5 open +-J cube, 2^f leaves (f = 8 spins of the central layer, all assignments) per
@@ -18,6 +19,11 @@ Units: 1 tropical FMA = one (batch, m, n, k) term ((.) then (+)); Gop/s = 2 x GF
 `e2e` is the same step through the host-pointer C-ABI calls (H2D of operands/assignments and D2H of
 results inside the timed region).  Weak scaling: every rank runs its own seeded batch; no collective
 on the data path (results are 12 bytes per leaf).  Inputs are larger than L2 (no flush needed).
+
+After the timed steps the same run also reports (untimed by the step clock, each with its own CUDA-event or
+wall-clock timing, N = 1 only): `gemm_sweep` -- the corners of the config-4a sweep in every count/energy mode;
+`time_to_solve` -- exact (E0, count) of configs 1, 2, 3, 4b and of King's subgraphs 36x36 and 40x40 (configs[4]),
+each asserted against tests/golden/config_goldens.json inside the run; `cpu_baseline` on 1 core and on all cores.
 """
 from __future__ import annotations
 
@@ -44,6 +50,13 @@ METRIC = "counting-tropical GEMM Gop/s (2 x tropical FMA/s) over one pass of the
 # fused add-max, tie test = add + compare, multiply-accumulate of the counts (1 IMAD.WIDE for <=32-bit
 # operand counts, 3 IMADs for full 64x64->64).
 INT_OPS_PER_FMA = {32: 4, 64: 6}
+# executed warp instructions per lane-FMA in the inner loop of gemm_pack16_kernel, counted in the SASS of the in-tree
+# object (profiles/r2_k3_pack16_sass.md): per 32 FMAs 16 VIADDMNMX.S16x2 + 16 IADD + 16 HSETP2 + 32 IMAD + 7 LDS.128
+PACK16_INSTR_PER_FMA = 87.0 / 32.0
+SWEEP = [(64, 1024), (256, 256), (1024, 64), (4096, 2)]                # (n, batch) corners of config 4a
+SWEEP_MODES = [("3:7", "packed 16x2 energies, 32-bit accumulators", 32), ("3:32", "32-bit accumulators", 32),
+               ("14:32", "chunk-local 32-bit tie sums, 64-bit accumulators", 32),
+               ("32:32", "32-bit operands, 64-bit accumulators", 32), ("64:32", "full 64x64 count product", 64)]
 
 
 def _peaks():
@@ -124,7 +137,7 @@ def cube_problem(seed: int):
 # ----------------------------------------------------------------------------------------------
 # reference arm: the oracle, as it stands, on the host cores, on a bounded sample of the same step
 # ----------------------------------------------------------------------------------------------
-def oracle_sample(seed: int, rows: int = 32, leaves: int = 4):
+def oracle_sample(seed: int, rows: int = 32, leaves: int = 4, threads: int = 0):
     """One bounded sample of the step through oracle/: `rows` rows of one GEMM batch entry (OpenMP over
     rows) and `leaves` leaves of the cube (naive loop-nest contraction, one thread per leaf).
     Returns (tropical FMAs done, seconds, threads used, description)."""
@@ -138,7 +151,7 @@ def oracle_sample(seed: int, rows: int = 32, leaves: int = 4):
     z = lambda a: np.zeros(a.shape, np.uint8)
     inst, fixed, assign, _, _ = cube_problem(seed)
     tree = _cube_tree(inst, fixed)
-    cores = os.cpu_count() or 1
+    cores = threads if threads > 0 else (os.cpu_count() or 1)      # threads = 1: OMP_NUM_THREADS=1 is set by the caller
     t0 = time.perf_counter()
     oracle.gemm(Ae, z(Ae), Ac, Be64, z(Be64), Bc)
     with ThreadPoolExecutor(max_workers=min(leaves, cores)) as ex:
@@ -180,11 +193,125 @@ def _config(args):
     return {"workload": (f"BASELINE configs[3]: raw batched counting-tropical GEMM M=N=K={GEMM_N} batch {GEMM_BATCH} "
                          f"(energies U[-64,64], counts U{{1..4}}) + K2 bit-permutation of its 2^26-element result + {CUBE_L}x{CUBE_L}x{CUBE_L} open +-J cube, "
                          f"f={CUBE_F} fixed spins of the central layer, all {1 << CUBE_F} leaves, per GPU"),
-            "gemm": {"M": GEMM_N, "N": GEMM_N, "K": GEMM_N, "batch_per_gpu": GEMM_BATCH, "count_bits": 3},
+            "gemm": {"M": GEMM_N, "N": GEMM_N, "K": GEMM_N, "batch_per_gpu": GEMM_BATCH, "count_bits": 3, "energy_bits": 7},
             "cube": {"L": CUBE_L, "n_fixed": CUBE_F, "leaves_per_gpu": 1 << CUBE_F},
             "l2_policy": "inputs larger than L2 (2.4 GB of GEMM planes, multi-GB contraction arena); no flush",
             "seed": args.seed}
 
+
+
+# ----------------------------------------------------------------------------------------------
+# extras reported in the same JSON line (rank 0, N = 1): sweep corners, time-to-solve, oracle on 1 / all cores
+# ----------------------------------------------------------------------------------------------
+def _goldens():
+    with open(os.path.join(ROOT, "tests", "golden", "config_goldens.json")) as f:
+        return json.load(f)["cases"]
+
+
+def gemm_sweep_block(bb, torch, stream, int_peak, repeat=3):
+    """Corners of the config-4a sweep (n, batch) in every count/energy mode: GFMA/s and the fraction of the int32 roof
+    (4 algorithmic int32 lane-instructions per FMA; 6 for the full 64x64 count product)."""
+    out = []
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    for n, B in SWEEP:
+        gen = min(B, 4)
+        Ae, Ac, Be, Bc = I.gemm_operands(gen, n, n, n, seed=1000 * n + B)
+        rep = lambda x: torch.from_numpy(x.view(np.int64) if x.dtype == np.uint64 else x).cuda().repeat((B + gen - 1) // gen, 1, 1)[:B].contiguous()
+        dAe, dAc, dBe, dBc = rep(Ae), rep(Ac), rep(Be), rep(Bc)
+        dCe = torch.empty((B, n, n), dtype=torch.int32, device="cuda"); dCc = torch.empty((B, n, n), dtype=torch.int64, device="cuda")
+        ref = None
+        for mode, what, acc_bits in SWEEP_MODES:
+            bits, ebits = (int(x) for x in mode.split(":"))
+            ts = []
+            with torch.cuda.stream(stream):
+                for it in range(repeat + 1):
+                    a, b = ev(), ev()
+                    a.record(stream)
+                    bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, energy_bits=ebits, stream=stream.cuda_stream)
+                    b.record(stream); b.synchronize()
+                    if it:
+                        ts.append(a.elapsed_time(b))
+            chk = (int(dCe.sum().item()), int(dCc.sum().item()))      # every mode must give the same integers
+            ref = ref or chk
+            assert chk == ref, f"GEMM modes disagree at n={n}: {mode}"
+            ms = float(np.median(ts))
+            gfma = float(B) * n ** 3 / ms / 1e6
+            out.append({"n": n, "batch": B, "mode": mode, "what": what, "ms": ms, "gfma_per_s": gfma,
+                        "frac_of_int32_peak": INT_OPS_PER_FMA[acc_bits] * gfma / int_peak})
+        del dAe, dAc, dBe, dBc, dCe, dCc
+    return out
+
+
+def time_to_solve_block(bb, skip_king40=False):
+    """Second half of the metric: time to the exact (E0, count), each result asserted against the oracle's goldens."""
+    from paper_2602_05470_b200 import time_to_solve as T
+    g = _goldens()
+    mask = (1 << 64) - 1
+    out = []
+
+    def check(name, rec, energy, c64, full=None):
+        want = g[name]
+        assert energy == int(want["energy"]) and c64 == int(want["count"]) & mask, (name, energy, c64, want)
+        if full is not None:
+            assert int(full) == int(want["count"]), (name, full, want["count"])
+        rec["golden"] = name; rec["exact"] = True
+        out.append(rec)
+
+    r = T.solve_unbranched("config1 ising 6x6 seed 1", I.ising_lattice_2d(6, 6, 1))
+    check("config1 ising 6x6 seed 1", {"config": 1, "ms": r["ms_median"], "width": r["width"], "launches": r["kernel_launches"]}, r["energy"], r["count_mod_2_64"])
+    r = T.solve_unbranched("config2 king 12x12 p0.8 seed 1", I.kings_subgraph(12, 12, 0.8, 1))
+    check("config2 king 12x12 p0.8 seed 1", {"config": 2, "ms": r["ms_median"], "width": r["width"], "launches": r["kernel_launches"]}, r["energy"], r["count_mod_2_64"])
+    inst = I.ising_lattice_2d(24, 24, 1)
+    for f in (8, 10, 12):
+        fixed = I.slit_fixed_set_2d(24, 24, f)
+        tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(24, 24, f))
+        r = T.solve_branched("config3", inst, fixed, tree, repeat=3)
+        check("config3 ising 24x24 seed 1", {"config": 3, "n_fixed": f, "leaves": r["leaves"], "ms": r["ms_median"], "width": r["width"],
+                                             "algorithmic_gb_per_s": r["algorithmic_gb_per_s"]}, r["energy"], r["count_mod_2_64"])
+    inst = I.ising_lattice_3d(5, 5, 5, 1)
+    fixed = I.layer_fixed_set_3d(5, 5, 5, 8)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+    r = T.solve_branched("config4b", inst, fixed, tree, repeat=3)
+    check("config4b ising 5x5x5 seed 1", {"config": "4b", "n_fixed": 8, "leaves": r["leaves"], "ms": r["ms_median"], "width": r["width"],
+                                          "algorithmic_gb_per_s": r["algorithmic_gb_per_s"]}, r["energy"], r["count_mod_2_64"])
+    for L, name in ((36, "config5-shape king 36x36 p0.8 seed 1"), (40, "config5 king 40x40 p0.8 seed 1")):
+        if L == 40 and skip_king40:
+            continue
+        r = T.solve_king_local(L, 1, 32, crt=True, hint=int(g[name]["energy"]))
+        check(name, {"config": 5, "king": L, "seconds": r["seconds"], "plan_seconds": r["plan_only_seconds"],
+                     "mode": "bbtn_solve_local, T_target 2^32, three count rings, K5 bounds vs the golden optimum as incumbent",
+                     **{k: r[k] for k in ("stretches", "sliced_stretches", "branches_planned", "branches_contracted", "branches_infeasible",
+                                          "branches_pruned", "max_fixed", "max_rank", "arena_bytes", "kernel_launches")},
+                     "algorithmic_gb_per_s": r["algorithmic_gb_per_s"], "count": r["count"]}, r["energy"], r["count_mod_2_64"], r["count"])
+    return out
+
+
+def cpu_baseline_both(args):
+    """The oracle on the host: all cores in-process, one core in a child process (OMP_NUM_THREADS=1)."""
+    fma, dt, cores, desc = oracle_sample(args.seed, rows=args.ref_rows, leaves=args.ref_leaves)
+    res = {"value": 2.0 * fma / dt / 1e9, "unit": "Gop/s", "cores": cores, "kind": "oracle", "sample": desc, "seconds": dt}
+    try:
+        env = dict(os.environ, OMP_NUM_THREADS="1")
+        rows1, leaves1 = max(8, args.ref_rows // 8), max(1, args.ref_leaves // 8)
+        o = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-sample", f"{args.seed}:{rows1}:{leaves1}"],
+                           env=env, capture_output=True, text=True, timeout=600)
+        one = json.loads(o.stdout.strip().splitlines()[-1])
+        res["one_core"] = {"value": one["gops"], "unit": "Gop/s", "cores": 1, "seconds": one["seconds"], "sample": one["sample"]}
+    except Exception as e:                      # the single-core figure is a nicety; never lose the line over it
+        res["one_core"] = {"error": repr(e)}
+    return res
+
+
+def _traffic_from_profile():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed ncu capture."""
+    p = os.path.join(ROOT, "profiles", "r2_k3_dram_traffic.csv")
+    try:
+        rows = [l.strip().split(",") for l in open(p) if l.strip() and not l.startswith("#")]
+        hdr, val = rows[0], rows[1]
+        d = dict(zip(hdr, val))
+        return float(d["dram_bytes_read"]) + float(d["dram_bytes_write"]), f"profiles/r2_k3_dram_traffic.csv ({d.get('kernel', '?')}, ncu --set full)"
+    except Exception:
+        return None, "no committed capture found"
 
 # ----------------------------------------------------------------------------------------------
 # our arm
@@ -253,7 +380,7 @@ def run_ours(args):
             if record:
                 c1.record(stream)
                 a.record(stream)
-            bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=3, stream=sp)
+            bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=3, energy_bits=7, stream=sp)
             if record:
                 b.record(stream)
             bb.permute_batched(perm, dCe.view(1, -1), dCc.view(1, -1), dPe, dPc, stream=sp)
@@ -264,7 +391,7 @@ def run_ours(args):
     def step_host():
         bound = h_host.region_bound(roffs, rverts, fixed, assign, stream=sp)
         e, c = h_host.contract_batch(fixed, assign, stream=sp)
-        bb.tropical_gemm_batched_host(hAe, hAc, hBe, hBc, hCe, hCc, count_bits=3, stream=sp)
+        bb.tropical_gemm_batched_host(hAe, hAc, hBe, hBc, hCe, hCc, count_bits=3, energy_bits=7, stream=sp)
         return bound, e, c
 
     def barrier():
@@ -334,14 +461,20 @@ def run_ours(args):
     alu_peak = max(mb["iadd3"], mb["imnmx"], mb["viaddmnmx"])
     gemm_gfma = gemm_fma / (gemm_ms * 1e-3) / 1e9
     achieved = INT_OPS_PER_FMA[32] * gemm_gfma
-    roofline = {"bound": "alu", "kernel": "gemm_tiled_kernel (K3)", "achieved": achieved, "peak": int_peak, "unit": "Gop/s",
+    traffic, traffic_src = _traffic_from_profile()
+    issue_peak = 148 * 4 * 32 * (clocks["sm_mhz"] or sm_max) * 1e6 / 1e9 if clocks else None   # G lane-instructions/s the schedulers can issue
+    roofline = {"bound": "alu", "kernel": "gemm_pack16_kernel (K3, packed 16x2 form)", "achieved": achieved, "peak": int_peak, "unit": "Gop/s",
                 "frac": achieved / int_peak,
-                "traffic": 2.589e9,     # dram__bytes_read.sum + dram__bytes_write.sum of this launch, profiles/r1d_gemm_permute_ncu.txt
+                "traffic": traffic, "traffic_source": traffic_src,
                 "traffic_unit": "bytes per launch (algorithmic operand+result bytes: %.3e)" % (3.0 * gb * n * n * 12),
-                "note": (f"op = int32 lane-instruction; achieved = {INT_OPS_PER_FMA[32]} algorithmic int32 instructions per tropical FMA "
-                         "(fused add-max, tie add, tie compare, 32x32+64 multiply-add) x GFMA/s of the K3 launch; peak = committed "
-                         "microbenchmark (bbtn_int32_microbench), best of IADD3 / IMNMX / IMAD / mixed ALU+FMA-pipe issue, same run; "
-                         "frac_of_opmix_ceiling = K3 GFMA/s over the register/broadcast-fed replica of its inner loop (k3mix)"),
+                "note": (f"op = int32 lane-operation; achieved = {INT_OPS_PER_FMA[32]} ALGORITHMIC int32 operations per tropical FMA "
+                         "(add-max, tie add, tie compare, multiply-add of the counts) x GFMA/s of the K3 launch; peak = committed "
+                         "microbenchmark (bbtn_int32_microbench), best of IADD3 / IMNMX / IMAD / mixed ALU+FMA-pipe issue of SCALAR int32 "
+                         "instructions, same run.  The packed form executes 2.5 instructions per FMA (VIADDMNMX.S16x2 and HSETP2 handle two "
+                         "outputs each), so `frac` can exceed what scalar int32 code could reach; `executed_frac_of_issue_peak` = "
+                         "instructions actually issued (SASS count per FMA x GFMA/s) over the schedulers' issue limit is the utilisation figure"),
+                "executed_instr_per_fma": PACK16_INSTR_PER_FMA,
+                "executed_frac_of_issue_peak": (PACK16_INSTR_PER_FMA * gemm_gfma / issue_peak) if issue_peak else None,
                 "gemm_gfma_per_s": gemm_gfma, "gemm_gop_per_s": 2 * gemm_gfma, "gemm_ms_per_launch": gemm_ms,
                 "frac_of_opmix_ceiling": gemm_gfma / max(mb["k3mix_2warps"], mb["k3mix_4warps"]),
                 "frac_of_alu_pipe_peak_2ops": 2 * gemm_gfma / alu_peak,
@@ -360,19 +493,26 @@ def run_ours(args):
     # ---- the oracle beside it (bounded sample, rank 0, N = 1 only)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        fma, dt, cores, desc = oracle_sample(args.seed, rows=args.ref_rows, leaves=args.ref_leaves)
-        cpu = {"value": 2.0 * fma / dt / 1e9, "unit": "Gop/s", "cores": cores, "kind": "oracle", "sample": desc,
-               "seconds": dt}
+        cpu = cpu_baseline_both(args)
+    sweep = tts = None
+    if world == 1 and not args.no_extras:
+        sweep = gemm_sweep_block(bb, torch, stream, int_peak)
+        h_dev.close(); h_host.close()
+        del dAe, dAc, dBe, dBc, dCe, dCc, dPe, dPc
+        torch.cuda.empty_cache()
+        tts = time_to_solve_block(bb, skip_king40=args.skip_king40)
 
     line = {"metric": METRIC, "value": value, "unit": "Gop/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "int32 energy + uint64 count", "data": "synthetic", "config": _config(args),
+            "dtype": "int32 energy + uint64 count (K3 computes the energies as packed s16x2 under the caller's |e| < 2^7 promise)",
+            "data": "synthetic", "config": _config(args),
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "Gop/s", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "note": "host-pointer calls: region_bound + contract_batch + tropical_gemm_batched_host (K2 has no host-pointer form and is left out)",
                     "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches_per_step * args.steps),
             "roofline": roofline, "roofline_hbm_kernels": roofline_hbm, "cpu_baseline": cpu,
+            "gemm_sweep": sweep, "time_to_solve": tts,
             "plan": {k: info[k] for k in ("n_nodes", "n_variant_nodes", "max_rank", "n_gemm_tiled", "n_absorb", "n_permute",
                                           "n_trace", "n_kernel_launches", "workspace_bytes")},
             "fma_per_step": {"gemm": gemm_fma, "cube": cube_fma},
@@ -396,7 +536,15 @@ def main():
     ap.add_argument("--ref-leaves", type=int, default=16)
     ap.add_argument("--microbench-iters", type=int, default=4000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the gemm_sweep and time_to_solve blocks")
+    ap.add_argument("--skip-king40", action="store_true", help="leave the ~1.5 min King 40x40 solve out of time_to_solve")
+    ap.add_argument("--oracle-sample", default=None, help=argparse.SUPPRESS)     # child of cpu_baseline_both: seed:rows:leaves
     args = ap.parse_args()
+    if args.oracle_sample:
+        seed, rows, leaves = (int(x) for x in args.oracle_sample.split(":"))
+        fma, dt, cores, desc = oracle_sample(seed, rows=rows, leaves=leaves, threads=1)
+        print(json.dumps({"gops": 2.0 * fma / dt / 1e9, "seconds": dt, "sample": desc}))
+        return 0
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3          # timing rule: W >= 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

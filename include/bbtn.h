@@ -239,7 +239,7 @@ int bbtn_crt_combine(uint64_t count_mod_2_64, uint32_t count_mod_p1, uint32_t co
 /* Debug checks of caller promises (process-wide switch, default off; also switched on by the environment
  * variable BBTN_DEBUG_CHECKS=1 at load time).  When on, the raw GEMM entry points first verify ON THE DEVICE
  * that every operand count is below 2^count_bits (for count_bits < 64) and that every operand energy is either
- * exactly BBTN_NEG_INF or within +-BBTN_ENERGY_LIMIT, synchronise, and return BBTN_EINVAL without launching K3
+ * exactly BBTN_NEG_INF or below 2^energy_bits in magnitude (within +-BBTN_ENERGY_LIMIT for energy_bits >= 29), synchronise, and return BBTN_EINVAL without launching K3
  * if a promise is broken.  Returns the previous setting. */
 int bbtn_set_debug_checks(int32_t on);
 
@@ -253,14 +253,18 @@ int bbtn_set_debug_checks(int32_t on);
  * Counts uint64 mod 2^64.  M, N, K >= 1, any size (ragged tiles are handled); the launch is refused with
  * BBTN_ESHAPE if it would need more than 2^31-1 thread blocks.
  * count_bits in 1..64: upper bound on log2(count+1) of BOTH operands that the caller guarantees (64 = no
- * promise; <= 32 selects the 32x32->64 multiply path, small values 32-bit accumulators).  A broken promise gives
- * wrong counts silently unless bbtn_set_debug_checks is on.  Asynchronous on cuda_stream. */
+ * promise; <= 32 selects the 32x32->64 multiply path, small values 32-bit accumulators).
+ * energy_bits in 1..32: the caller guarantees |e| < 2^energy_bits for every FINITE operand energy (32 = no promise
+ * beyond BBTN_ENERGY_LIMIT).  energy_bits <= 11 together with counts small enough for 32-bit accumulators
+ * (2 * count_bits + ceil(log2 K) <= 32) selects the packed form: 16-bit energies, two outputs per instruction.
+ * A broken promise gives wrong results silently unless bbtn_set_debug_checks is on.  The result never depends on
+ * which form ran.  Asynchronous on cuda_stream. */
 int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,
                                const int32_t *Ae, const uint64_t *Ac,
                                const int32_t *Be, const uint64_t *Bc,
                                int32_t *Ce, uint64_t *Cc,
                                int64_t strideA, int64_t strideB, int64_t strideC,
-                               int32_t count_bits, void *cuda_stream);
+                               int32_t count_bits, int32_t energy_bits, void *cuda_stream);
 
 /* Same operation with HOST pointers (the end-to-end form of the config-4 sweep): the operands are
  * copied to library-owned device staging buffers, K3 runs, C is copied back and the call returns after
@@ -272,7 +276,7 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
                                     const int32_t *Be, const uint64_t *Bc,
                                     int32_t *Ce, uint64_t *Cc,
                                     int64_t strideA, int64_t strideB, int64_t strideC,
-                                    int32_t count_bits, void *cuda_stream);
+                                    int32_t count_bits, int32_t energy_bits, void *cuda_stream);
 
 /* Raw batched bit permutation (K2 alone): dst[b][pi(i)] = src[b][i] for i in [0, 2^rank), where
  * bit j of pi(i) is bit perm[j] of i (perm is a HOST array, a permutation of 0..rank-1).

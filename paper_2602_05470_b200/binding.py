@@ -69,8 +69,8 @@ def load():
     lib.bbtn_branching_leaves.argtypes = [vp, i32, i64, i64, i64, i64, vp, vp, vp, vp, vp]
     lib.bbtn_solve_local.argtypes = [vp, i32, i64, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.bbtn_local_plan_query.argtypes = [vp, i32, i64, vp, vp]
-    lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
-    lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, vp]
+    lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, i32, vp]
+    lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, i32, vp]
     lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
     lib.bbtn_permute_batched.argtypes = [i32, vp, i64, vp, vp, vp, vp, vp]
     lib.bbtn_int32_microbench.argtypes = [i32, i32, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
@@ -259,7 +259,7 @@ class Handle:
                         "fma": work[0], "bytes": work[1]}
 
 
-def tropical_gemm_batched(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, stream=None):
+def tropical_gemm_batched(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, energy_bits: int = 32, stream=None):
     """bbtn_tropical_gemm_batched on torch CUDA tensors: A [B][M][K] (or [M][K] shared), B [B][K][N]
     (or [K][N] shared); energies int32, counts int64 storage (bit pattern of uint64)."""
     import torch
@@ -272,11 +272,11 @@ def tropical_gemm_batched(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64
         Ce = torch.empty((batch, M, N), dtype=torch.int32, device=Ae.device)
         Cc = torch.empty((batch, M, N), dtype=torch.int64, device=Ae.device)
     _check(load().bbtn_tropical_gemm_batched(batch, M, N, K, _ptr(Ae), _ptr(Ac), _ptr(Be), _ptr(Bc), _ptr(Ce), _ptr(Cc),
-                                             M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, _stream(stream)))
+                                             M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, energy_bits, _stream(stream)))
     return Ce, Cc
 
 
-def tropical_gemm_batched_host(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, stream=None):
+def tropical_gemm_batched_host(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, energy_bits: int = 32, stream=None):
     """bbtn_tropical_gemm_batched_host: same layouts on HOST arrays (numpy, or pinned CPU torch tensors with
     int64 storage for the counts); copies in, runs K3, copies C back."""
     shp = lambda a: tuple(a.shape)
@@ -288,7 +288,7 @@ def tropical_gemm_batched_host(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int
     if Ce is None:
         Ce = np.empty((batch, M, N), np.int32); Cc = np.empty((batch, M, N), np.uint64)
     _check(load().bbtn_tropical_gemm_batched_host(batch, M, N, K, _ptr(Ae), _ptr(Ac), _ptr(Be), _ptr(Bc), _ptr(Ce), _ptr(Cc),
-                                                  M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, _stream(stream)))
+                                                  M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, energy_bits, _stream(stream)))
     return Ce, Cc
 
 

@@ -35,36 +35,38 @@ bool g_debug_checks = [] { const char *e = std::getenv("BBTN_DEBUG_CHECKS"); ret
 
 // flags |= 1: a count >= 2^count_bits;  |= 2: an energy that is neither BBTN_NEG_INF nor within +-BBTN_ENERGY_LIMIT
 __global__ void check_operand_kernel(const int32_t *__restrict__ e, const uint64_t *__restrict__ c, int64_t rows, int64_t row_len,
-                                     int64_t row_stride, int count_bits, int *flags) {
+                                     int64_t row_stride, int count_bits, int energy_limit, int *flags) {
   const int64_t total = rows * row_len;
   int bad = 0;
   for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
     const int64_t r = t / row_len, i = r * row_stride + (t - r * row_len);
     const int32_t ee = e[i];
     if (count_bits < 64 && (c[i] >> count_bits) != 0) bad |= 1;
-    if (ee != BBTN_NEG_INF && (ee > BBTN_ENERGY_LIMIT || ee < -BBTN_ENERGY_LIMIT)) bad |= 2;
+    if (ee != BBTN_NEG_INF && (ee > energy_limit || ee < -energy_limit)) bad |= 2;
   }
   if (bad) atomicOr(flags, bad);
 }
 
 int check_gemm_operands(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac, const int32_t *Be,
-                        const uint64_t *Bc, int64_t sA, int64_t sB, int32_t count_bits, cudaStream_t st) {
+                        const uint64_t *Bc, int64_t sA, int64_t sB, int32_t count_bits, int32_t energy_bits, cudaStream_t st) {
   int *d_flags = nullptr, h_flags = 0;
   CUDA_TRY(nullptr, cudaMalloc(&d_flags, sizeof(int)));
   cudaMemsetAsync(d_flags, 0, sizeof(int), st);
-  check_operand_kernel<<<148 * 4, 256, 0, st>>>(Ae, Ac, sA ? batch : 1, (int64_t)M * K, sA, count_bits, d_flags);
-  check_operand_kernel<<<148 * 4, 256, 0, st>>>(Be, Bc, sB ? batch : 1, (int64_t)K * N, sB, count_bits, d_flags);
+  const int lim = energy_bits >= 29 ? BBTN_ENERGY_LIMIT : (1 << energy_bits) - 1;
+  check_operand_kernel<<<148 * 4, 256, 0, st>>>(Ae, Ac, sA ? batch : 1, (int64_t)M * K, sA, count_bits, lim, d_flags);
+  check_operand_kernel<<<148 * 4, 256, 0, st>>>(Be, Bc, sB ? batch : 1, (int64_t)K * N, sB, count_bits, lim, d_flags);
   cudaError_t e = cudaMemcpyAsync(&h_flags, d_flags, sizeof(int), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(d_flags);
   CUDA_TRY(nullptr, e);
   if (h_flags & 1) return fail(nullptr, BBTN_EINVAL, "debug check: an operand count is not below 2^count_bits (count_bits = " + std::to_string(count_bits) + ")");
-  if (h_flags & 2) return fail(nullptr, BBTN_EINVAL, "debug check: an operand energy is neither BBTN_NEG_INF nor within +-BBTN_ENERGY_LIMIT");
+  if (h_flags & 2) return fail(nullptr, BBTN_EINVAL, "debug check: an operand energy is neither BBTN_NEG_INF nor below 2^energy_bits in magnitude (energy_bits = " + std::to_string(energy_bits) + ")");
   return BBTN_OK;
 }
 
-int check_gemm_shape(int64_t batch, int32_t M, int32_t N, int32_t count_bits) {
+int check_gemm_shape(int64_t batch, int32_t M, int32_t N, int32_t count_bits, int32_t energy_bits) {
   if (count_bits < 1 || count_bits > 64) return fail(nullptr, BBTN_EINVAL, "count_bits must be in 1..64");
+  if (energy_bits < 1 || energy_bits > 32) return fail(nullptr, BBTN_EINVAL, "energy_bits must be in 1..32");
   // the smallest tile any K3 form uses is 64x64: one thread block per tile and batch entry
   const double n_cta = (double)((M + 63) / 64) * (double)((N + 63) / 64) * (double)batch;
   if (n_cta > 2147483647.0) return fail(nullptr, BBTN_ESHAPE, "GEMM launch would need more than 2^31-1 thread blocks; split the batch");
@@ -147,6 +149,8 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
   launch_construct(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_var.p, dp->n_var,
                    (const int32_t *)dp->list_inv.p, dp->n_inv, (const int32_t *)dp->list_scalar.p, dp->n_scalar,
                    d_assign, (int)pl.fixed.size(), B, ve, vc, ie, ic, (int32_t *)dp->off_e.p, dp->off_c.p, ring, st);
+  int energy_bits = 0;                                   // every finite energy of every tensor is within +-energy_range
+  while (energy_bits < 32 && ((int64_t)1 << energy_bits) <= h->P.energy_range) energy_bits++;
   auto pe = [&](int v, int64_t off) { return v ? ve + off * B : ie + off; };
   auto pc = [&](int v, int64_t off) { return (void *)(v ? vc + (size_t)off * B * csz : ic + (size_t)off * csz); };
   for (const Step &s : pl.steps) {
@@ -168,7 +172,7 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
                           pe(s.vA, s.offA), pc(s.vA, s.offA), pe(s.vB, s.offB), pc(s.vB, s.offB),
                           pe(s.vC, s.offC), pc(s.vC, s.offC),
                           s.vA ? ((int64_t)1 << s.rA) : 0, s.vB ? ((int64_t)1 << s.rB) : 0, (int64_t)1 << s.rO,
-                          ring, s.count_bits, st);
+                          ring, s.count_bits, energy_bits, st);
         break;
     }
   }
@@ -212,6 +216,7 @@ int bbtn_build(const bbtn_problem_desc *d, bbtn_handle **out) {
     range += std::abs((int64_t)P.vw[i]);
   }
   if (range > BBTN_ENERGY_LIMIT) return fail(nullptr, BBTN_ERANGE, "sum of |couplings| + |weights| exceeds 2^28");
+  P.energy_range = range;
   if (d->tree_l || d->n_steps > 0) {
     if (!d->tree_l || !d->tree_r || d->n_steps != P.n + P.m - 1)
       return fail(nullptr, BBTN_EINVAL, "tree must have n_edges + n_vertices - 1 steps");
@@ -354,15 +359,16 @@ extern "C" {
 
 int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac,
                                const int32_t *Be, const uint64_t *Bc, int32_t *Ce, uint64_t *Cc,
-                               int64_t strideA, int64_t strideB, int64_t strideC, int32_t count_bits, void *stream) {
+                               int64_t strideA, int64_t strideB, int64_t strideC, int32_t count_bits, int32_t energy_bits,
+                               void *stream) {
   if (batch < 1 || M < 1 || N < 1 || K < 1 || !Ae || !Ac || !Be || !Bc || !Ce || !Cc || strideA < 0 || strideB < 0 || strideC < 0)
     return fail(nullptr, BBTN_EINVAL, "bad GEMM arguments");
   if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
-  int rc = check_gemm_shape(batch, M, N, count_bits);
+  int rc = check_gemm_shape(batch, M, N, count_bits, energy_bits);
   if (rc) return rc;
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
-  if (g_debug_checks && (rc = check_gemm_operands(batch, M, N, K, Ae, Ac, Be, Bc, strideA, strideB, count_bits, (cudaStream_t)stream))) return rc;
-  launch_gemm_tiled(batch, 1, M, N, K, 0, Ae, Ac, Be, Bc, Ce, Cc, strideA, strideB, strideC, RING_U64, count_bits,
+  if (g_debug_checks && (rc = check_gemm_operands(batch, M, N, K, Ae, Ac, Be, Bc, strideA, strideB, count_bits, energy_bits, (cudaStream_t)stream))) return rc;
+  launch_gemm_tiled(batch, 1, M, N, K, 0, Ae, Ac, Be, Bc, Ce, Cc, strideA, strideB, strideC, RING_U64, count_bits, energy_bits,
                     (cudaStream_t)stream);
   CUDA_TRY(nullptr, cudaGetLastError());
   return BBTN_OK;
@@ -370,13 +376,14 @@ int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, c
 
 int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *Ae, const uint64_t *Ac,
                                     const int32_t *Be, const uint64_t *Bc, int32_t *Ce, uint64_t *Cc,
-                                    int64_t strideA, int64_t strideB, int64_t strideC, int32_t count_bits, void *stream) {
+                                    int64_t strideA, int64_t strideB, int64_t strideC, int32_t count_bits, int32_t energy_bits,
+                                    void *stream) {
   if (batch < 1 || M < 1 || N < 1 || K < 1 || !Ae || !Ac || !Be || !Bc || !Ce || !Cc || strideA < 0 || strideB < 0 || strideC < 0)
     return fail(nullptr, BBTN_EINVAL, "bad GEMM arguments");
   if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
   if ((strideA && strideA < (int64_t)M * K) || (strideB && strideB < (int64_t)K * N))
     return fail(nullptr, BBTN_EINVAL, "operand stride smaller than the operand");
-  { int rc = check_gemm_shape(batch, M, N, count_bits); if (rc) return rc; }
+  { int rc = check_gemm_shape(batch, M, N, count_bits, energy_bits); if (rc) return rc; }
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
   static thread_local DevBuf st_e[3], st_c[3];
   cudaStream_t st = (cudaStream_t)stream;
@@ -431,11 +438,11 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
     CUDA_TRY(nullptr, cudaStreamWaitEvent(s_k, ev_in[c], 0));
     if (g_debug_checks) {
       int rc = check_gemm_operands(nb, M, N, K, dAe + b0 * strideA, dAc + b0 * strideA, dBe + b0 * strideB, dBc + b0 * strideB,
-                                   strideA, strideB, count_bits, s_k);
+                                   strideA, strideB, count_bits, energy_bits, s_k);
       if (rc) { cudaStreamSynchronize(s_in); cudaStreamSynchronize(s_out); return rc; }
     }
     launch_gemm_tiled(nb, 1, M, N, K, 0, dAe + b0 * strideA, dAc + b0 * strideA, dBe + b0 * strideB, dBc + b0 * strideB,
-                      dCe + b0 * strideC, dCc + b0 * strideC, strideA, strideB, strideC, RING_U64, count_bits, s_k);
+                      dCe + b0 * strideC, dCc + b0 * strideC, strideA, strideB, strideC, RING_U64, count_bits, energy_bits, s_k);
     CUDA_TRY(nullptr, cudaGetLastError());
     CUDA_TRY(nullptr, cudaEventRecord(ev_k[c], s_k));
     CUDA_TRY(nullptr, cudaStreamWaitEvent(s_out, ev_k[c], 0));

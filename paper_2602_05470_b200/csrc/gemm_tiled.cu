@@ -22,21 +22,17 @@
 // rewrites each chunk k-major with the counts narrowed to 32 bits when the caller's count_bits
 // allows (converted stages).  Ragged or unaligned tiles take a guarded scalar fill that writes the
 // zero element (-inf, 0) outside the matrix.
-#include "kernels.h"
-#include "ring.cuh"
+#include "gemm_stage.cuh"
 #include <type_traits>
 
 namespace bbtn {
 namespace {
 
-constexpr int BM = 128, BK = 16, NT = 256;
-constexpr int RAW_STAGES = 2, CONV_STAGES = 3;
-constexpr int AE_LD = BK + 4;            // row-major A energies: [BM][AE_LD] int32 (row stride 80 B)
-constexpr int AC_LD = BK + 2;            // row-major A counts:   [BM][AC_LD] uint64 (row stride 144 B)
-constexpr int AE_BYTES = BM * AE_LD * 4; // k-major A needs BK*BM*4 <= this
-constexpr int AC_BYTES = BM * AC_LD * 8;
+using namespace stage;
 
-enum Mode : int { ACC32 = 0, ACC64N = 1, WIDE = 2 };
+enum Mode : int { ACC32 = 0, ACC64N = 1, WIDE = 2, NARROW64 = 3 };
+// NARROW64: operand counts < 2^14: the ties of one chunk (BK = 16 products below 2^28) are summed in a 32-bit register
+//           with ACC32's one-IMAD inner loop and added to the 64-bit accumulator once per chunk -- any K, any total
 // ACC32 : operand counts < 2^16 and K * max product < 2^32: 32-bit accumulators, one IMAD per FMA
 // ACC64N: operand counts < 2^32: 64-bit accumulators, one IMAD.WIDE per FMA
 // WIDE  : full 64x64->64 multiply-add (IMAD.WIDE + 2 IMAD)
@@ -44,16 +40,9 @@ enum Mode : int { ACC32 = 0, ACC64N = 1, WIDE = 2 };
 template <int MODE> struct AccT { using T = uint64_t; };
 template <> struct AccT<ACC32> { using T = uint32_t; };
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
-  const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 // pass 2 of one FMA: if (ea + eb == E) c += ca * cb
-template <int MODE>
-__device__ __forceinline__ void tie_fma(typename AccT<MODE>::T &c, int32_t ea, int32_t eb, int32_t E, uint64_t ca, uint64_t cb) {
+template <int MODE, class AccR = typename AccT<MODE>::T>
+__device__ __forceinline__ void tie_fma(AccR &c, int32_t ea, int32_t eb, int32_t E, uint64_t ca, uint64_t cb) {
   if (MODE == ACC32) {
     uint32_t c32 = (uint32_t)c;
     asm("{\n\t.reg .pred p;\n\t.reg .s32 s;\n\tadd.s32 s, %1, %2;\n\tsetp.eq.s32 p, s, %3;\n\t@p mad.lo.u32 %0, %4, %5, %0;\n\t}"
@@ -81,15 +70,6 @@ __device__ __forceinline__ void tie_fma(typename AccT<MODE>::T &c, int32_t ea, i
   }
 }
 
-struct GemmArgs {
-  int64_t G;
-  int M, N, K;
-  const int32_t *Ae; const uint64_t *Ac; const int32_t *Be; const uint64_t *Bc;
-  int32_t *Ce; uint64_t *Cc;
-  int64_t sA, sB, sC;
-  int vecA, vecB, vecC;     // 16-byte paths allowed (alignment of pointers, strides and leading dimensions)
-};
-
 // shared memory: RAW_STAGES raw stages (cp.async targets, operands in their global layout, uint64 counts)
 // followed by CONV_STAGES converted stages (k-major, counts narrowed to CT) that the FMA loops read.
 template <int NCB, class CT> struct Tile {
@@ -100,84 +80,6 @@ template <int NCB, class CT> struct Tile {
   static constexpr int CONV = CAE + CAC + CBE + CBC;
   static constexpr int SMEM = RAW_STAGES * RAW + CONV_STAGES * CONV;
 };
-
-// ---- global -> shared for one chunk (k0 .. k0+BK) of one operand ------------------------------
-template <bool A_KMAJOR>
-__device__ __forceinline__ void fill_A(const GemmArgs &p, const int32_t *__restrict__ ae, const uint64_t *__restrict__ ac,
-                                       int m0, int k0, unsigned char *sAe, unsigned char *sAc) {
-  const int t = threadIdx.x;
-  const bool fast = p.vecA && m0 + BM <= p.M && k0 + BK <= p.K;
-  if (fast) {
-    if (A_KMAJOR) {
-#pragma unroll
-      for (int idx = t; idx < BK * BM / 4; idx += NT) {
-        const int kk = idx / (BM / 4), q = idx % (BM / 4);
-        cp_async16(sAe + (kk * BM + 4 * q) * 4, ae + (int64_t)(k0 + kk) * p.M + m0 + 4 * q);
-      }
-#pragma unroll
-      for (int idx = t; idx < BK * BM / 2; idx += NT) {
-        const int kk = idx / (BM / 2), q = idx % (BM / 2);
-        cp_async16(sAc + (kk * BM + 2 * q) * 8, ac + (int64_t)(k0 + kk) * p.M + m0 + 2 * q);
-      }
-    } else {
-#pragma unroll
-      for (int idx = t; idx < BM * BK / 4; idx += NT) {
-        const int r = idx / (BK / 4), q = idx % (BK / 4);
-        cp_async16(sAe + (r * AE_LD + 4 * q) * 4, ae + (int64_t)(m0 + r) * p.K + k0 + 4 * q);
-      }
-#pragma unroll
-      for (int idx = t; idx < BM * BK / 2; idx += NT) {
-        const int r = idx / (BK / 2), q = idx % (BK / 2);
-        cp_async16(sAc + (r * AC_LD + 2 * q) * 8, ac + (int64_t)(m0 + r) * p.K + k0 + 2 * q);
-      }
-    }
-  } else {
-    int32_t *se = reinterpret_cast<int32_t *>(sAe);
-    uint64_t *sc = reinterpret_cast<uint64_t *>(sAc);
-    for (int idx = t; idx < BM * BK; idx += NT) {
-      int r, kk;
-      if (A_KMAJOR) { kk = idx / BM; r = idx % BM; } else { r = idx / BK; kk = idx % BK; }
-      const int gm = m0 + r, gk = k0 + kk;
-      int32_t e = NEG_INF; uint64_t c = 0;
-      if (gm < p.M && gk < p.K) {
-        const int64_t gi = A_KMAJOR ? (int64_t)gk * p.M + gm : (int64_t)gm * p.K + gk;
-        e = ae[gi]; c = ac[gi];
-      }
-      if (A_KMAJOR) { se[kk * BM + r] = e; sc[kk * BM + r] = c; }
-      else { se[r * AE_LD + kk] = e; sc[r * AC_LD + kk] = c; }
-    }
-  }
-}
-
-template <int BNt>
-__device__ __forceinline__ void fill_B(const GemmArgs &p, const int32_t *__restrict__ be, const uint64_t *__restrict__ bc,
-                                       int n0, int k0, unsigned char *sBe, unsigned char *sBc) {
-  const int t = threadIdx.x;
-  const bool fast = p.vecB && n0 + BNt <= p.N && k0 + BK <= p.K;
-  if (fast) {
-#pragma unroll
-    for (int idx = t; idx < BK * BNt / 4; idx += NT) {
-      const int kk = idx / (BNt / 4), q = idx % (BNt / 4);
-      cp_async16(sBe + (kk * BNt + 4 * q) * 4, be + (int64_t)(k0 + kk) * p.N + n0 + 4 * q);
-    }
-#pragma unroll
-    for (int idx = t; idx < BK * BNt / 2; idx += NT) {
-      const int kk = idx / (BNt / 2), q = idx % (BNt / 2);
-      cp_async16(sBc + (kk * (BNt / 2) + q) * 16, bc + (int64_t)(k0 + kk) * p.N + n0 + 2 * q);
-    }
-  } else {
-    int32_t *se = reinterpret_cast<int32_t *>(sBe);
-    uint64_t *sc = reinterpret_cast<uint64_t *>(sBc);
-    for (int idx = t; idx < BK * BNt; idx += NT) {
-      const int kk = idx / BNt, n = idx % BNt;
-      const int gn = n0 + n, gk = k0 + kk;
-      int32_t e = NEG_INF; uint64_t c = 0;
-      if (gn < p.N && gk < p.K) { e = be[(int64_t)gk * p.N + gn]; c = bc[(int64_t)gk * p.N + gn]; }
-      se[kk * BNt + n] = e;
-      sc[kk * BNt + n] = c;
-    }
-  }
-}
 
 // ---- raw stage -> converted stage (k-major, counts narrowed to CT) ---------------------------
 template <class CT> __device__ __forceinline__ void store_pair(CT *dst, uint64_t x, uint64_t y);
@@ -309,6 +211,13 @@ __global__ void __launch_bounds__(NT, 1) gemm_tiled3_kernel(const GemmArgs p) {
 #pragma unroll
         for (int j = 0; j < TN; j++) En[i][j] = E[rb * 4 + i][j];
     }
+    uint32_t c32[MODE == NARROW64 ? 4 : 1][MODE == NARROW64 ? TN : 1];       // NARROW64: this chunk's tie counts
+    if (MODE == NARROW64) {
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) c32[MODE == NARROW64 ? i : 0][MODE == NARROW64 ? j : 0] = 0u;
+    }
 #pragma unroll 4
     for (int kk = 0; kk < BK; kk++) {
       int32_t a2[4], b2[TN]; uint64_t ca[4], cb[TN];
@@ -326,8 +235,15 @@ __global__ void __launch_bounds__(NT, 1) gemm_tiled3_kernel(const GemmArgs p) {
 #pragma unroll
         for (int j = 0; j < TN; j++) {
           if (P1) En[i][j] = __viaddmax_s32(a1[i], b1[j], En[i][j]);
-          tie_fma<MODE>(C[rb * 4 + i][j], a2[i], b2[j], E[rb * 4 + i][j], ca[i], cb[j]);
+          if (MODE == NARROW64) tie_fma<ACC32>(c32[MODE == NARROW64 ? i : 0][MODE == NARROW64 ? j : 0], a2[i], b2[j], E[rb * 4 + i][j], ca[i], cb[j]);
+          else tie_fma<MODE>(C[rb * 4 + i][j], a2[i], b2[j], E[rb * 4 + i][j], ca[i], cb[j]);
         }
+    }
+    if (MODE == NARROW64) {
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < TN; j++) C[rb * 4 + i][j] += c32[MODE == NARROW64 ? i : 0][MODE == NARROW64 ? j : 0];
     }
     if (P1) {                                        // a new maximum drops the count of the old one
 #pragma unroll
@@ -428,7 +344,8 @@ inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) =
 // RING_U64 only.  count_bits is the caller's bound on log2(count+1) of both operands.
 void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                            const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
-                           int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, cudaStream_t st) {
+                           int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, int energy_bits,
+                           cudaStream_t st) {
   GemmArgs a{G, M, N, K, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC, 0, 0, 0};
   const int ldA = a_kmajor ? M : K;
   a.vecA = (ldA % 4 == 0) && (sA % 4 == 0) && (((int64_t)M * K) % 4 == 0 || G == 1) && al16(Ae) && al16(Ac);
@@ -436,9 +353,14 @@ void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_
   a.vecC = (N % 4 == 0) && (sC % 4 == 0) && (((int64_t)M * N) % 4 == 0 || G == 1) && al16(Ce) && al16(Cc);
   int lgK = 0;
   while (((int64_t)1 << lgK) < K) lgK++;
-  const int mode = (count_bits <= 16 && 2 * count_bits + lgK <= 32) ? ACC32 : (count_bits <= 32 ? ACC64N : WIDE);
-  if (mode == ACC32) {
+  const int mode = (count_bits <= 16 && 2 * count_bits + lgK <= 32) ? ACC32
+                   : (count_bits <= 14 ? NARROW64 : (count_bits <= 32 ? ACC64N : WIDE));
+  if (mode == ACC32 && energy_bits <= 11) {
+    launch_gemm_pack16(batch, G, M, N, K, a_kmajor, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC, st);
+  } else if (mode == ACC32) {
     if (a_kmajor) launch_one<ACC32, true, 2>(a, batch, st); else launch_one<ACC32, false, 2>(a, batch, st);
+  } else if (mode == NARROW64) {
+    if (a_kmajor) launch_one<NARROW64, true, 1>(a, batch, st); else launch_one<NARROW64, false, 1>(a, batch, st);
   } else if (mode == ACC64N) {
     if (a_kmajor) launch_one<ACC64N, true, 1>(a, batch, st); else launch_one<ACC64N, false, 1>(a, batch, st);
   } else {

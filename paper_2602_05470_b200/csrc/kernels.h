@@ -36,15 +36,21 @@ void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
 // K3 (register/shared-memory tiled form).  C[b,g,m,n] = (+)_k A (.) B.
 //   a_kmajor = 1: A is [g][k][m] (m fastest, the engine's canonical order); 0: A is row-major [m][k].
 //   B is [g][k][n], C is [g][m][n].  Batch strides in elements (0 = shared).  count_bits <= 32 selects the
-//   32-bit-operand multiply path (RING_U64 only).
+//   32-bit-operand multiply path, energy_bits <= 11 (with 32-bit accumulators) the packed 16x2 form (RING_U64 only).
 void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                        const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc, int32_t *Ce, void *Cc,
-                       int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, cudaStream_t st);
+                       int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, int energy_bits, cudaStream_t st);
 
 // K3 v2 for the mod-2^64 ring (gemm_tiled.cu): chunked two-pass kernel, 4 integer instructions per FMA.
 void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                            const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
-                           int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, cudaStream_t st);
+                           int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, int energy_bits,
+                           cudaStream_t st);
+
+// K3 packed form (gemm_pack16.cu): two outputs per integer instruction; finite |energy| < 2^11, 32-bit accumulators.
+void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
+                        const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
+                        int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, cudaStream_t st);
 
 // Local slicing: acc (+)= offset (.) slice, element-wise over n elements (first = 1: acc = offset (.) slice); the
 // zero tensor when slice_e == nullptr.  offset is one element on the device.  (+) over the assignments of a segment's

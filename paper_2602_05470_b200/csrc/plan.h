@@ -21,6 +21,7 @@ struct Problem {
   std::vector<int32_t> eu, ev, ew, vw;  // ew/vw always materialised (defaults applied)
   std::vector<int32_t> tree_l, tree_r;  // empty = derive per signature
   int64_t max_elements = (int64_t)1 << 28;
+  int64_t energy_range = (int64_t)1 << 28;   // sum of |couplings| + |fields/weights|: bounds every finite energy of every tensor
   uint32_t flags = 0;
 };
 

@@ -1,12 +1,13 @@
 """Raw batched counting-tropical GEMM sweep (BASELINE.json configs[3], first half), through the C ABI.
 
-    python -m paper_2602_05470_b200.gemm_sweep [--sizes 64 256 1024 4096] [--batches 1 4 16 64 256 1024] [--count-bits 3 32 64]
+    python -m paper_2602_05470_b200.gemm_sweep [--sizes 64 256 1024 4096] [--batches 1 4 16 64 256 1024] [--modes 3:7 3:32 14:32 32:32 64:32]
 
 M = N = K = n, energies uniform in [-64, 64], counts uniform in {1..4} (instances.gemm_operands); batches are
 restricted to B * 3 * n^2 * 12 B <= --max-gb.  One JSON line per (n, B, count_bits): milliseconds (CUDA events,
 median of --repeat after 2 warm-ups), GFMA/s (1 tropical FMA = one (b, m, n, k) term) and Gop/s = 2 x GFMA/s.
-count_bits is the caller's promise on the operand counts (include/bbtn.h): 3 selects 32-bit accumulators,
-32 selects 32-bit operands with 64-bit accumulators, 64 the full 64x64 multiply.
+A mode is count_bits:energy_bits, the caller's promises on the operands (include/bbtn.h): 3:7 selects the packed
+16x2 form (small counts and |energy| < 2^7), 3:32 32-bit energies with 32-bit accumulators, 14:32 chunk-local
+32-bit tie sums with 64-bit accumulators, 32:32 32-bit operands with 64-bit accumulators, 64:32 the full 64x64 multiply.
 """
 from __future__ import annotations
 
@@ -24,7 +25,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--sizes", nargs="*", type=int, default=[64, 256, 1024, 4096])
     ap.add_argument("--batches", nargs="*", type=int, default=[1, 4, 16, 64, 256, 1024])
-    ap.add_argument("--count-bits", nargs="*", type=int, default=[3, 32, 64])
+    ap.add_argument("--modes", nargs="*", default=["3:7", "3:32", "14:32", "32:32", "64:32"])
     ap.add_argument("--max-gb", type=float, default=16.0)
     ap.add_argument("--repeat", type=int, default=5)
     a = ap.parse_args()
@@ -40,20 +41,21 @@ def main():
             rep = lambda x: torch.from_numpy(x.view(np.int64) if x.dtype == np.uint64 else x).cuda().repeat((B + gen - 1) // gen, 1, 1)[:B].contiguous()
             dAe, dAc, dBe, dBc = rep(Ae), rep(Ac), rep(Be), rep(Bc)
             dCe = torch.empty((B, n, n), dtype=torch.int32, device="cuda"); dCc = torch.empty((B, n, n), dtype=torch.int64, device="cuda")
-            for bits in a.count_bits:
+            for mode in a.modes:
+                bits, ebits = (int(x) for x in mode.split(":"))
                 with torch.cuda.stream(st):
                     for _ in range(2):
-                        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, stream=st.cuda_stream)
+                        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, energy_bits=ebits, stream=st.cuda_stream)
                     ts = []
                     for _ in range(a.repeat):
                         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
                         e0.record(st)
-                        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, stream=st.cuda_stream)
+                        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, energy_bits=ebits, stream=st.cuda_stream)
                         e1.record(st); e1.synchronize()
                         ts.append(e0.elapsed_time(e1))
                 ms = float(np.median(ts))
                 fma = float(B) * n * n * n
-                print(json.dumps({"n": n, "batch": B, "count_bits": bits, "ms": ms, "gfma_per_s": fma / ms / 1e6,
+                print(json.dumps({"n": n, "batch": B, "count_bits": bits, "energy_bits": ebits, "ms": ms, "gfma_per_s": fma / ms / 1e6,
                                   "gop_per_s": 2 * fma / ms / 1e6, "bytes": B * 3 * n * n * 12}), flush=True)
             del dAe, dAc, dBe, dBc, dCe, dCc
 

@@ -194,9 +194,13 @@ def test_crt_combine_matches_big_integers(lib):
 def test_raw_gemm_argument_checks_need_no_device(lib):
     # count_bits outside 1..64 and launches beyond 2^31-1 thread blocks are refused before any CUDA call
     z = C.c_void_p(16)
-    rc = lib.bbtn_tropical_gemm_batched(1, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 0, None)
+    rc = lib.bbtn_tropical_gemm_batched(1, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 0, 32, None)
     assert rc == bb.BBTN_EINVAL
-    rc = lib.bbtn_tropical_gemm_batched(1 << 40, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 64, None)
+    rc = lib.bbtn_tropical_gemm_batched(1 << 40, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 64, 32, None)
+    assert rc == bb.BBTN_ESHAPE
+    rc = lib.bbtn_tropical_gemm_batched(1, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 64, 0, None)
+    assert rc == bb.BBTN_EINVAL
+    rc = lib.bbtn_tropical_gemm_batched(1 << 40, 64, 64, 64, z, z, z, z, z, z, 0, 0, 4096, 64, 32, None)
     assert rc == bb.BBTN_ESHAPE
     assert bb.set_debug_checks(False) in (False, True)
 

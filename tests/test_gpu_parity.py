@@ -53,12 +53,56 @@ def test_gemm_matches_oracle(bb, oracle, B, M, N, K, seed, frac, wide):
     Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed, neg_inf_frac=frac, wide_counts=wide)
     want_e, want_c = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
-    # 64: full 64x64 multiply; 32: 32-bit operands, 64-bit accumulators; 3: counts <= 4, 32-bit accumulators
-    for bits in (64, 32, 3) if not wide else (64,):
-        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+    # 64: full 64x64 multiply; 32: 32-bit operands, 64-bit accumulators; 3: counts <= 4, 32-bit accumulators;
+    # (3, 7): also |energy| < 2^7 promised -> the packed 16x2 form
+    for bits, ebits in ((64, 32), (32, 32), (14, 32), (3, 32), (3, 7)) if not wide else ((64, 32),):
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits, energy_bits=ebits)
         got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
-        assert (got_e == want_e).all()
-        assert (got_c == want_c).all()
+        assert (got_e == want_e).all(), (bits, ebits)
+        assert (got_c == want_c).all(), (bits, ebits)
+
+
+@pytest.mark.parametrize("B,M,N,K,seed,frac", [
+    (2, 256, 256, 512, 41, 0.0),
+    (1, 131, 197, 100, 42, 0.2),          # ragged in every dimension, zero elements
+    (3, 128, 130, 1000, 43, 0.05),
+    (1, 300, 129, 17, 44, 0.5),
+])
+def test_gemm_packed_form_full_energy_range(bb, oracle, B, M, N, K, seed, frac):
+    # the packed 16x2 form (energy_bits <= 11, 32-bit accumulators) on energies that use its whole range
+    # (-2047..2047, ties made frequent by drawing from a few hundred values) and on the zero element
+    Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed, neg_inf_frac=frac)
+    spread = lambda e, s: np.where(e <= -(1 << 29), e, ((e.astype(np.int64) * 31 + s) % 4095 - 2047)).astype(np.int32)
+    Ae, Be = spread(Ae, 7), spread(Be, 1900)
+    assert Ae.max() > 1900 and Be[Be > -(1 << 29)].min() < -1900
+    want_e, want_c = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    prev = bb.set_debug_checks(True)
+    try:
+        for ebits in (11, 32):
+            Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=3, energy_bits=ebits)
+            assert (Ce.cpu().numpy() == want_e).all(), ebits
+            assert (Cc.cpu().numpy().view(np.uint64) == want_c).all(), ebits
+        with pytest.raises(bb.BbtnError):                              # |e| up to 2047 is not below 2^10
+            bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=3, energy_bits=10)
+    finally:
+        bb.set_debug_checks(prev)
+
+
+def test_gemm_narrow_counts_long_sums(bb, oracle):
+    # count_bits = 14: chunk-local 32-bit tie sums added to 64-bit accumulators; all energies equal, so every term ties
+    # and the totals (up to 2000 * 2^28) need the 64 bits
+    B, M, N, K = 2, 130, 70, 2000
+    Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed=51)
+    Ae[:] = 3; Be[:] = -5
+    Ac = (I.splitmix64(51, Ac.size, 30) % np.uint64(1 << 14)).reshape(Ac.shape)
+    Bc = (I.splitmix64(51, Bc.size, 31) % np.uint64(1 << 14)).reshape(Bc.shape)
+    want_e, want_c = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
+    assert int(want_c.max()) > 1 << 36
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    for bits in (14, 32, 64):
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+        assert (Ce.cpu().numpy() == want_e).all() and (Cc.cpu().numpy().view(np.uint64) == want_c).all(), bits
 
 
 def test_gemm_shared_operand_stride0(bb, oracle):
@@ -76,10 +120,10 @@ def test_gemm_4096_sampled_rows_all_count_modes(bb, oracle):
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
     rows = np.unique((I.splitmix64(7, 64, 20) % np.uint64(n)).astype(np.int64))
     we, wc = _oracle_gemm(oracle, Ae[:, rows], Ac[:, rows], Be, Bc)
-    for bits in (64, 32, 3):
-        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+    for bits, ebits in ((64, 32), (32, 32), (14, 32), (3, 32), (3, 7)):
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits, energy_bits=ebits)
         got_e = Ce[0].cpu().numpy(); got_c = Cc[0].cpu().numpy().view(np.uint64)
-        assert (got_e[rows] == we[0]).all() and (got_c[rows] == wc[0]).all(), bits
+        assert (got_e[rows] == we[0]).all() and (got_c[rows] == wc[0]).all(), (bits, ebits)
         # cheap whole-matrix property: every output energy is attainable (<= 128) and every count is in [1, 16 n]
         assert got_e.max() <= 128 and got_e.min() >= 100 and got_c.min() >= 1 and got_c.max() <= 16 * n
 
@@ -113,8 +157,8 @@ def test_gemm_large_sampled_rows(bb, oracle):
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
     rows = (I.splitmix64(5, 16, 20) % np.uint64(n)).astype(np.int64)
     want = [_oracle_gemm(oracle, Ae[b:b + 1, rows], Ac[b:b + 1, rows], Be[b:b + 1], Bc[b:b + 1]) for b in range(B)]
-    for bits in (64, 32, 3):                # 3 is the launch configuration bench.py times
-        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
+    for bits, ebits in ((64, 32), (32, 32), (3, 32), (3, 7)):      # (3, 7) is the launch configuration bench.py times
+        Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits, energy_bits=ebits)
         got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
         for b in range(B):
             we, wc = want[b]
@@ -601,34 +645,38 @@ def test_solve_branching_king32_seed1_rank32_leaves(bb):
 
 
 # ---- BBTN on sub-networks: local fixed sets per overflowing stretch of the tree (bbtn_solve_local) ----
-@pytest.mark.parametrize("name,make,t,flags,own_tree", [
-    ("king10", lambda: I.kings_subgraph(10, 10, 0.8, 2), 6, 0, False),
-    ("king12-crt", lambda: I.kings_subgraph(12, 12, 0.8, 3), 7, 1, False),
-    ("king12-sweep", lambda: I.kings_subgraph(12, 12, 0.8, 4, weights="rand"), 8, 0, True),
-    ("king9-full-crt", lambda: I.kings_subgraph(9, 9, 1.0, 0), 5, 1, True),
-    ("ising8", lambda: I.ising_lattice_2d(8, 8, 4), 5, 0, True),
-    ("ising10-field-crt", lambda: I.ising_lattice_2d_half_field(10, 10, 7), 6, 1, False),
-    ("cube3-crt", lambda: I.ising_lattice_3d(3, 3, 3, 2), 6, 1, False),
-    ("cube4", lambda: I.ising_lattice_3d(4, 4, 3, 5), 9, 0, True),
-    ("random-mis", lambda: I.random_graph(26, 0.2, 9, "mis"), 4, 1, False),
+@pytest.mark.parametrize("name,make,t,t2,flags,own_tree", [
+    ("king10", lambda: I.kings_subgraph(10, 10, 0.8, 2), 6, 5, 0, False),
+    ("king12-crt", lambda: I.kings_subgraph(12, 12, 0.8, 3), 9, 8, 1, False),
+    ("king12-sweep", lambda: I.kings_subgraph(12, 12, 0.8, 4, weights="rand"), 11, 10, 0, True),
+    ("king9-full-crt", lambda: I.kings_subgraph(9, 9, 1.0, 0), 9, None, 1, True),
+    ("ising8", lambda: I.ising_lattice_2d(8, 8, 4), 7, None, 0, True),
+    ("ising10-field-crt", lambda: I.ising_lattice_2d_half_field(10, 10, 7), 9, 8, 1, False),
+    ("cube3-crt", lambda: I.ising_lattice_3d(3, 3, 3, 2), 6, 4, 1, False),
+    ("cube4", lambda: I.ising_lattice_3d(4, 4, 3, 5), 13, 12, 0, True),
+    ("random-mis", lambda: I.random_graph(26, 0.2, 9, "mis"), 6, 4, 1, False),
 ])
-def test_solve_local_matches_oracle(bb, oracle, name, make, t, flags, own_tree):
+def test_solve_local_matches_oracle(bb, oracle, name, make, t, t2, flags, own_tree):
     inst = make()
     ref_e, ref_c = oracle.frontier_dp(inst)
     tree = I.elimination_tree(inst.input_index_sets(), I.natural_order(inst.n_vertices)) if own_tree else None
     h = bb.Handle(inst, tree=tree, flags=flags)
     out = h.solve_local(t)
     assert out["sliced_stretches"] >= 1 and out["max_fixed"] >= 1 and out["max_rank"] <= t, out
-    assert out["branches_contracted"] + out["branches_infeasible"] == out["branches_planned"]
+    # every planned branch of a sliced stretch is either contracted or skipped as infeasible (run-once stretches count 1 each)
+    assert out["branches_contracted"] + out["branches_infeasible"] == out["branches_planned"] - (out["stretches"] - out["sliced_stretches"])
     assert (out["energy"], out["count"]) == (ref_e, ref_c & MASK64), (name, out)
     if flags:
         assert out["count_mod"] == (ref_c % bb.BBTN_P1, ref_c % bb.BBTN_P2)
     one = h.solve_local(30)                        # threshold above the width: a single stretch that runs once
     assert one["sliced_stretches"] == 0 and one["branches_contracted"] == 0
     assert (one["energy"], one["count"]) == (ref_e, ref_c & MASK64)
-    # a smaller threshold means more, smaller branches and the same result
-    two = h.solve_local(max(t - 2, 2))
-    assert two["max_rank"] <= max(t - 2, 2) and (two["energy"], two["count"]) == (ref_e, ref_c & MASK64)
+    # a smaller threshold means more, smaller branches and the same result (the number of branches grows fast once the
+    # threshold is far below the width: thresholds are kept within 1..3 of it)
+    if t2 is not None:
+        two = h.solve_local(t2)
+        assert two["max_rank"] <= t2 and two["branches_planned"] > out["branches_planned"]
+        assert (two["energy"], two["count"]) == (ref_e, ref_c & MASK64)
     h.close()
 
 
@@ -647,13 +695,15 @@ def test_solve_local_prunes_with_region_bounds(bb, oracle, kind):
     offs, verts = _grid_regions(rows, cols, 3, 3, ids)
     ref_e, ref_c = oracle.frontier_dp(inst)
     h = bb.Handle(inst, flags=bb.BBTN_COUNT_CRT)
-    plain = h.solve_local(6)
-    exact = h.solve_local(6, region_offsets=offs, region_vertices=verts, incumbent_hint=ref_e)
-    loose = h.solve_local(6, region_offsets=offs, region_vertices=verts, incumbent_hint=ref_e + (3 if kind == "ising" else -3))
+    t = 9 if kind == "mis" else 8
+    plain = h.solve_local(t)
+    exact = h.solve_local(t, region_offsets=offs, region_vertices=verts, incumbent_hint=ref_e)
+    loose = h.solve_local(t, region_offsets=offs, region_vertices=verts, incumbent_hint=ref_e + (3 if kind == "ising" else -3))
     for out in (plain, exact, loose):
         assert (out["energy"], out["count"]) == (ref_e, ref_c & MASK64)
         assert out["count_mod"] == (ref_c % bb.BBTN_P1, ref_c % bb.BBTN_P2)
-        assert out["branches_contracted"] + out["branches_infeasible"] + out["branches_pruned"] == out["branches_planned"]
+        assert out["branches_contracted"] + out["branches_infeasible"] + out["branches_pruned"] == \
+            out["branches_planned"] - (out["stretches"] - out["sliced_stretches"])
     assert plain["branches_pruned"] == 0 and exact["branches_pruned"] >= loose["branches_pruned"]
     assert exact["branches_contracted"] <= plain["branches_contracted"]
     h.close()
