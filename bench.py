@@ -51,8 +51,8 @@ METRIC = "counting-tropical GEMM Gop/s (2 x tropical FMA/s) over one pass of the
 # operand counts, 3 IMADs for full 64x64->64).
 INT_OPS_PER_FMA = {32: 4, 64: 6}
 # executed warp instructions per lane-FMA in the inner loop of gemm_pack16_kernel, counted in the SASS of the in-tree
-# object (profiles/r2_k3_pack16_sass.md): per 32 FMAs 16 VIADDMNMX.S16x2 + 16 IADD + 16 HSETP2 + 32 IMAD + 7 LDS.128
-PACK16_INSTR_PER_FMA = 87.0 / 32.0
+# object (profiles/r2_k3_pack16_sass.md): per 128 FMAs 64 VIADDMNMX.S16x2 + 64 adds + 64 HSETP2 + 128 IMAD + 28 LDS.128 + 16 others
+PACK16_INSTR_PER_FMA = 364.0 / 128.0
 SWEEP = [(64, 1024), (256, 256), (1024, 64), (4096, 2)]                # (n, batch) corners of config 4a
 SWEEP_MODES = [("3:7", "packed 16x2 energies, 32-bit accumulators", 32), ("3:32", "32-bit accumulators", 32),
                ("14:32", "chunk-local 32-bit tie sums, 64-bit accumulators", 32),
@@ -476,7 +476,7 @@ def run_ours(args):
                 "executed_instr_per_fma": PACK16_INSTR_PER_FMA,
                 "executed_frac_of_issue_peak": (PACK16_INSTR_PER_FMA * gemm_gfma / issue_peak) if issue_peak else None,
                 "gemm_gfma_per_s": gemm_gfma, "gemm_gop_per_s": 2 * gemm_gfma, "gemm_ms_per_launch": gemm_ms,
-                "frac_of_opmix_ceiling": gemm_gfma / max(mb["k3mix_2warps"], mb["k3mix_4warps"]),
+                "frac_of_scalar_opmix_ceiling": gemm_gfma / max(mb["k3mix_2warps"], mb["k3mix_4warps"]),
                 "frac_of_alu_pipe_peak_2ops": 2 * gemm_gfma / alu_peak,
                 "microbench_Gops": mb, "share_of_step": gemm_ms * args.steps / ms,
                 "hbm_peak_gbs": hbm_peak, "hbm_peak_kind": peak_kind}

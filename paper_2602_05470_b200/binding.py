@@ -20,7 +20,7 @@ _lib = None
 BBTN_OK, BBTN_EINVAL, BBTN_ENOMEM, BBTN_ECUDA, BBTN_ESHAPE, BBTN_ERANGE = range(6)
 BBTN_NEG_INF = -(1 << 30)
 BBTN_COUNT_CRT, BBTN_IO_DEVICE, BBTN_NO_GRAPH = 0x1, 0x2, 0x4
-BBTN_FORCE_STREAMING, BBTN_FORCE_TILED = 0x10, 0x20
+BBTN_FORCE_STREAMING, BBTN_FORCE_TILED, BBTN_SEARCH_ONLY, BBTN_NO_FUSED = 0x10, 0x20, 0x40, 0x80
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
 EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query",

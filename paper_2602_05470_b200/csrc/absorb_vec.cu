@@ -51,6 +51,12 @@ template <> struct V4<uint32_t> {
   __device__ __forceinline__ void store(uint32_t *p) const { *reinterpret_cast<uint4 *>(p) = make_uint4(v[0], v[1], v[2], v[3]); }
 };
 
+template <> struct V4<NoCount> {                 // search mode: no count plane
+  NoCount v[4];
+  __device__ __forceinline__ void load(const NoCount *) {}
+  __device__ __forceinline__ void store(NoCount *) const {}
+};
+
 __device__ __forceinline__ void load_e4(const int32_t *p, int32_t *d) {
   const int4 a = *reinterpret_cast<const int4 *>(p);
   d[0] = a.x; d[1] = a.y; d[2] = a.z; d[3] = a.w;
@@ -111,7 +117,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
           int32_t acc_e[4]; CT acc_c[4];
           const uint32_t fbf = p.foldB[f];
 #pragma unroll
-          for (int u = 0; u < 4; u++) { acc_e[u] = NEG_INF; acc_c[u] = 0; }
+          for (int u = 0; u < 4; u++) { acc_e[u] = NEG_INF; acc_c[u] = czero<R>(); }
           if (in_regs) {
 #pragma unroll
             for (int k = 0; k < 2; k++) {
@@ -120,7 +126,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
 #pragma unroll
                 for (int u = 0; u < 4; u++) {
                   const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-                  oplus<R>(acc_e[u], acc_c[u], e4[k][u] + be[ib], R::mul(c4[k].v[u], bc[ib]));
+                  oplus<R>(acc_e[u], acc_c[u], e4[k][u] + be[ib], R::mul(c4[k].v[u], ldc<R>(bc, ib)));
                 }
               }
             }
@@ -133,7 +139,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
 #pragma unroll
               for (int u = 0; u < 4; u++) {
                 const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-                oplus<R>(acc_e[u], acc_c[u], ex[u] + be[ib], R::mul(cx.v[u], bc[ib]));
+                oplus<R>(acc_e[u], acc_c[u], ex[u] + be[ib], R::mul(cx.v[u], ldc<R>(bc, ib)));
               }
             }
           }
@@ -157,13 +163,13 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
           const uint32_t fbf = p.foldB[f];
 #pragma unroll
           for (int u = 0; u < 4; u++) {
-            acc_e[u] = NEG_INF; acc_c[u] = 0;
+            acc_e[u] = NEG_INF; acc_c[u] = czero<R>();
 #pragma unroll
             for (int k = 0; k < 2; k++) {
               // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
               const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
               const uint32_t ib = tbo[j] + fbf + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-              oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], bc[ib]));
+              oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], ldc<R>(bc, ib)));
             }
           }
           V4<CT> oc;
@@ -187,7 +193,7 @@ inline bool al32(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 31) =
 bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                        int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
   if (s.rO < 4 || s.nK > 3 || s.rA < 3) return false;
-  if (!al16(Ae) || !al16(Ac) || !al16(Ce) || !al16(Cc)) return false;
+  if (!al16(Ae) || !al16(Ce) || (ring != RING_NONE && (!al16(Ac) || !al16(Cc)))) return false;
   if (ring == RING_U64 && (!al32(Ac) || !al32(Cc))) return false;       // 32-byte count vectors
   int lp;
   if (s.addA[0] == 1u && s.addA[1] == 2u) {

@@ -111,21 +111,57 @@ int upload_tables(bbtn_handle *h, DevPlan *dp) {
   if (!pl.scalar_inputs.empty())
     CUDA_TRY(h, cudaMemcpy(dp->list_scalar.p, pl.scalar_inputs.data(), pl.scalar_inputs.size() * 4, cudaMemcpyHostToDevice));
   CUDA_TRY(h, dp->inv_e.ensure((size_t)pl.arena_invariant_elems * 4));
-  CUDA_TRY(h, dp->inv_c.ensure((size_t)pl.arena_invariant_elems * 8));
+  CUDA_TRY(h, dp->inv_c.ensure((h->P.flags & BBTN_SEARCH_ONLY) ? 0 : (size_t)pl.arena_invariant_elems * 8));
   dp->tables_ready = true;
+  return BBTN_OK;
+}
+
+// Can the plan run as one launch with every tensor of a leaf in shared memory?  (fused_tree.cu)
+int prepare_fused(bbtn_handle *h, DevPlan *dp) {
+  if (dp->fused >= 0) return BBTN_OK;
+  dp->fused = 0;
+  const Plan &pl = dp->plan;
+  if (h->P.flags & BBTN_NO_FUSED) return BBTN_OK;
+  const int64_t arena = pl.arena_variant_elems + pl.arena_invariant_elems;
+  if (pl.max_rank > 13 || arena > 60000 || pl.steps.empty()) return BBTN_OK;
+  int max_smem = 0, dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if ((int64_t)fused_tree_smem_bytes((int)arena, RING_U64) > (int64_t)max_smem) return BBTN_OK;
+  std::vector<FusedStep> fs;
+  for (const Step &s : pl.steps) {
+    if ((s.kind != STEP_ABSORB && s.kind != STEP_REDUCE) || s.rO > 13 || s.nK > 13 || s.n_slice) return BBTN_OK;
+    FusedStep f;
+    std::memset(&f, 0, sizeof(f));
+    f.rO = s.rO; f.nK = s.nK;
+    f.offA = (int32_t)((s.vA ? 0 : pl.arena_variant_elems) + s.offA);
+    f.offB = (int32_t)((s.vB ? 0 : pl.arena_variant_elems) + s.offB);
+    f.offC = (int32_t)((s.vC ? 0 : pl.arena_variant_elems) + s.offC);
+    for (int q = 0; q < s.rO; q++) { f.addA[q] = (uint16_t)s.addA[q]; f.addB[q] = (uint16_t)s.addB[q]; }
+    for (int j = 0; j < s.nK; j++) { f.kA[j] = (uint16_t)s.kA[j]; f.kB[j] = (uint16_t)s.kB[j]; }
+    fs.push_back(f);
+  }
+  std::vector<int32_t> lb;
+  for (size_t t = 0; t < pl.inputs.size(); t++) if (pl.inputs[t].rank > 0) lb.push_back((int32_t)t);
+  CUDA_TRY(h, dp->fused_steps.ensure(fs.size() * sizeof(FusedStep)));
+  CUDA_TRY(h, cudaMemcpy(dp->fused_steps.p, fs.data(), fs.size() * sizeof(FusedStep), cudaMemcpyHostToDevice));
+  CUDA_TRY(h, dp->list_build.upload(lb));
+  dp->n_build = (int)lb.size(); dp->fused_arena = (int)arena;
+  dp->fused = 1;
   return BBTN_OK;
 }
 
 int ensure_batch(bbtn_handle *h, DevPlan *dp, int64_t B, bool host_io) {
   const Plan &pl = dp->plan;
-  if (B > dp->B_cap) {
+  if (B > dp->B_cap && dp->fused != 1) {
     size_t need = (size_t)pl.arena_variant_elems * (size_t)B;
     size_t free_b = 0, total_b = 0;
     CUDA_TRY(h, cudaMemGetInfo(&free_b, &total_b));
-    if (need * 12 > free_b + dp->var_e.bytes + dp->var_c.bytes)
-      return fail(h, BBTN_ENOMEM, "batch needs " + std::to_string(need * 12) + " bytes of device memory");
+    const size_t per_elem = (h->P.flags & BBTN_SEARCH_ONLY) ? 4 : 12;      // search mode has no count plane
+    if (need * per_elem > free_b + dp->var_e.bytes + dp->var_c.bytes)
+      return fail(h, BBTN_ENOMEM, "batch needs " + std::to_string(need * per_elem) + " bytes of device memory");
     CUDA_TRY(h, dp->var_e.ensure(need * 4));
-    CUDA_TRY(h, dp->var_c.ensure(need * 8));
+    CUDA_TRY(h, dp->var_c.ensure(need * (per_elem - 4)));
     CUDA_TRY(h, dp->off_e.ensure((size_t)B * 4));
     CUDA_TRY(h, dp->off_c.ensure((size_t)B * 8));
     dp->B_cap = B;
@@ -145,7 +181,7 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
   const Plan &pl = dp->plan;
   int32_t *ve = (int32_t *)dp->var_e.p, *ie = (int32_t *)dp->inv_e.p;
   char *vc = (char *)dp->var_c.p, *ic = (char *)dp->inv_c.p;
-  const size_t csz = ring == 0 ? 8 : 4;
+  const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
   launch_construct(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_var.p, dp->n_var,
                    (const int32_t *)dp->list_inv.p, dp->n_inv, (const int32_t *)dp->list_scalar.p, dp->n_scalar,
                    d_assign, (int)pl.fixed.size(), B, ve, vc, ie, ic, (int32_t *)dp->off_e.p, dp->off_c.p, ring, st);
@@ -224,6 +260,10 @@ int bbtn_build(const bbtn_problem_desc *d, bbtn_handle **out) {
   }
   P.max_elements = d->max_elements_per_leaf > 0 ? d->max_elements_per_leaf : ((int64_t)1 << 28);
   h->force_mode = (d->flags & BBTN_FORCE_STREAMING) ? 1 : ((d->flags & BBTN_FORCE_TILED) ? 2 : 0);
+  if (d->flags & BBTN_SEARCH_ONLY) {
+    if (d->flags & (BBTN_COUNT_CRT | BBTN_FORCE_TILED)) return fail(nullptr, BBTN_EINVAL, "BBTN_SEARCH_ONLY excludes BBTN_COUNT_CRT and BBTN_FORCE_TILED");
+    h->force_mode = 1;                                   // the energy-only kernels are the streaming forms
+  }
   // validate the tree once on the unsliced network
   if (!P.tree_l.empty()) {
     Plan tmp; std::string err;
@@ -252,8 +292,9 @@ int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, int64
   }
   info->rho = pl.rho;
   info->fma_variant = pl.fma_variant; info->fma_invariant = pl.fma_invariant;
-  info->bytes_per_call = pl.bytes_variant * (double)B + pl.bytes_invariant;
-  info->workspace_bytes = (pl.arena_variant_elems * B + pl.arena_invariant_elems) * 12;
+  const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;      // 4 B per element instead of 12
+  info->bytes_per_call = (pl.bytes_variant * (double)B + pl.bytes_invariant) / (search ? 3.0 : 1.0);
+  info->workspace_bytes = (pl.arena_variant_elems * B + pl.arena_invariant_elems) * (search ? 4 : 12);
   int n_var = 0, n_inv = 0;
   for (const InputRec &r : pl.inputs) if (r.rank > 0) (r.variant ? n_var : n_inv)++;
   // K1: variant tensors, invariant tensors, offset[b]; K4: finalize
@@ -264,7 +305,8 @@ int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, int64
 int bbtn_contract_batch(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, const uint8_t *assign, int64_t B,
                         int32_t *energy, uint64_t *count, uint32_t *count_mod, void *stream) {
   if (!h) return fail(nullptr, BBTN_EINVAL, "null handle");
-  if (B < 1 || !energy || !count || (n_fixed > 0 && !assign)) return fail(h, BBTN_EINVAL, "bad batch arguments");
+  if (B < 1 || !energy || (!count && !(h->P.flags & BBTN_SEARCH_ONLY)) || (n_fixed > 0 && !assign))
+    return fail(h, BBTN_EINVAL, "bad batch arguments");
   const bool crt = (h->P.flags & BBTN_COUNT_CRT) != 0;
   if (count_mod && !crt) return fail(h, BBTN_EINVAL, "count_mod needs a handle built with BBTN_COUNT_CRT");
   if (!have_device()) return fail(h, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
@@ -289,7 +331,8 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
   // a power of two (padding leaves = assignment 0, results dropped): the CUDA graph of this fixed set is then
   // captured once per size class instead of once per distinct B (the host B&B loop sends ragged batches).
   const int64_t B_user = B;
-  if (!dev_io) {
+  if ((rc = prepare_fused(h, dp))) return rc;
+  if (!dev_io && dp->fused != 1) {
     int64_t bp = 1; while (bp < B) bp <<= 1;
     // pad only when the padded arena fits; a ragged B just above a power of two must not turn into ENOMEM
     size_t free_b = 0, total_b = 0;
@@ -309,10 +352,19 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
         CUDA_TRY(h, cudaMemsetAsync((char *)dp->assign.p + (size_t)B_user * n_fixed, 0, (size_t)(B - B_user) * n_fixed, st));
     }
   }
-  const int n_rings = (crt && d_mod) ? 3 : 1;
+  const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;
+  const int n_rings = search ? 1 : ((crt && d_mod) ? 3 : 1);
+  const int ring0 = search ? (int)RING_NONE : (int)RING_U64;
   const bool use_graph = allow_graph && !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
-  if (!use_graph) {
-    for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring, st);
+  if (dp->fused == 1) {
+    const Plan &pl = dp->plan;
+    for (int ring = 0; ring < n_rings; ring++)
+      launch_fused_tree(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_build.p, dp->n_build,
+                        (const int32_t *)dp->list_scalar.p, dp->n_scalar, d_assign, n_fixed, B, (const FusedStep *)dp->fused_steps.p,
+                        (int)pl.steps.size(), dp->fused_arena, (int)pl.arena_variant_elems, (int)pl.result_offset,
+                        d_energy, d_count, d_mod, ring0 + ring, st);
+  } else if (!use_graph) {
+    for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring0 + ring, st);
   } else {
     const void *io[4] = {d_assign, d_energy, d_count, d_mod};
     const bool stale = dp->graph_B != B || (int)dp->graphs.size() != n_rings || std::memcmp(io, dp->graph_io, sizeof(io)) != 0;
@@ -325,7 +377,7 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
       for (int ring = 0; ring < n_rings && ce == cudaSuccess; ring++) {
         cudaGraph_t g = nullptr; cudaGraphExec_t ge = nullptr;
         if ((ce = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal)) != cudaSuccess) break;
-        enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring, cs);
+        enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring0 + ring, cs);
         ce = cudaStreamEndCapture(cs, &g);          // always ends the capture, also after a failed launch
         if (ce == cudaSuccess) ce = cudaGraphInstantiate(&ge, g, 0);
         if (g) cudaGraphDestroy(g);
@@ -346,10 +398,11 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
     // stage into temporaries so that outputs stay untouched on error
     std::vector<int32_t> te((size_t)B_user); std::vector<uint64_t> tc((size_t)B_user); std::vector<uint32_t> tm(count_mod ? (size_t)B_user * 2 : 0);
     CUDA_TRY(h, cudaMemcpyAsync(te.data(), d_energy, (size_t)B_user * 4, cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(h, cudaMemcpyAsync(tc.data(), d_count, (size_t)B_user * 8, cudaMemcpyDeviceToHost, st));
+    if (count) CUDA_TRY(h, cudaMemcpyAsync(tc.data(), d_count, (size_t)B_user * 8, cudaMemcpyDeviceToHost, st));
     if (count_mod) CUDA_TRY(h, cudaMemcpyAsync(tm.data(), d_mod, (size_t)B_user * 8, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(h, cudaStreamSynchronize(st));
-    std::memcpy(energy, te.data(), (size_t)B_user * 4); std::memcpy(count, tc.data(), (size_t)B_user * 8);
+    std::memcpy(energy, te.data(), (size_t)B_user * 4);
+    if (count) std::memcpy(count, tc.data(), (size_t)B_user * 8);
     if (count_mod) std::memcpy(count_mod, tm.data(), (size_t)B_user * 8);
   }
   return BBTN_OK;

@@ -148,7 +148,7 @@ struct Brancher {
       std::string err;
       int rc = make_plan(*P, trail, h->force_mode, false, dp->plan, err, true, false);
       if (rc) return fail(h, rc, err);
-      dp->tables_ready = false; dp->B_cap = 0; dp->graph_B = -1;
+      dp->tables_ready = false; dp->B_cap = 0; dp->graph_B = -1; dp->fused = -1;
       const int64_t bytes = dp->plan.arena_variant_elems * 12;
       if (mem_budget <= 0 || bytes <= mem_budget || tt <= 4) return emit_leaf(&dp->plan);
       while (tt > 4 && rho(tt) == 0) tt--;

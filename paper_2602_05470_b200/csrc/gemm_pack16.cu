@@ -19,7 +19,7 @@
 //   * every half is below 0x7C00: read as an fp16 bit pattern it is a finite non-negative number, and for
 //     those the order (and equality) of bit patterns is the order of the numbers -- which is why the
 //     half-precision compare HSETP2 can deliver the integer tie test for both halves at once.
-// Tile 128 x 128, 256 threads, 8 x 8 outputs per thread (8 rows x 4 packed column pairs), BK = 16, raw cp.async
+// Tile 128 x 128, 512 threads (4 warps per SM sub-partition), 4 x 8 outputs per thread (4 rows x 4 packed column pairs), BK = 16, raw cp.async
 // stages + converted (encoded, k-major) stages as in gemm_tiled.cu.
 #include "gemm_stage.cuh"
 #include <type_traits>
@@ -31,6 +31,7 @@ using namespace stage;
 
 constexpr int BIAS = 11903, FINITE2 = 15872;   // enc(e) = e + BIAS;  half >= FINITE2  <=>  finite sum
 constexpr int BN = 128;
+constexpr int PT = 512;                            // threads per CTA: 4 x 8 outputs each, 4 warps per SM sub-partition
 constexpr int P_RAW = AE_BYTES + AC_BYTES + BK * BN * 4 + BK * BN * 8;
 constexpr int P_CAE = BK * BM * 4, P_CAC = BK * BM * 4, P_CBE = BK * (BN / 2) * 4, P_CBC = BK * BN * 4;
 constexpr int P_CONV = P_CAE + P_CAC + P_CBE + P_CBC;
@@ -39,15 +40,27 @@ static_assert(P_SMEM <= 227 * 1024, "shared memory budget");
 
 __device__ __forceinline__ uint32_t enc(int32_t e) { return e < ZERO_BELOW ? 0u : (uint32_t)(e + BIAS); }
 
-// pass 2 for one packed pair: s2 = a2 + b2; the halves that equal E2 add their count products
+// pass 2 for one packed pair: s2 = a2 + b2; the halves that equal E2 add their count products.
+// ON_ALU: the add is written with a carry-out, which only the ALU pipe's IADD3 has; left alone ptxas issues every one
+// of these adds as IMAD.IADD and the FMA pipe (2 IMAD + 1 add per pair) becomes the bottleneck while the ALU pipe
+// (VIADDMNMX + HSETP2) idles a third of the time.  Alternating the two forms balances the pipes.
+template <bool ON_ALU>
 __device__ __forceinline__ void tie2(uint32_t &c_lo, uint32_t &c_hi, uint32_t a2, uint32_t b2, uint32_t E2, uint32_t ca,
                                      uint32_t cb_lo, uint32_t cb_hi) {
-  asm("{\n\t.reg .pred p, q;\n\t.reg .b32 s;\n\t"
-      "add.u32 s, %2, %3;\n\t"
-      "setp.eq.f16x2 p|q, s, %4;\n\t"
-      "@p mad.lo.u32 %0, %5, %6, %0;\n\t"
-      "@q mad.lo.u32 %1, %5, %7, %1;\n\t}"
-      : "+r"(c_lo), "+r"(c_hi) : "r"(a2), "r"(b2), "r"(E2), "r"(ca), "r"(cb_lo), "r"(cb_hi));
+  if (ON_ALU)
+    asm("{\n\t.reg .pred p, q;\n\t.reg .b32 s;\n\t"
+        "add.cc.u32 s, %2, %3;\n\t"
+        "setp.eq.f16x2 p|q, s, %4;\n\t"
+        "@p mad.lo.u32 %0, %5, %6, %0;\n\t"
+        "@q mad.lo.u32 %1, %5, %7, %1;\n\t}"
+        : "+r"(c_lo), "+r"(c_hi) : "r"(a2), "r"(b2), "r"(E2), "r"(ca), "r"(cb_lo), "r"(cb_hi));
+  else
+    asm("{\n\t.reg .pred p, q;\n\t.reg .b32 s;\n\t"
+        "add.u32 s, %2, %3;\n\t"
+        "setp.eq.f16x2 p|q, s, %4;\n\t"
+        "@p mad.lo.u32 %0, %5, %6, %0;\n\t"
+        "@q mad.lo.u32 %1, %5, %7, %1;\n\t}"
+        : "+r"(c_lo), "+r"(c_hi) : "r"(a2), "r"(b2), "r"(E2), "r"(ca), "r"(cb_lo), "r"(cb_hi));
 }
 // a new maximum in a half drops the count of the old one
 __device__ __forceinline__ void reset2(uint32_t &c_lo, uint32_t &c_hi, uint32_t En2, uint32_t E2) {
@@ -70,38 +83,38 @@ __device__ __forceinline__ void convert_pack16(const unsigned char *raw, unsigne
   uint32_t *cBc = reinterpret_cast<uint32_t *>(conv + P_CAE + P_CAC + P_CBE);
   if (A_KMAJOR) {
 #pragma unroll
-    for (int idx = t; idx < BK * BM / 4; idx += NT) {
+    for (int idx = t; idx < BK * BM / 4; idx += PT) {
       const int4 v = *reinterpret_cast<const int4 *>(rAe + 16 * idx);
       *reinterpret_cast<uint4 *>(cAe + 4 * idx) = make_uint4(enc(v.x) * 0x10001u, enc(v.y) * 0x10001u, enc(v.z) * 0x10001u, enc(v.w) * 0x10001u);
     }
 #pragma unroll
-    for (int idx = t; idx < BK * BM / 2; idx += NT) {
+    for (int idx = t; idx < BK * BM / 2; idx += PT) {
       const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rAc + 16 * idx);
       *reinterpret_cast<uint2 *>(cAc + 2 * idx) = make_uint2((uint32_t)v.x, (uint32_t)v.y);
     }
   } else {
-    const int r = t % BM, kb = (t / BM) * (BK / 2);
-#pragma unroll
-    for (int q = 0; q < BK / 8; q++) {
-      const int4 v = *reinterpret_cast<const int4 *>(rAe + (r * AE_LD + kb + 4 * q) * 4);
-      cAe[(kb + 4 * q + 0) * BM + r] = enc(v.x) * 0x10001u; cAe[(kb + 4 * q + 1) * BM + r] = enc(v.y) * 0x10001u;
-      cAe[(kb + 4 * q + 2) * BM + r] = enc(v.z) * 0x10001u; cAe[(kb + 4 * q + 3) * BM + r] = enc(v.w) * 0x10001u;
+    // transpose: lane = row, so the k-major stores of a warp are contiguous; each thread moves 4 k of one row
+    const int r = t % BM, kb = (t / BM) * 4;               // PT / BM = 4 groups x 4 k = BK
+    {
+      const int4 v = *reinterpret_cast<const int4 *>(rAe + (r * AE_LD + kb) * 4);
+      cAe[(kb + 0) * BM + r] = enc(v.x) * 0x10001u; cAe[(kb + 1) * BM + r] = enc(v.y) * 0x10001u;
+      cAe[(kb + 2) * BM + r] = enc(v.z) * 0x10001u; cAe[(kb + 3) * BM + r] = enc(v.w) * 0x10001u;
     }
 #pragma unroll
-    for (int q = 0; q < BK / 4; q++) {
+    for (int q = 0; q < 2; q++) {
       const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rAc + (r * AC_LD + kb + 2 * q) * 8);
       cAc[(kb + 2 * q + 0) * BM + r] = (uint32_t)v.x; cAc[(kb + 2 * q + 1) * BM + r] = (uint32_t)v.y;
     }
   }
 #pragma unroll
-  for (int idx = t; idx < BK * BN / 4; idx += NT) {            // 4 consecutive columns -> two packed words
+  for (int idx = t; idx < BK * BN / 4; idx += PT) {            // 4 consecutive columns -> two packed words
     const int kk = idx / (BN / 4), c4 = idx % (BN / 4);       // columns 4*c4 .. 4*c4+3: q = c4 / 16, tx = c4 % 16
     const int4 v = *reinterpret_cast<const int4 *>(rBe + 16 * idx);
     *reinterpret_cast<uint2 *>(cBe + kk * (BN / 2) + (c4 % 16) * 4 + (c4 / 16) * 2) =
         make_uint2(enc(v.x) | (enc(v.y) << 16), enc(v.z) | (enc(v.w) << 16));
   }
 #pragma unroll
-  for (int idx = t; idx < BK * BN / 2; idx += NT) {
+  for (int idx = t; idx < BK * BN / 2; idx += PT) {
     const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rBc + 16 * idx);
     *reinterpret_cast<uint2 *>(cBc + 2 * idx) = make_uint2((uint32_t)v.x, (uint32_t)v.y);
   }
@@ -113,7 +126,7 @@ __device__ __forceinline__ void lds4(const uint32_t *src, uint32_t *dst) {
 }
 
 template <bool A_KMAJOR>
-__global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
+__global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
   extern __shared__ __align__(16) unsigned char smem[];
   unsigned char *conv_base = smem + RAW_STAGES * P_RAW;
 
@@ -126,14 +139,14 @@ __global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
   const int32_t *be = p.Be + b * p.sB + g * (int64_t)p.K * p.N; const uint64_t *bc = p.Bc + b * p.sB + g * (int64_t)p.K * p.N;
   int32_t *ce = p.Ce + b * p.sC + g * (int64_t)p.M * p.N; uint64_t *cc = p.Cc + b * p.sC + g * (int64_t)p.M * p.N;
 
-  // a warp covers 8 tx x 4 ty (as in gemm_tiled.cu): A fetches touch 4 distinct 16-byte granules, B fetches 8
+  // a warp covers 8 tx x 4 ty: A fetches touch 4 distinct 16-byte granules, B fetches 8; 16 warps = 2 (tx) x 8 (ty)
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tx = (w & 1) * 8 + (lane & 7), ty = (w >> 1) * 4 + (lane >> 3);
+  const int tx = (w & 1) * 8 + (lane & 7), ty = (w >> 1) * 4 + (lane >> 3);      // tx 0..15, ty 0..31
 
-  // rows: rb*64 + ty*4 + i (rb = 0,1; i = 0..3); columns: q*64 + tx*4 + 2p + half (q = 0,1; p = 0,1)
-  uint32_t E2[8][4], C[8][8];
+  // rows: ty*4 + i (i = 0..3); columns: q*64 + tx*4 + 2p + half (q = 0,1; p = 0,1)
+  uint32_t E2[4][4], C[4][8];
 #pragma unroll
-  for (int i = 0; i < 8; i++) {
+  for (int i = 0; i < 4; i++) {
 #pragma unroll
     for (int j = 0; j < 4; j++) E2[i][j] = 0u;
 #pragma unroll
@@ -144,8 +157,8 @@ __global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
   auto issue = [&](int c) {
     if (c < n_chunks) {
       unsigned char *s = smem + (c % RAW_STAGES) * P_RAW;
-      fill_A<A_KMAJOR>(p, ae, ac, m0, c * BK, s, s + AE_BYTES);
-      fill_B<BN>(p, be, bc, n0, c * BK, s + AE_BYTES + AC_BYTES, s + AE_BYTES + AC_BYTES + BK * BN * 4);
+      fill_A<A_KMAJOR, PT>(p, ae, ac, m0, c * BK, s, s + AE_BYTES);
+      fill_B<BN, PT>(p, be, bc, n0, c * BK, s + AE_BYTES + AC_BYTES, s + AE_BYTES + AC_BYTES + BK * BN * 4);
     }
     cp_async_commit();
   };
@@ -154,8 +167,8 @@ __global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
   };
 
   // pass 1 of one chunk on row block rb: En2 <- max(En2, a2 + b2)
-  auto pass1 = [&](const unsigned char *s1, int rb, uint32_t (&En)[4][4]) {
-    const uint32_t *a1e = reinterpret_cast<const uint32_t *>(s1) + rb * 64 + ty * 4;
+  auto pass1 = [&](const unsigned char *s1, uint32_t (&En)[4][4]) {
+    const uint32_t *a1e = reinterpret_cast<const uint32_t *>(s1) + ty * 4;
     const uint32_t *b1e = reinterpret_cast<const uint32_t *>(s1 + P_CAE + P_CAC) + tx * 4;
 #pragma unroll 4
     for (int kk = 0; kk < BK; kk++) {
@@ -169,12 +182,12 @@ __global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
   };
 
   // one unit: pass 2 of chunk c on row block rb, interleaved with pass 1 of chunk c+1 on the same rows
-  auto unit = [&](auto do_p1, auto rb_tag, int c) {
+  auto unit = [&](auto do_p1, int c) {
     constexpr bool P1 = decltype(do_p1)::value;
-    constexpr int rb = decltype(rb_tag)::value;
+    constexpr int rb = 0;
     const unsigned char *s2 = conv_base + (c % CONV_STAGES) * P_CONV;
     const unsigned char *s1 = conv_base + ((c + 1) % CONV_STAGES) * P_CONV;
-    const int mrow = rb * 64 + ty * 4;
+    const int mrow = ty * 4;
     const uint32_t *a2e = reinterpret_cast<const uint32_t *>(s2) + mrow;
     const uint32_t *a2c = reinterpret_cast<const uint32_t *>(s2 + P_CAE) + mrow;
     const uint32_t *b2e = reinterpret_cast<const uint32_t *>(s2 + P_CAE + P_CAC) + tx * 4;
@@ -201,7 +214,10 @@ __global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
 #pragma unroll
         for (int j = 0; j < 4; j++) {                        // j = q*2 + p: columns q*64 + tx*4 + 2p, +1
           if (P1) En[i][j] = __viaddmax_s16x2(a1[i], b1[j], En[i][j]);
-          tie2(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], a2[i], b2[j], E2[rb * 4 + i][j], ca[i], cb[2 * j], cb[2 * j + 1]);
+          if ((i * 4 + j) % 8 < 5)                       // 10 of 16 adds on the ALU pipe: ALU 42 / FMA 38 instructions per kk
+            tie2<true>(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], a2[i], b2[j], E2[rb * 4 + i][j], ca[i], cb[2 * j], cb[2 * j + 1]);
+          else
+            tie2<false>(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], a2[i], b2[j], E2[rb * 4 + i][j], ca[i], cb[2 * j], cb[2 * j + 1]);
         }
     }
     if (P1) {
@@ -222,39 +238,21 @@ __global__ void __launch_bounds__(NT, 1) gemm_pack16_kernel(const GemmArgs p) {
   convert(0); convert(1);
   __syncthreads();
   issue(2);
-#pragma unroll
-  for (int rb = 0; rb < 2; rb++) {
-    uint32_t En[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; i++)
-#pragma unroll
-      for (int j = 0; j < 4; j++) En[i][j] = 0u;
-    pass1(conv_base, rb, En);
-#pragma unroll
-    for (int i = 0; i < 4; i++)
-#pragma unroll
-      for (int j = 0; j < 4; j++) E2[rb * 4 + i][j] = En[i][j];
-  }
+  pass1(conv_base, E2);
 
   for (int c = 0; c < n_chunks; c++) {
     cp_async_wait<0>();
     __syncthreads();
     convert(c + 2);
     issue(c + 3);
-    if (c + 1 < n_chunks) {
-      unit(std::true_type{}, std::integral_constant<int, 0>{}, c);
-      unit(std::true_type{}, std::integral_constant<int, 1>{}, c);
-    } else {
-      unit(std::false_type{}, std::integral_constant<int, 0>{}, c);
-      unit(std::false_type{}, std::integral_constant<int, 1>{}, c);
-    }
+    if (c + 1 < n_chunks) unit(std::true_type{}, c); else unit(std::false_type{}, c);
   }
   cp_async_wait<0>();
 
   // ---------------- epilogue: decode, canonicalise, store ----------------
 #pragma unroll
-  for (int i = 0; i < 8; i++) {
-    const int gm = m0 + (i >> 2) * 64 + ty * 4 + (i & 3);
+  for (int i = 0; i < 4; i++) {
+    const int gm = m0 + ty * 4 + i;
     if (gm >= p.M) continue;
 #pragma unroll
     for (int q = 0; q < 2; q++) {
@@ -298,10 +296,10 @@ void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kma
   const int64_t n_cta = (int64_t)((N + BN - 1) / BN) * ((M + BM - 1) / BM) * batch * G;
   if (a_kmajor) {
     cudaFuncSetAttribute(gemm_pack16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM);
-    gemm_pack16_kernel<true><<<dim3((unsigned)n_cta), NT, P_SMEM, st>>>(a);
+    gemm_pack16_kernel<true><<<dim3((unsigned)n_cta), PT, P_SMEM, st>>>(a);
   } else {
     cudaFuncSetAttribute(gemm_pack16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM);
-    gemm_pack16_kernel<false><<<dim3((unsigned)n_cta), NT, P_SMEM, st>>>(a);
+    gemm_pack16_kernel<false><<<dim3((unsigned)n_cta), PT, P_SMEM, st>>>(a);
   }
 }
 

@@ -7,7 +7,7 @@
 namespace bbtn {
 namespace stage {
 
-constexpr int BM = 128, BK = 16, NT = 256;
+constexpr int BM = 128, BK = 16, NT = 256;   // NT: threads of the 32-bit kernels (the fill functions take it as a parameter)
 constexpr int RAW_STAGES = 2, CONV_STAGES = 3;
 constexpr int AE_LD = BK + 4;            // row-major A energies: [BM][AE_LD] int32 (row stride 80 B)
 constexpr int AC_LD = BK + 2;            // row-major A counts:   [BM][AC_LD] uint64 (row stride 144 B)
@@ -31,7 +31,7 @@ struct GemmArgs {
 };
 
 // ---- global -> shared for one chunk (k0 .. k0+BK) of one operand ------------------------------
-template <bool A_KMAJOR>
+template <bool A_KMAJOR, int NT = 256>
 __device__ __forceinline__ void fill_A(const GemmArgs &p, const int32_t *__restrict__ ae, const uint64_t *__restrict__ ac,
                                        int m0, int k0, unsigned char *sAe, unsigned char *sAc) {
   const int t = threadIdx.x;
@@ -78,7 +78,7 @@ __device__ __forceinline__ void fill_A(const GemmArgs &p, const int32_t *__restr
   }
 }
 
-template <int BNt>
+template <int BNt, int NT = 256>
 __device__ __forceinline__ void fill_B(const GemmArgs &p, const int32_t *__restrict__ be, const uint64_t *__restrict__ bc,
                                        int n0, int k0, unsigned char *sBe, unsigned char *sBc) {
   const int t = threadIdx.x;

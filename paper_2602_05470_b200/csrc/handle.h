@@ -39,6 +39,10 @@ struct DevPlan {
   int n_var = 0, n_inv = 0, n_scalar = 0;
   DevBuf var_e, var_c, inv_e, inv_c, off_e, off_c;
   DevBuf assign, energy, count, count_mod;      // staging for host-pointer calls
+  // small networks (every tensor of a leaf fits shared memory): the whole plan runs as one launch (fused_tree.cu)
+  DevBuf fused_steps, list_build;
+  int fused = -1;                               // -1 not decided yet, 0 no, 1 yes
+  int n_build = 0, fused_arena = 0;
   bool tables_ready = false;
   int64_t B_cap = 0;
   std::vector<cudaGraphExec_t> graphs;          // per ring, for graph_B

@@ -1,38 +1,11 @@
 // kernels.cu -- K1 construct, K3 streaming/long-reduction forms, K4 finalize (sm_100a).
 #include "kernels.h"
 #include "ring.cuh"
+#include "construct.cuh"
+#include <type_traits>
 
 namespace bbtn {
 namespace {
-
-// ---------------------------------------------------------------------------------------------
-// Input tensor entries, max-plus form (PAPER.md:49 Ising B and w, :55 MWIS B and w; A1-A3):
-//   Ising  bond [su][sv] = +J*sigma(su)*sigma(sv), vertex [s] = +h*sigma(s), sigma(s) = 2s-1, count 1
-//   MIS    bond = (0,1) except [1][1] = zero element; vertex = (0,1), (w,1)
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ int32_t entry_energy(int kind, int type, int32_t w, int su, int sv) {
-  if (kind == 0) {
-    int32_t s = (2 * su - 1) * (type == 0 ? (2 * sv - 1) : 1);
-    return w * s;
-  }
-  if (type == 0) return (su & sv) ? NEG_INF : 0;
-  return su ? w : 0;
-}
-
-// value of input tensor `r` at free bits (xu, xv), pre-summing single-owner indices (reading A7)
-template <class R>
-__device__ __forceinline__ void input_element(int kind, const InputRec &r, int fu_val, int fv_val, int xu, int xv,
-                                              int32_t &e, typename R::T &c) {
-  e = NEG_INF; c = 0;
-  const int nu = r.su ? 2 : 1, nv = r.sv ? 2 : 1;
-  for (int a = 0; a < nu; a++)
-    for (int b = 0; b < nv; b++) {
-      int su = r.fu >= 0 ? fu_val : (r.su ? a : xu);
-      int sv = r.v < 0 ? 0 : (r.fv >= 0 ? fv_val : (r.sv ? b : xv));
-      int32_t ee = entry_energy(kind, r.type, r.w, su, sv);
-      if (ee > ZERO_BELOW) oplus<R>(e, c, ee, R::from_small(1));
-    }
-}
 
 template <class R>
 __global__ void construct_tensors_kernel(int kind, const InputRec *__restrict__ inputs, const int32_t *__restrict__ list,
@@ -52,7 +25,7 @@ __global__ void construct_tensors_kernel(int kind, const InputRec *__restrict__ 
       int32_t e; typename R::T c;
       input_element<R>(kind, r, fu_val, fv_val, xu, xv, e, c);
       out_e[base + x] = e;
-      out_c[base + x] = c;
+      stc<R>(out_c, base + x, c);
     }
   }
 }
@@ -73,7 +46,7 @@ __global__ void construct_offset_kernel(int kind, const InputRec *__restrict__ i
       acc_e += e; acc_c = R::mul(acc_c, c);
       canonicalise<R>(acc_e, acc_c);
     }
-    off_e[b] = acc_e; off_c[b] = acc_c;
+    off_e[b] = acc_e; stc<R>(off_c, b, acc_c);
   }
 }
 
@@ -99,17 +72,17 @@ __global__ void absorb_kernel(AbsorbArgs p, const int32_t *__restrict__ Ae, cons
     for (int q = 0; q < p.rO; q++) if ((o >> q) & 1u) { a0 += p.addA[q]; b0 += p.addB[q]; }
     const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
     const int32_t *be = Be + b * p.sB; const typename R::T *bc = Bc + b * p.sB;
-    int32_t acc_e = NEG_INF; typename R::T acc_c = 0;
+    int32_t acc_e = NEG_INF; typename R::T acc_c = czero<R>();
     for (uint64_t k = 0; k < (1ull << p.nK); k++) {        // nK may be 32
       uint32_t ia = a0, ib = b0;
       for (int j = 0; j < p.nK; j++) if ((k >> j) & 1ull) { ia += p.kA[j]; ib += p.kB[j]; }
       const int32_t e = ae[ia] + be[ib];
-      const typename R::T c = R::mul(ac[ia], bc[ib]);
+      const typename R::T c = R::mul(ldc<R>(ac, ia), ldc<R>(bc, ib));
       oplus<R>(acc_e, acc_c, e, c);
     }
     canonicalise<R>(acc_e, acc_c);
     Ce[b * p.sC + o] = acc_e;
-    Cc[b * p.sC + o] = acc_c;
+    stc<R>(Cc, b * p.sC + o, acc_c);
   }
 }
 
@@ -125,7 +98,7 @@ __global__ void reduce_kernel(ReduceArgs p, const int32_t *__restrict__ Ae, cons
                               const int32_t *__restrict__ Be, const typename R::T *__restrict__ Bc,
                               int32_t *__restrict__ Ce, typename R::T *__restrict__ Cc) {
   __shared__ int32_t sh_e[32];
-  __shared__ typename R::T sh_c[32];
+  __shared__ typename std::conditional<R::kCounts, typename R::T, char>::type sh_c[32];
   const int64_t t = blockIdx.x;
   const int64_t b = t >> p.rO;
   const uint32_t o = (uint32_t)t & ((1u << p.rO) - 1u);
@@ -133,34 +106,34 @@ __global__ void reduce_kernel(ReduceArgs p, const int32_t *__restrict__ Ae, cons
   for (int q = 0; q < p.rO; q++) if ((o >> q) & 1u) { a0 += p.addA[q]; b0 += p.addB[q]; }
   const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
   const int32_t *be = Be + b * p.sB; const typename R::T *bc = Bc + b * p.sB;
-  int32_t acc_e = NEG_INF; typename R::T acc_c = 0;
+  int32_t acc_e = NEG_INF; typename R::T acc_c = czero<R>();
   for (uint64_t k = threadIdx.x; k < (1ull << p.nK); k += blockDim.x) {      // nK may be 32
     uint32_t ia = a0, ib = b0;
     for (int j = 0; j < p.nK; j++) if ((k >> j) & 1ull) { ia += p.kA[j]; ib += p.kB[j]; }
-    oplus<R>(acc_e, acc_c, ae[ia] + be[ib], R::mul(ac[ia], bc[ib]));
+    oplus<R>(acc_e, acc_c, ae[ia] + be[ib], R::mul(ldc<R>(ac, ia), ldc<R>(bc, ib)));
   }
   // warp (+), then across warps
   for (int d = 16; d > 0; d >>= 1) {
     int32_t oe = __shfl_xor_sync(0xffffffffu, acc_e, d);
-    typename R::T oc = __shfl_xor_sync(0xffffffffu, acc_c, d);
+    typename R::T oc = shfl_xor_c<R>(acc_c, d);
     oplus<R>(acc_e, acc_c, oe, oc);
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  if (lane == 0) { sh_e[warp] = acc_e; sh_c[warp] = acc_c; }
+  if (lane == 0) { sh_e[warp] = acc_e; if constexpr (R::kCounts) sh_c[warp] = acc_c; }
   __syncthreads();
   if (warp == 0) {
     const int nw = blockDim.x >> 5;
     acc_e = lane < nw ? sh_e[lane] : NEG_INF;
-    acc_c = lane < nw ? sh_c[lane] : 0;
+    if constexpr (R::kCounts) acc_c = lane < nw ? sh_c[lane] : 0;
     for (int d = 16; d > 0; d >>= 1) {
       int32_t oe = __shfl_xor_sync(0xffffffffu, acc_e, d);
-      typename R::T oc = __shfl_xor_sync(0xffffffffu, acc_c, d);
+      typename R::T oc = shfl_xor_c<R>(acc_c, d);
       oplus<R>(acc_e, acc_c, oe, oc);
     }
     if (lane == 0) {
       canonicalise<R>(acc_e, acc_c);
       Ce[b * p.sC + o] = acc_e;
-      Cc[b * p.sC + o] = acc_c;
+      stc<R>(Cc, b * p.sC + o, acc_c);
     }
   }
 }
@@ -175,11 +148,14 @@ __global__ void finalize_kernel(int kind, int64_t B, const int32_t *__restrict__
                                 int32_t *__restrict__ energy, uint64_t *__restrict__ count,
                                 uint32_t *__restrict__ count_mod, int ring) {
   for (int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; b < B; b += (int64_t)gridDim.x * blockDim.x) {
-    int32_t e = off_e[b]; typename R::T c = off_c[b];
-    if (root_e) { e += root_e[b * root_stride]; c = R::mul(c, root_c[b * root_stride]); }
+    int32_t e = off_e[b]; typename R::T c = ldc<R>(off_c, b);
+    if (root_e) { e += root_e[b * root_stride]; c = R::mul(c, ldc<R>(root_c, b * root_stride)); }
     canonicalise<R>(e, c);
     const bool zero = e == NEG_INF;
-    if (ring == 0) {
+    if constexpr (!R::kCounts) {                       // search mode: the energy alone; the count output reads 0
+      energy[b] = zero ? NEG_INF : (kind == 0 ? -e : e);
+      if (count) count[b] = 0;
+    } else if (ring == 0) {
       energy[b] = zero ? NEG_INF : (kind == 0 ? -e : e);
       count[b] = (uint64_t)c;
     } else if (count_mod) {
@@ -194,15 +170,15 @@ __global__ void accumulate_kernel(int64_t n, const int32_t *__restrict__ slice_e
                                   const int32_t *__restrict__ off_e, const typename R::T *__restrict__ off_c,
                                   int32_t *__restrict__ acc_e, typename R::T *__restrict__ acc_c, int first) {
   int32_t oe = 0; typename R::T oc = R::from_small(1);
-  if (slice_e) { oe = off_e[0]; oc = off_c[0]; }
+  if (slice_e) { oe = off_e[0]; oc = ldc<R>(off_c, 0); }
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    int32_t e = NEG_INF; typename R::T c = 0;
+    int32_t e = NEG_INF; typename R::T c = czero<R>();
     if (slice_e) {
-      e = slice_e[i] + oe; c = R::mul(slice_c[i], oc);
+      e = slice_e[i] + oe; c = R::mul(ldc<R>(slice_c, i), oc);
       canonicalise<R>(e, c);
-      if (!first) { int32_t ae = acc_e[i]; typename R::T ac = acc_c[i]; oplus<R>(ae, ac, e, c); e = ae; c = ac; }
+      if (!first) { int32_t ae = acc_e[i]; typename R::T ac = ldc<R>(acc_c, i); oplus<R>(ae, ac, e, c); e = ae; c = ac; }
     }
-    acc_e[i] = e; acc_c[i] = c;
+    acc_e[i] = e; stc<R>(acc_c, i, c);
   }
 }
 

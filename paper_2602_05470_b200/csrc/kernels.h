@@ -7,7 +7,7 @@
 
 namespace bbtn {
 
-enum RingId : int { RING_U64 = 0, RING_P1 = 1, RING_P2 = 2 };   // counts mod 2^64 / mod 2^31-1 / mod 2^31-19
+enum RingId : int { RING_U64 = 0, RING_P1 = 1, RING_P2 = 2, RING_NONE = 3 };   // counts mod 2^64 / mod 2^31-1 / mod 2^31-19 / no counts (search mode)
 
 constexpr int32_t kNegInf = -(1 << 30);
 constexpr int32_t kZeroThreshold = -(1 << 29);   // e < threshold  <=>  zero element (reading A8)
@@ -57,6 +57,18 @@ void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kma
 // locally fixed indices (Eq. 3, on a sub-network; plan.h "local slicing").
 void launch_accumulate(int64_t n, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
                        int32_t *acc_e, void *acc_c, int first, int ring, cudaStream_t st);
+
+// K1..K4 of a small network in ONE launch (fused_tree.cu): one CTA per leaf, every tensor in shared memory.
+// A step is C[o] = (+)_k A[fa(o) + ka(k)] (.) B[fb(o) + kb(k)] with shared-memory element offsets.
+struct FusedStep {
+  int32_t rO, nK, offA, offB, offC, pad;
+  uint16_t addA[16], addB[16], kA[16], kB[16];
+};
+size_t fused_tree_smem_bytes(int arena_elems, int ring);
+void launch_fused_tree(int kind, const InputRec *d_inputs, const int32_t *d_list_build, int n_build,
+                       const int32_t *d_list_scalar, int n_scalar, const uint8_t *d_assign, int n_fixed, int64_t B,
+                       const FusedStep *d_steps, int n_steps, int arena_elems, int inv_base, int result_off,
+                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, cudaStream_t st);
 
 // K4: (E[b], c[b]) = offset[b] (.) root[b]; canonicalise; convert to reported units.
 //   root_e == nullptr: the network is all scalars.  root_stride 0: root is leaf-invariant.

@@ -43,7 +43,7 @@ struct LocalRun {
     for (const LocalSeg &s : lp->segs) if (s.fixed.empty()) { list_host.insert(list_host.end(), s.list_scalar.begin(), s.list_scalar.end()); n_gsc += (int)s.list_scalar.size(); }
     CUDA_TRY(h, lists.upload(list_host));
     CUDA_TRY(h, arena_e.ensure((size_t)pl.arena_variant_elems * 4));
-    CUDA_TRY(h, arena_c.ensure((size_t)pl.arena_variant_elems * 8));
+    CUDA_TRY(h, arena_c.ensure((h->P.flags & BBTN_SEARCH_ONLY) ? 0 : (size_t)pl.arena_variant_elems * 8));
     CUDA_TRY(h, off_e.ensure(4 * 4)); CUDA_TRY(h, off_c.ensure(4 * 8));
     CUDA_TRY(h, res_e.ensure(4)); CUDA_TRY(h, res_c.ensure(8)); CUDA_TRY(h, res_m.ensure(8));
     return BBTN_OK;
@@ -52,7 +52,7 @@ struct LocalRun {
   void launch_steps(const LocalSeg &s, uint32_t x, int ring) {
     const Plan &pl = lp->plan;
     int32_t *ve = (int32_t *)arena_e.p; char *vc = (char *)arena_c.p;
-    const size_t csz = ring == 0 ? 8 : 4;
+    const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
     auto pe = [&](int64_t off) { return ve + off; };
     auto pc = [&](int64_t off) { return (void *)(vc + (size_t)off * csz); };
     for (int q = s.step_begin; q < s.step_end; q++) {
@@ -67,9 +67,10 @@ struct LocalRun {
 
   int run_ring(int ring, int32_t *d_energy, uint64_t *d_count, uint32_t *d_mod) {
     const Plan &pl = lp->plan;
+    const bool first_ring = ring == RING_U64 || ring == RING_NONE;
     const int kind = P->kind;
     int32_t *ve = (int32_t *)arena_e.p; char *vc = (char *)arena_c.p;
-    const size_t csz = ring == 0 ? 8 : 4;
+    const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
     const InputRec *d_in = (const InputRec *)inputs.p;
     const int32_t *d_l = (const int32_t *)lists.p;
     int32_t *oe = (int32_t *)off_e.p; char *oc = (char *)off_c.p;
@@ -102,7 +103,7 @@ struct LocalRun {
         std::vector<char> skip(chunk, 0);
         for (uint32_t i = 0; i < chunk; i++)
           for (auto &pr : adj_pairs) if ((((x0 + i) >> pr.first) & 1u) && (((x0 + i) >> pr.second) & 1u)) { skip[i] = 1; break; }
-        if (ring == 0) for (uint32_t i = 0; i < chunk; i++) n_infeasible += skip[i];
+        if (first_ring) for (uint32_t i = 0; i < chunk; i++) n_infeasible += skip[i];
         if (have_inc && n_regions > 0) {
           // global pruning: a branch whose bound is strictly worse than the incumbent holds no optimum
           std::vector<int32_t> bound(chunk);
@@ -111,7 +112,7 @@ struct LocalRun {
           for (uint32_t i = 0; i < chunk; i++) {
             if (skip[i]) continue;
             const bool worse = kind == BBTN_ISING ? bound[i] > inc : bound[i] < inc;
-            if (bound[i] == BBTN_NEG_INF || worse) { skip[i] = 1; if (ring == 0) n_pruned++; }
+            if (bound[i] == BBTN_NEG_INF || worse) { skip[i] = 1; if (first_ring) n_pruned++; }
           }
         }
         CUDA_TRY(h, assign.ensure(rows.size()));
@@ -125,7 +126,7 @@ struct LocalRun {
                             ve + s.acc_off, vc + (size_t)s.acc_off * csz, first ? 1 : 0, ring, st);
           n_launches += 3;
           first = false;
-          if (ring == 0) n_contracted++;
+          if (first_ring) n_contracted++;
         }
         CUDA_TRY(h, cudaStreamSynchronize(st));               // `rows` is about to go out of scope
       }
@@ -165,19 +166,20 @@ void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out)
   }
 }
 
-void write_plan_stats(const LocalPlan &lp, int64_t *stats, double *work) {
+void write_plan_stats(const LocalPlan &lp, int64_t *stats, double *work, bool search) {
   if (stats) {
     std::memset(stats, 0, 10 * sizeof(int64_t));
     stats[0] = (int64_t)lp.segs.size(); stats[1] = lp.n_sliced_segs;
     stats[2] = lp.n_slices > 9e18 ? INT64_MAX : (int64_t)lp.n_slices;
-    stats[6] = lp.max_fixed; stats[7] = lp.plan.max_rank; stats[8] = lp.plan.arena_variant_elems * 12;
+    stats[6] = lp.max_fixed; stats[7] = lp.plan.max_rank; stats[8] = lp.plan.arena_variant_elems * (search ? 4 : 12);
   }
-  if (work) { work[0] = lp.fma_total; work[1] = lp.bytes_total; }
+  if (work) { work[0] = lp.fma_total; work[1] = lp.bytes_total / (search ? 3.0 : 1.0); }
 }
 
 // plan at log2_target, lowering the threshold while no candidate's arena fits the memory budget; among the
 // candidates that fit, the one that moves the fewest bytes
 int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, LocalPlan &lp, std::unique_ptr<Problem> &P_out) {
+  const int64_t per_elem = (h->P.flags & BBTN_SEARCH_ONLY) ? 4 : 12;
   std::vector<std::unique_ptr<Problem>> cands;
   candidate_trees(h, cands);
   std::string last_err; int last_rc = BBTN_ESHAPE;
@@ -187,7 +189,7 @@ int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, Loca
       LocalPlan cur; std::string err;
       int rc = make_local_plan(*cands[i], cap, cur, err);
       if (rc) { last_rc = rc; last_err = err; continue; }
-      if (budget > 0 && cur.plan.arena_variant_elems * 12 > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
+      if (budget > 0 && cur.plan.arena_variant_elems * per_elem > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
       if (best < 0 || cur.bytes_total < best_lp.bytes_total) { best = (int)i; best_lp = std::move(cur); }
     }
     if (best >= 0) { lp = std::move(best_lp); P_out = std::move(cands[best]); return BBTN_OK; }
@@ -205,7 +207,7 @@ int bbtn_local_plan_query(bbtn_handle *h, int32_t log2_target, int64_t mem_budge
   LocalPlan lp; std::unique_ptr<Problem> P;
   int rc = plan_within_budget(h, log2_target, mem_budget_bytes, lp, P);
   if (rc) return rc;
-  write_plan_stats(lp, stats, work);
+  write_plan_stats(lp, stats, work, (h->P.flags & BBTN_SEARCH_ONLY) != 0);
   return BBTN_OK;
 }
 
@@ -233,9 +235,10 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
   run.roff = region_offsets; run.rv = region_vertices; run.n_regions = n_regions;
   run.have_inc = incumbent_hint != BBTN_NEG_INF; run.inc = incumbent_hint;
   if ((rc = run.upload())) return rc;
-  const int n_rings = (crt && count_mod) ? 3 : 1;
+  const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;
+  const int n_rings = search ? 1 : ((crt && count_mod) ? 3 : 1);
   for (int ring = 0; ring < n_rings; ring++)
-    if ((rc = run.run_ring(ring, (int32_t *)run.res_e.p, (uint64_t *)run.res_c.p, (uint32_t *)run.res_m.p))) return rc;
+    if ((rc = run.run_ring(search ? (int)RING_NONE : ring, (int32_t *)run.res_e.p, (uint64_t *)run.res_c.p, (uint32_t *)run.res_m.p))) return rc;
   int32_t e; uint64_t c; uint32_t cm[2] = {0, 0};
   CUDA_TRY(h, cudaMemcpyAsync(&e, run.res_e.p, 4, cudaMemcpyDeviceToHost, run.st));
   CUDA_TRY(h, cudaMemcpyAsync(&c, run.res_c.p, 8, cudaMemcpyDeviceToHost, run.st));
@@ -243,7 +246,7 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
   CUDA_TRY(h, cudaStreamSynchronize(run.st));
   *energy = e; *count = c;
   if (count_mod) { count_mod[0] = cm[0]; count_mod[1] = cm[1]; }
-  write_plan_stats(lp, stats, work);
+  write_plan_stats(lp, stats, work, (h->P.flags & BBTN_SEARCH_ONLY) != 0);
   if (stats) { stats[3] = run.n_contracted; stats[4] = run.n_infeasible; stats[5] = run.n_pruned; stats[9] = run.n_launches; }
   return BBTN_OK;
 }

@@ -11,6 +11,7 @@ namespace bbtn {
 
 struct RingU64 {
   using T = uint64_t;
+  static constexpr bool kCounts = true;
   static __device__ __forceinline__ T mul(T a, T b) { return a * b; }
   static __device__ __forceinline__ T add(T a, T b) { return a + b; }
   static __device__ __forceinline__ T from_small(uint32_t x) { return x; }
@@ -19,6 +20,7 @@ struct RingU64 {
 template <uint32_t P>
 struct RingMod {
   using T = uint32_t;
+  static constexpr bool kCounts = true;
   // P = 2^31 - C with a small C (1 and 19 for the two primes), so 2^31 == C (mod P): fold the high part of the
   // 62-bit product down twice instead of dividing.  x = hi*2^31 + lo  ->  hi*C + lo < (C+1)*2^31  ->  < 2^31 + C*(C+1).
   static constexpr uint32_t C = 0x80000000u - P;
@@ -33,11 +35,37 @@ struct RingMod {
   static __device__ __forceinline__ T from_small(uint32_t x) { return x % P; }
 };
 
+// Search mode (PAPER.md:55 "the tropical number inf for optimization problems"; :81-91): plain max-plus, no count
+// plane at all.  The count type is an empty object; kernels reach counts only through ldc/stc below, which touch no
+// memory for this ring, so the planes may be null.
+struct NoCount {};
+struct RingNone {
+  using T = NoCount;
+  static constexpr bool kCounts = false;
+  static __device__ __forceinline__ T mul(T, T) { return T{}; }
+  static __device__ __forceinline__ T add(T, T) { return T{}; }
+  static __device__ __forceinline__ T from_small(uint32_t) { return T{}; }
+};
+
 using RingP1 = RingMod<2147483647u>;
 using RingP2 = RingMod<2147483629u>;
 
 constexpr int32_t NEG_INF = -(1 << 30);
 constexpr int32_t ZERO_BELOW = -(1 << 29);
+
+// count-plane accesses (no-ops for RingNone)
+template <class R> __device__ __forceinline__ typename R::T ldc(const typename R::T *p, int64_t i) {
+  if constexpr (R::kCounts) return p[i]; else return typename R::T{};
+}
+template <class R> __device__ __forceinline__ void stc(typename R::T *p, int64_t i, typename R::T v) {
+  if constexpr (R::kCounts) p[i] = v;
+}
+template <class R> __device__ __forceinline__ typename R::T czero() {
+  if constexpr (R::kCounts) return (typename R::T)0; else return typename R::T{};
+}
+template <class R> __device__ __forceinline__ typename R::T shfl_xor_c(typename R::T v, int d) {
+  if constexpr (R::kCounts) return __shfl_xor_sync(0xffffffffu, v, d); else return v;
+}
 
 // acc (+)= (e, c)
 template <class R>
@@ -48,15 +76,24 @@ __device__ __forceinline__ void oplus(int32_t &acc_e, typename R::T &acc_c, int3
 
 template <class R>
 __device__ __forceinline__ void canonicalise(int32_t &e, typename R::T &c) {
-  if (e < ZERO_BELOW) { e = NEG_INF; c = 0; }
+  if (e < ZERO_BELOW) { e = NEG_INF; c = czero<R>(); }
 }
 
 }  // namespace bbtn
+
+// dispatch over the three count rings only (kernels the search mode never launches: tiled GEMM, permute)
+#define BBTN_RING_DISPATCH3(ring, ...)                                  \
+  do {                                                                  \
+    if ((ring) == 0) { using R = ::bbtn::RingU64; __VA_ARGS__; }        \
+    else if ((ring) == 1) { using R = ::bbtn::RingP1; __VA_ARGS__; }    \
+    else { using R = ::bbtn::RingP2; __VA_ARGS__; }                     \
+  } while (0)
 
 // dispatch a templated launcher over the ring id
 #define BBTN_RING_DISPATCH(ring, ...)                                   \
   do {                                                                  \
     if ((ring) == 0) { using R = ::bbtn::RingU64; __VA_ARGS__; }        \
     else if ((ring) == 1) { using R = ::bbtn::RingP1; __VA_ARGS__; }    \
-    else { using R = ::bbtn::RingP2; __VA_ARGS__; }                     \
+    else if ((ring) == 2) { using R = ::bbtn::RingP2; __VA_ARGS__; }    \
+    else { using R = ::bbtn::RingNone; __VA_ARGS__; }                   \
   } while (0)

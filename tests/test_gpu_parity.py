@@ -197,7 +197,10 @@ def test_permute_structured(bb, oracle):
 
 
 # ---- whole path: K1 -> (K2) -> K3 -> K4 -----------------------------------------------
-MODES = {"auto": 0, "streaming": 0x10, "tiled": 0x20, "auto_nograph": 0x4}
+# auto / streaming run small networks as ONE launch (one CTA per leaf, tensors in shared memory); the *_nofused modes
+# keep the per-node kernels (K1, streaming K3, K4) covered on the same instances
+MODES = {"auto": 0, "streaming": 0x10, "tiled": 0x20, "auto_nograph": 0x4, "nofused": 0x80, "streaming_nofused": 0x90,
+         "nofused_nograph": 0x84}
 
 
 def _check_leaves(bb, oracle, inst, tree, fixed, assign, flags=0, sample=None):
@@ -735,6 +738,59 @@ def test_config5_kings_40x40_exact_size_and_count(bb):
     assert out["energy"] == int(g["energy"]) and out["count"] == c & MASK64, out
     assert bb.crt_combine(out["count"], *out["count_mod"]) == c
     h.close()
+
+
+# ---- ground-state SEARCH mode: plain max-plus, no count plane (BBTN_SEARCH_ONLY) ----
+@pytest.mark.parametrize("case", range(5))
+def test_search_mode_energies_match_oracle(bb, oracle, case):
+    # PAPER.md:55 ("the tropical number inf for optimization problems"), :81-91: the optimum alone.  Every leaf energy must
+    # equal the counting oracle's energy (max-plus without counts is its energy half); counts read 0
+    if case == 0:
+        inst = I.ising_lattice_2d(7, 8, 3, field_h=1)
+    elif case == 1:
+        inst = I.kings_subgraph(8, 8, 0.8, 4, weights="rand")          # weighted MIS
+    elif case == 2:
+        inst = I.ising_lattice_3d(3, 3, 4, 5)
+    elif case == 3:
+        inst = I.random_graph(22, 0.2, 7, "mis")
+    else:
+        inst = I.kings_subgraph(4, 4, 1.0, 1)                          # infeasible leaves
+    n = inst.n_vertices
+    fixed = np.array([0, 1, 5], np.int32) if case == 4 else I.random_order(n, 70 + case)[:4]
+    assign = I.all_assignments(len(fixed))
+    for tree in (None, I.elimination_tree(inst.input_index_sets(), I.natural_order(n))):
+        h = bb.Handle(inst, tree=tree, flags=bb.BBTN_SEARCH_ONLY)
+        energy, count = h.contract_batch(fixed, assign)
+        assert (count == 0).all()
+        for b in range(len(assign)):
+            we, _ = oracle.frontier_dp(inst, None, fixed, assign[b])
+            assert int(energy[b]) == (NEG_INF if we is None else we), (case, b)
+        e1, _ = h.contract_batch()
+        assert int(e1[0]) == oracle.frontier_dp(inst)[0]
+        h.close()
+
+
+def test_search_mode_drivers_and_large_kings(bb, oracle):
+    # the solve drivers in search mode: host B&B with K5 pruning, rho-driven branching, local branching
+    k = I.kings_subgraph(12, 12, 0.8, 5, weights="rand")
+    want = oracle.frontier_dp(k)[0]
+    ids = _king_ids(k, 12, 12)
+    offs, verts = _grid_regions(12, 12, 3, 3, ids)
+    branch = np.array([ids[r][6] for r in range(12) if ids[r][6] >= 0], np.int32)
+    h = bb.Handle(k, flags=bb.BBTN_SEARCH_ONLY)
+    assert h.solve_bb(branch, 3, offs, verts, max_batch=64)["energy"] == want
+    assert h.solve_branching(7)["energy"] == want
+    out = h.solve_local(9, region_offsets=offs, region_vertices=verts, incumbent_hint=want)
+    assert out["energy"] == want and out["count"] == 0 and out["sliced_stretches"] >= 1
+    with pytest.raises(bb.BbtnError):
+        bb.Handle(k, flags=bb.BBTN_SEARCH_ONLY | bb.BBTN_COUNT_CRT)
+    h.close()
+    # MIS size of the 36x36 and 40x40 King's subgraphs (goldens by the oracle's sparse DP): 4 B per element
+    for L, name in ((36, "config5-shape king 36x36 p0.8 seed 1"), (40, "config5 king 40x40 p0.8 seed 1")):
+        h = bb.Handle(I.kings_subgraph(L, L, 0.8, 1), flags=bb.BBTN_SEARCH_ONLY)
+        out = h.solve_local(32)
+        assert out["energy"] == int(_goldens()[name]["energy"]) and out["count"] == 0, out
+        h.close()
 
 
 @pytest.mark.parametrize("L", [16, 20, 24])
