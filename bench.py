@@ -457,6 +457,12 @@ def run_ours(args):
                         (8, "2iadd+imad_2op"), (9, "k3mix_2warps"), (10, "k3mix_4warps")):
         t_ms, ops = bb.int32_microbench(which, args.microbench_iters if which < 9 else max(args.microbench_iters // 16, 50))
         mb[name] = ops / (t_ms * 1e-3) / 1e9          # G lane-ops/s (which <= 8) or GFMA/s (K3 instruction mix)
+    # building blocks of the packed / 64-bit forms: clocks per warp instruction (or per round) on one SM sub-partition
+    blocks = {}
+    for which, name in ((11, "VIADDMNMX.S16x2"), (12, "HSETP2+SEL"), (13, "ISETP+SEL"), (14, "IMAD.WIDE (64-bit accumulate)"),
+                        (15, "packed pair = 2 FMAs: VIADDMNMX.S16x2 + add + HSETP2 + 2 @p IMAD")):
+        t_ms, rounds = bb.int32_microbench(which, max(args.microbench_iters // 4, 100))
+        blocks[name] = 1.0 / (rounds / 32 / (148 * 4) / (t_ms * 1e-3) / (sm_max * 1e6))
     int_peak = max(mb[k] for k in ("iadd3+imad", "iadd+imad_2op", "2iadd+imad_2op", "iadd3", "imnmx", "imad"))
     alu_peak = max(mb["iadd3"], mb["imnmx"], mb["viaddmnmx"])
     gemm_gfma = gemm_fma / (gemm_ms * 1e-3) / 1e9
@@ -478,7 +484,7 @@ def run_ours(args):
                 "gemm_gfma_per_s": gemm_gfma, "gemm_gop_per_s": 2 * gemm_gfma, "gemm_ms_per_launch": gemm_ms,
                 "frac_of_scalar_opmix_ceiling": gemm_gfma / max(mb["k3mix_2warps"], mb["k3mix_4warps"]),
                 "frac_of_alu_pipe_peak_2ops": 2 * gemm_gfma / alu_peak,
-                "microbench_Gops": mb, "share_of_step": gemm_ms * args.steps / ms,
+                "microbench_Gops": mb, "microbench_clk_per_warp_round_per_smsp": blocks, "share_of_step": gemm_ms * args.steps / ms,
                 "hbm_peak_gbs": hbm_peak, "hbm_peak_kind": peak_kind}
     # the HBM-bound kernels of the same step (rank 0's timings), against the measured copy bandwidth
     roofline_hbm = [

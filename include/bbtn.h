@@ -295,9 +295,11 @@ int bbtn_permute_batched(int32_t rank, const int32_t *perm, int64_t batch,
  * (VIADDMNMX), 3 = IMAD chain, 4 = mixed 3-operand IADD3+IMAD (both pipes), 7 / 8 = mixed two-operand
  * IADD:IMAD at 1:1 / 2:1, 9 / 10 = the instruction stream of K3's inner loop (fused add-max, add, tie
  * compare, predicated IMAD, operand LDS.128 from a broadcast table) at 2 / 4+ warps per SM sub-partition;
- * 5, 6 = earlier op-mix kernels (kept for comparison, not used by bench.py).
+ * 5, 6 = earlier op-mix kernels (kept for comparison, not used by bench.py); 11..15 = issue rates of the building
+ * blocks of the packed and 64-bit forms with operands that change every round: 11 VIADDMNMX.S16x2, 12 HSETP2 + SEL,
+ * 13 ISETP + SEL, 14 IMAD.WIDE with 64-bit accumulate, 15 the packed pair (add-max16x2, add, HSETP2, 2 predicated IMAD).
  * Runs `iters` unrolled rounds on every SM; returns elapsed milliseconds (CUDA events) and the
- * number of lane-operations (which <= 4, 7, 8) or tropical FMAs (5, 6, 9, 10) executed. */
+ * number of lane-operations (which <= 4, 7, 8), tropical FMAs (5, 6, 9, 10) or lane-rounds (11..15) executed. */
 int bbtn_int32_microbench(int32_t which, int32_t iters, double *milliseconds, double *operations,
                           void *cuda_stream);
 

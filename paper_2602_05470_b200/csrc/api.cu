@@ -549,7 +549,7 @@ int bbtn_crt_combine(uint64_t c64, uint32_t r1, uint32_t r2, uint64_t out[2]) {
 }
 
 int bbtn_int32_microbench(int32_t which, int32_t iters, double *ms, double *ops, void *stream) {
-  if (which < 0 || which > 10 || iters < 1 || !ms || !ops) return fail(nullptr, BBTN_EINVAL, "bad microbench arguments");
+  if (which < 0 || which > 15 || iters < 1 || !ms || !ops) return fail(nullptr, BBTN_EINVAL, "bad microbench arguments");
   if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device");
   int rc = run_microbench(which, iters, ms, ops, (cudaStream_t)stream);
   if (rc) return fail(nullptr, BBTN_ECUDA, "microbenchmark failed");

@@ -145,6 +145,43 @@ __global__ void __launch_bounds__(256) k3mix_kernel(int iters, int32_t seed, uin
   if (s == 0x12345678u) sink[0] = s;
 }
 
+// Issue rates of the instructions the packed and the 64-bit forms of K3 are built from, with operands that change
+// every round (nothing can be hoisted): which = 11 VIADDMNMX.S16x2, 12 HSETP2 (+ one SEL that consumes a predicate),
+// 13 ISETP (+ SEL), 14 IMAD.WIDE with a 64-bit accumulate, 15 the packed pair of gemm_pack16.cu
+// (VIADDMNMX.S16x2 + add + HSETP2 + 2 predicated IMAD = two tropical FMAs).
+template <int WHICH>
+__global__ void __launch_bounds__(512) pipe2_kernel(int iters, uint32_t seed, uint32_t *sink) {
+  uint32_t acc[8], c[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) { acc[i] = seed + threadIdx.x * (i + 1); c[i] = seed ^ i; }
+  const uint32_t k0 = seed * 7 + threadIdx.x;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int u = 0; u < 8; u++) {
+#pragma unroll
+      for (int i = 0; i < 8; i++) {
+        if (WHICH == 11) acc[i] = __viaddmax_s16x2(acc[(i + 1) & 7], k0, acc[i]);
+        else if (WHICH == 12) asm volatile("{.reg .pred p,q; setp.eq.f16x2 p|q, %0, %1; selp.u32 %0, %1, %2, p; }" : "+r"(acc[i]) : "r"(acc[(i + 1) & 7]), "r"(k0));
+        else if (WHICH == 13) asm volatile("{.reg .pred p; setp.eq.s32 p, %0, %1; selp.u32 %0, %1, %2, p; }" : "+r"(acc[i]) : "r"(acc[(i + 1) & 7]), "r"(k0));
+        else if (WHICH == 14) {
+          unsigned long long w = ((unsigned long long)c[i] << 32) | acc[i];
+          asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(w) : "r"(acc[(i + 1) & 7]), "r"(k0));
+          acc[i] = (uint32_t)w; c[i] = (uint32_t)(w >> 32);
+        } else {
+          uint32_t s;
+          acc[i] = __viaddmax_s16x2(acc[(i + 1) & 7], k0, acc[i]);
+          asm volatile("{.reg .pred p,q; add.u32 %2, %3, %4; setp.eq.f16x2 p|q, %2, %5; @p mad.lo.u32 %0, %3, %4, %0; @q mad.lo.u32 %1, %4, %4, %1;}"
+                       : "+r"(c[i]), "+r"(c[(i + 4) & 7]), "=r"(s) : "r"(acc[(i + 2) & 7]), "r"(k0), "r"(acc[i]));
+        }
+      }
+    }
+  }
+  uint32_t r = 0;
+#pragma unroll
+  for (int i = 0; i < 8; i++) r += c[i] ^ acc[i];
+  if (r == 0x12345678u) sink[0] = r;
+}
+
 }  // namespace
 
 int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t st) {
@@ -155,6 +192,7 @@ int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t s
   int grid = 148 * 8, block = 256;
   if (which == 9) { grid = 148; block = 256; }          // 2 warps per SM sub-partition, as K3 runs
   if (which == 10) { grid = 148 * 4; block = 256; }     // same mix, 4+ warps per sub-partition
+  if (which >= 11) { grid = 148 * 4; block = 512; }
   auto launch = [&](int n) {
     switch (which) {
       case 7: mix2_kernel<7><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
@@ -165,6 +203,11 @@ int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t s
       case 2: pipe_kernel<2><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
       case 3: pipe_kernel<3><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
       case 4: pipe_kernel<4><<<grid, block, 0, st>>>(n, 12345, (int32_t *)sink); break;
+      case 11: pipe2_kernel<11><<<grid, block, 0, st>>>(n, 12345u, (uint32_t *)sink); break;
+      case 12: pipe2_kernel<12><<<grid, block, 0, st>>>(n, 12345u, (uint32_t *)sink); break;
+      case 13: pipe2_kernel<13><<<grid, block, 0, st>>>(n, 12345u, (uint32_t *)sink); break;
+      case 14: pipe2_kernel<14><<<grid, block, 0, st>>>(n, 12345u, (uint32_t *)sink); break;
+      case 15: pipe2_kernel<15><<<grid, block, 0, st>>>(n, 12345u, (uint32_t *)sink); break;
       case 5: opmix_kernel<true><<<grid, block, 0, st>>>(n, 12345, (uint64_t *)sink); break;
       default: opmix_kernel<false><<<grid, block, 0, st>>>(n, 12345, (uint64_t *)sink); break;
     }
@@ -188,6 +231,8 @@ int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t s
     *ops = threads * (double)iters * 8.0 * 16.0;   // lane-instructions
   } else if (which == 9 || which == 10) {
     *ops = threads * (double)iters * 16.0 * 32.0;   // tropical FMAs (4 instructions each + 9 LDS.128 per 32)
+  } else if (which >= 11) {
+    *ops = threads * (double)iters * 64.0;          // rounds: one instruction (11, 14), one compare + SEL (12, 13), one packed pair (15)
   } else {
     *ops = threads * (double)iters * 64.0;     // tropical FMAs
   }
