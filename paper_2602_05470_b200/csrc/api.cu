@@ -139,6 +139,9 @@ int prepare_fused(bbtn_handle *h, DevPlan *dp) {
     f.offC = (int32_t)((s.vC ? 0 : pl.arena_variant_elems) + s.offC);
     for (int q = 0; q < s.rO; q++) { f.addA[q] = (uint16_t)s.addA[q]; f.addB[q] = (uint16_t)s.addB[q]; }
     for (int j = 0; j < s.nK; j++) { f.kA[j] = (uint16_t)s.kA[j]; f.kB[j] = (uint16_t)s.kB[j]; }
+    if (s.nK <= 3)
+      for (int k = 0; k < (1 << s.nK); k++)
+        for (int j = 0; j < s.nK; j++) if ((k >> j) & 1) { f.kkA[k] += (uint16_t)s.kA[j]; f.kkB[k] += (uint16_t)s.kB[j]; }
     fs.push_back(f);
   }
   std::vector<int32_t> lb;

@@ -7,7 +7,7 @@
 // (K1), walks the plan's steps in order -- C[o] = (+)_k A[fa(o) + ka(k)] (.) B[fb(o) + kb(k)], the streaming
 // form of K3 with the bit permutations folded into the addressing -- with a block barrier between steps, and
 // finalises (K4).  Leaf-invariant subtrees are recomputed by every CTA (cheaper than a second launch at this size).
-// Step descriptors are prefetched one step ahead into shared memory.
+// Step descriptors are prefetched two steps ahead (global -> register -> shared memory).
 #include "construct.cuh"
 #include "kernels.h"
 
@@ -37,11 +37,16 @@ __global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const Input
   const int t = threadIdx.x;
   constexpr int WORDS = (int)(sizeof(FusedStep) / 4);
 
-  auto prefetch = [&](int s) {                       // descriptor of step s -> desc[s & 1]
-    if (s < n_steps && t < WORDS)
-      reinterpret_cast<uint32_t *>(desc + (s & 1))[t] = reinterpret_cast<const uint32_t *>(steps + s)[t];
+  // descriptors travel global -> register -> shared memory TWO steps ahead: the word of step s+2 is requested while
+  // step s runs and is parked in shared memory at the top of step s+1, so no step ever waits for a global load
+  auto fetch = [&](int s) -> uint32_t {
+    return (s < n_steps && t < WORDS) ? __ldg(reinterpret_cast<const uint32_t *>(steps + s) + t) : 0u;
   };
-  prefetch(0);
+  auto park = [&](int s, uint32_t w) {               // descriptor word of step s -> desc[s & 1]
+    if (s < n_steps && t < WORDS) reinterpret_cast<uint32_t *>(desc + (s & 1))[t] = w;
+  };
+  park(0, fetch(0));
+  uint32_t pre = fetch(1);
 
   // ---- K1: the sliced input tensors of this leaf, and the product of its scalar inputs
   for (int i = t; i < n_build; i += FT) {
@@ -71,18 +76,33 @@ __global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const Input
   // ---- K3, step by step
   for (int s = 0; s < n_steps; s++) {
     const FusedStep &d = desc[s & 1];
-    prefetch(s + 1);
+    park(s + 1, pre);
+    pre = fetch(s + 2);
     const int rO = d.rO, nK = d.nK;
     const int32_t *ae = te + d.offA, *be = te + d.offB;
     const CT *ac = tc + d.offA, *bc = tc + d.offB;
+    // a thread's outputs are o = t + j * FT: the low 9 bits of o never change, their address part is computed once
+    // (unused table entries are 0, so the loops below need no rank tests and unroll into independent loads)
+    uint32_t a_lo = 0, b_lo = 0;
+#pragma unroll
+    for (int q = 0; q < 9; q++) { const uint32_t m = 0u - ((t >> q) & 1u); a_lo += d.addA[q] & m; b_lo += d.addB[q] & m; }
     for (int o = t; o < (1 << rO); o += FT) {
-      uint32_t a0 = 0, b0 = 0;
-      for (int q = 0; q < rO; q++) if ((o >> q) & 1) { a0 += d.addA[q]; b0 += d.addB[q]; }
+      uint32_t a0 = a_lo, b0 = b_lo;
+#pragma unroll
+      for (int q = 9; q < 13; q++) { const uint32_t m = 0u - ((o >> q) & 1u); a0 += d.addA[q] & m; b0 += d.addB[q] & m; }
       int32_t acc_e = NEG_INF; CT acc_c = czero<R>();
-      for (int k = 0; k < (1 << nK); k++) {
-        uint32_t ia = a0, ib = b0;
-        for (int j = 0; j < nK; j++) if ((k >> j) & 1) { ia += d.kA[j]; ib += d.kB[j]; }
-        oplus<R>(acc_e, acc_c, ae[ia] + be[ib], R::mul(ldc<R>(ac, ia), ldc<R>(bc, ib)));
+      if (nK <= 3) {
+#pragma unroll 4
+        for (int k = 0; k < (1 << nK); k++) {
+          const uint32_t ia = a0 + d.kkA[k], ib = b0 + d.kkB[k];
+          oplus<R>(acc_e, acc_c, ae[ia] + be[ib], R::mul(ldc<R>(ac, ia), ldc<R>(bc, ib)));
+        }
+      } else {
+        for (int k = 0; k < (1 << nK); k++) {
+          uint32_t ia = a0, ib = b0;
+          for (int j = 0; j < nK; j++) if ((k >> j) & 1) { ia += d.kA[j]; ib += d.kB[j]; }
+          oplus<R>(acc_e, acc_c, ae[ia] + be[ib], R::mul(ldc<R>(ac, ia), ldc<R>(bc, ib)));
+        }
       }
       canonicalise<R>(acc_e, acc_c);
       te[d.offC + o] = acc_e; stc<R>(tc, d.offC + o, acc_c);

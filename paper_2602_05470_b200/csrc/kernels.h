@@ -62,7 +62,8 @@ void launch_accumulate(int64_t n, const int32_t *slice_e, const void *slice_c, c
 // A step is C[o] = (+)_k A[fa(o) + ka(k)] (.) B[fb(o) + kb(k)] with shared-memory element offsets.
 struct FusedStep {
   int32_t rO, nK, offA, offB, offC, pad;
-  uint16_t addA[16], addB[16], kA[16], kB[16];
+  uint16_t addA[16], addB[16], kA[16], kB[16];   // unused entries are 0
+  uint16_t kkA[8], kkB[8];                        // nK <= 3: the summed offsets of every k, ready to add
 };
 size_t fused_tree_smem_bytes(int arena_elems, int ring);
 void launch_fused_tree(int kind, const InputRec *d_inputs, const int32_t *d_list_build, int n_build,
