@@ -209,9 +209,14 @@ int bbtn_branching_leaves(bbtn_handle *h, int32_t log2_target, int64_t mem_budge
  * given, those whose K5 bound is strictly worse than the incumbent (ties kept, reading A14).
  *   incumbent_hint  energy (reported units) of a feasible configuration known to the caller; BBTN_NEG_INF = none
  *   mem_budget_bytes  0 = 94 % of the free device memory; the threshold is lowered until the arena fits
- *   stats[0..9] = stretches, sliced stretches, branches planned (sum of 2^|F|), branches contracted, branches
- *                 infeasible, branches pruned by bound, largest |F|, largest tensor rank, arena bytes, kernel launches
- *   work[0..1]  = tropical FMAs, algorithmic bytes over all planned branches (12 B per element read or written)
+ * The branches of one stretch share one plan (one signature F): the survivors are contracted as BATCHES, as many at
+ * a time as fit the memory budget (the batch axis of K1 and K3; slices of the stored tensors are addressed per batch
+ * entry from the branch's assignment row), so a stretch with many small branches costs a few launch sequences.
+ *   stats[0..11] = stretches, sliced stretches, branches planned (sum of 2^|F|), branches contracted, branches
+ *                  infeasible, branches pruned by bound, largest |F|, largest tensor rank, arena bytes, kernel launches,
+ *                  branches in flight per launch sequence, launch sequences
+ *   work[0..3]   = tropical FMAs and algorithmic bytes over all planned branches (12 B per element read or written),
+ *                  the same two over the branches actually contracted
  * Host pointers only.  Errors: EINVAL, ESHAPE (a stretch needs more than 24 fixed variables, or the tree joins two
  * overflowing parts so that no local set exists), ENOMEM, ECUDA. */
 int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes,
@@ -221,7 +226,7 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
                      void *cuda_stream);
 
 /* The plan bbtn_solve_local would run, without running it (host only, no device): stats / work as above
- * (the run-time entries 3, 4, 5, 9 are zero).  mem_budget_bytes = 0 means no memory limit here. */
+ * (the run-time entries 3, 4, 5, 9, 10, 11 and work[2..3] are zero).  mem_budget_bytes = 0 means no memory limit here. */
 int bbtn_local_plan_query(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t *stats, double *work);
 
 /* Host-side (+) over leaf results in reported units (Eq. 3's outer sum; "the final

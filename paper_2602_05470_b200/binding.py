@@ -215,19 +215,21 @@ class Handle:
         return out
 
     _LOCAL_STATS = ("stretches", "sliced_stretches", "branches_planned", "branches_contracted", "branches_infeasible",
-                    "branches_pruned", "max_fixed", "max_rank", "arena_bytes", "kernel_launches")
+                    "branches_pruned", "max_fixed", "max_rank", "arena_bytes", "kernel_launches", "branches_in_flight",
+                    "launch_sequences")
 
     def solve_local(self, log2_target: int, mem_budget_bytes: int = 0, region_offsets=None, region_vertices=None,
                     incumbent_hint=BBTN_NEG_INF, stream=None):
         """bbtn_solve_local: BBTN on sub-networks (local fixed sets per overflowing stretch of the tree)."""
-        e = C.c_int32(); c = C.c_uint64(); cm = (C.c_uint32 * 2)(); stats = (C.c_int64 * 10)(); work = (C.c_double * 2)()
+        e = C.c_int32(); c = C.c_uint64(); cm = (C.c_uint32 * 2)(); stats = (C.c_int64 * 12)(); work = (C.c_double * 4)()
         crt = bool(self.flags & BBTN_COUNT_CRT)
         ro = None if region_offsets is None else _np(region_offsets, np.int32)
         rv = None if region_vertices is None else _np(region_vertices, np.int32)
         _check(load().bbtn_solve_local(self._h, log2_target, mem_budget_bytes, _ptr(ro), _ptr(rv), 0 if ro is None else len(ro) - 1,
                                        incumbent_hint, C.addressof(e), C.addressof(c), C.addressof(cm) if crt else None,
                                        C.addressof(stats), C.addressof(work), _stream(stream)), self._h)
-        out = {"energy": e.value, "count": c.value, "fma": work[0], "bytes": work[1]}
+        out = {"energy": e.value, "count": c.value, "fma": work[0], "bytes": work[1], "fma_contracted": work[2],
+               "bytes_contracted": work[3]}
         out.update({k: stats[i] for i, k in enumerate(self._LOCAL_STATS)})
         if crt:
             out["count_mod"] = (cm[0], cm[1])
@@ -235,7 +237,7 @@ class Handle:
 
     def local_plan_query(self, log2_target: int, mem_budget_bytes: int = 0) -> dict:
         """bbtn_local_plan_query (host only)."""
-        stats = (C.c_int64 * 10)(); work = (C.c_double * 2)()
+        stats = (C.c_int64 * 12)(); work = (C.c_double * 4)()
         _check(load().bbtn_local_plan_query(self._h, log2_target, mem_budget_bytes, C.addressof(stats), C.addressof(work)), self._h)
         out = {"fma": work[0], "bytes": work[1]}
         out.update({k: stats[i] for i, k in enumerate(self._LOCAL_STATS)})

@@ -28,6 +28,8 @@ struct AbsorbVecArgs {
   uint32_t addA[32], addB[32];    // per output bit
   uint32_t kA[8], kB[8];          // per summed bit
   int64_t sA, sB, sC, n_tiles;    // batch strides (elements), tiles over all batch entries
+  const uint8_t *xs; int nF;      // local slicing: rows [nb][nF] of 0/1 and the strides of the fixed indices
+  uint32_t sliceA[24], sliceB[24];
 };
 
 template <class CT> struct V4;
@@ -96,8 +98,13 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
     const uint32_t hi = (uint32_t)(t - (b << tiles_per_entry_lg));
     uint32_t a_hi = 0, b_hi = 0;
     for (int q = 0; q < tiles_per_entry_lg; q++) if ((hi >> q) & 1u) { a_hi += p.addA[p.tb + q]; b_hi += p.addB[p.tb + q]; }
-    const int32_t *ae = Ae + b * p.sA + a_hi; const CT *ac = Ac + b * p.sA + a_hi;
-    const int32_t *be = Be + b * p.sB + b_hi; const CT *bc = Bc + b * p.sB + b_hi;
+    int64_t oA = b * p.sA + a_hi, oB = b * p.sB + b_hi;
+    if (p.nF) {
+      const uint8_t *x = p.xs + b * p.nF;
+      for (int j = 0; j < p.nF; j++) if (x[j]) { oA += p.sliceA[j]; oB += p.sliceB[j]; }
+    }
+    const int32_t *ae = Ae + oA; const CT *ac = Ac + oA;
+    const int32_t *be = Be + oB; const CT *bc = Bc + oB;
     int32_t *ce = Ce + b * p.sC + ((int64_t)hi << p.tb); CT *cc = Cc + b * p.sC + ((int64_t)hi << p.tb);
 #pragma unroll
     for (int j = 0; j < VPT; j++) {
@@ -191,8 +198,9 @@ inline bool al32(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 31) =
 
 // Returns false when the step does not fit the vectorised form (the caller then runs the scalar kernel).
 bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
-                       int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
+                       int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs) {
   if (s.rO < 4 || s.nK > 3 || s.rA < 3) return false;
+  if (xs) for (int j = 0; j < s.n_slice; j++) if (s.sliceA[j] & 3u) return false;   // a slice would break the 16-byte reads of A
   if (!al16(Ae) || !al16(Ce) || (ring != RING_NONE && (!al16(Ac) || !al16(Cc)))) return false;
   if (ring == RING_U64 && (!al32(Ac) || !al32(Cc))) return false;       // 32-byte count vectors
   int lp;
@@ -216,9 +224,11 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
   }
   // the 16-byte reads of A must stay 4-element aligned: every offset that can be added is a multiple of 4
   for (int q = 2; q < s.rO; q++) if (p.addA[q] & 3u) return false;
-  p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
-  p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
+  p.sA = (s.vA && !s.xA) ? ((int64_t)1 << s.rA) : 0;
+  p.sB = (s.vB && !s.xB) ? ((int64_t)1 << s.rB) : 0;
   p.sC = (int64_t)1 << s.rO;
+  p.xs = xs; p.nF = xs ? s.n_slice : 0;
+  for (int j = 0; j < 24; j++) { p.sliceA[j] = s.sliceA[j]; p.sliceB[j] = s.sliceB[j]; }
   p.n_tiles = nb << (rOe - p.tb);
   const int64_t cap = 148 * 8;
   const int grid = (int)(p.n_tiles < cap ? p.n_tiles : cap);

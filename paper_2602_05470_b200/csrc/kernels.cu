@@ -58,7 +58,19 @@ struct AbsorbArgs {
   int rO, nK;
   uint32_t addA[32], addB[32], kA[32], kB[32];
   int64_t sA, sB, sC, total;
+  const uint8_t *xs; int nF;               // local slicing: rows [nb][nF] of 0/1 and the strides of the fixed indices
+  uint32_t sliceA[24], sliceB[24];
 };
+
+// element offset of batch entry b's operands: b * stride, plus the strides of the locally fixed indices that are set
+template <class ARGS>
+__device__ __forceinline__ void batch_offsets(const ARGS &p, int64_t b, int64_t &oA, int64_t &oB) {
+  oA = b * p.sA; oB = b * p.sB;
+  if (p.nF) {
+    const uint8_t *x = p.xs + b * p.nF;
+    for (int j = 0; j < p.nF; j++) if (x[j]) { oA += p.sliceA[j]; oB += p.sliceB[j]; }
+  }
+}
 
 template <class R>
 __global__ void absorb_kernel(AbsorbArgs p, const int32_t *__restrict__ Ae, const typename R::T *__restrict__ Ac,
@@ -70,8 +82,10 @@ __global__ void absorb_kernel(AbsorbArgs p, const int32_t *__restrict__ Ae, cons
     const uint32_t o = (uint32_t)(t & omask);
     uint32_t a0 = 0, b0 = 0;
     for (int q = 0; q < p.rO; q++) if ((o >> q) & 1u) { a0 += p.addA[q]; b0 += p.addB[q]; }
-    const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
-    const int32_t *be = Be + b * p.sB; const typename R::T *bc = Bc + b * p.sB;
+    int64_t oA, oB;
+    batch_offsets(p, b, oA, oB);
+    const int32_t *ae = Ae + oA; const typename R::T *ac = Ac + oA;
+    const int32_t *be = Be + oB; const typename R::T *bc = Bc + oB;
     int32_t acc_e = NEG_INF; typename R::T acc_c = czero<R>();
     for (uint64_t k = 0; k < (1ull << p.nK); k++) {        // nK may be 32
       uint32_t ia = a0, ib = b0;
@@ -91,6 +105,8 @@ struct ReduceArgs {
   int rO, nK;
   uint32_t addA[32], addB[32], kA[32], kB[32];
   int64_t sA, sB, sC;
+  const uint8_t *xs; int nF;
+  uint32_t sliceA[24], sliceB[24];
 };
 
 template <class R>
@@ -104,8 +120,10 @@ __global__ void reduce_kernel(ReduceArgs p, const int32_t *__restrict__ Ae, cons
   const uint32_t o = (uint32_t)t & ((1u << p.rO) - 1u);
   uint32_t a0 = 0, b0 = 0;
   for (int q = 0; q < p.rO; q++) if ((o >> q) & 1u) { a0 += p.addA[q]; b0 += p.addB[q]; }
-  const int32_t *ae = Ae + b * p.sA; const typename R::T *ac = Ac + b * p.sA;
-  const int32_t *be = Be + b * p.sB; const typename R::T *bc = Bc + b * p.sB;
+  int64_t oA, oB;
+  batch_offsets(p, b, oA, oB);
+  const int32_t *ae = Ae + oA; const typename R::T *ac = Ac + oA;
+  const int32_t *be = Be + oB; const typename R::T *bc = Bc + oB;
   int32_t acc_e = NEG_INF; typename R::T acc_c = czero<R>();
   for (uint64_t k = threadIdx.x; k < (1ull << p.nK); k += blockDim.x) {      // nK may be 32
     uint32_t ia = a0, ib = b0;
@@ -164,19 +182,21 @@ __global__ void finalize_kernel(int kind, int64_t B, const int32_t *__restrict__
   }
 }
 
-// acc (+)= offset (.) slice   (local slicing: the (+) over the slices of a segment)
+// acc (+)= (+)_b offset[b] (.) slice[b]   (local slicing: the (+) over the slices of a segment)
 template <class R>
-__global__ void accumulate_kernel(int64_t n, const int32_t *__restrict__ slice_e, const typename R::T *__restrict__ slice_c,
+__global__ void accumulate_kernel(int64_t n, int64_t nb, const int32_t *__restrict__ slice_e, const typename R::T *__restrict__ slice_c,
                                   const int32_t *__restrict__ off_e, const typename R::T *__restrict__ off_c,
                                   int32_t *__restrict__ acc_e, typename R::T *__restrict__ acc_c, int first) {
-  int32_t oe = 0; typename R::T oc = R::from_small(1);
-  if (slice_e) { oe = off_e[0]; oc = ldc<R>(off_c, 0); }
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     int32_t e = NEG_INF; typename R::T c = czero<R>();
     if (slice_e) {
-      e = slice_e[i] + oe; c = R::mul(ldc<R>(slice_c, i), oc);
+      if (!first) { e = acc_e[i]; c = ldc<R>(acc_c, i); }
+      for (int64_t b = 0; b < nb; b++) {
+        int32_t se = slice_e[b * n + i] + off_e[b]; typename R::T sc = R::mul(ldc<R>(slice_c, b * n + i), ldc<R>(off_c, b));
+        canonicalise<R>(se, sc);
+        oplus<R>(e, c, se, sc);
+      }
       canonicalise<R>(e, c);
-      if (!first) { int32_t ae = acc_e[i]; typename R::T ac = ldc<R>(acc_c, i); oplus<R>(ae, ac, e, c); e = ae; c = ac; }
     }
     acc_e[i] = e; stc<R>(acc_c, i, c);
   }
@@ -209,13 +229,15 @@ void launch_construct(int kind, const InputRec *d_inputs, const int32_t *d_list_
 }
 
 void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
-                   int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
-  if (launch_absorb_vec(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st)) return;   // 16-byte form (absorb_vec.cu)
+                   int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs) {
+  if (launch_absorb_vec(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st, xs)) return;   // 16-byte form (absorb_vec.cu)
   AbsorbArgs p;
   p.rO = s.rO; p.nK = s.nK;
   for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
-  p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
-  p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
+  p.sA = (s.vA && !s.xA) ? ((int64_t)1 << s.rA) : 0;
+  p.sB = (s.vB && !s.xB) ? ((int64_t)1 << s.rB) : 0;
+  p.xs = xs; p.nF = xs ? s.n_slice : 0;
+  for (int j = 0; j < 24; j++) { p.sliceA[j] = s.sliceA[j]; p.sliceB[j] = s.sliceB[j]; }
   p.sC = (int64_t)1 << s.rO;
   p.total = nb << s.rO;
   BBTN_RING_DISPATCH(ring, {
@@ -225,12 +247,14 @@ void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
 }
 
 void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
-                   int32_t *Ce, void *Cc, int ring, cudaStream_t st) {
+                   int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs) {
   ReduceArgs p;
   p.rO = s.rO; p.nK = s.nK;
   for (int i = 0; i < 32; i++) { p.addA[i] = s.addA[i]; p.addB[i] = s.addB[i]; p.kA[i] = s.kA[i]; p.kB[i] = s.kB[i]; }
-  p.sA = s.vA ? ((int64_t)1 << s.rA) : 0;
-  p.sB = s.vB ? ((int64_t)1 << s.rB) : 0;
+  p.sA = (s.vA && !s.xA) ? ((int64_t)1 << s.rA) : 0;
+  p.sB = (s.vB && !s.xB) ? ((int64_t)1 << s.rB) : 0;
+  p.xs = xs; p.nF = xs ? s.n_slice : 0;
+  for (int j = 0; j < 24; j++) { p.sliceA[j] = s.sliceA[j]; p.sliceB[j] = s.sliceB[j]; }
   p.sC = (int64_t)1 << s.rO;
   const int64_t total = nb << s.rO;
   BBTN_RING_DISPATCH(ring, {
@@ -239,11 +263,11 @@ void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac,
   });
 }
 
-void launch_accumulate(int64_t n, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
+void launch_accumulate(int64_t n, int64_t nb, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
                        int32_t *acc_e, void *acc_c, int first, int ring, cudaStream_t st) {
   BBTN_RING_DISPATCH(ring, {
     using CT = typename R::T;
-    accumulate_kernel<R><<<grid_for(n, 256), 256, 0, st>>>(n, slice_e, (const CT *)slice_c, off_e, (const CT *)off_c, acc_e,
+    accumulate_kernel<R><<<grid_for(n, 256), 256, 0, st>>>(n, nb, slice_e, (const CT *)slice_c, off_e, (const CT *)off_c, acc_e,
                                                            (CT *)acc_c, first);
   });
 }

@@ -26,12 +26,14 @@ void launch_permute(int rank, const int32_t *perm, int64_t batch, const int32_t 
                     int32_t *dst_e, void *dst_c, int ring, cudaStream_t st);
 
 // K3 (streaming form, permutation fused into the operand addressing) and its long-reduction form.
+//   xs (local slicing, Step::n_slice > 0): device rows [nb][n_slice] of 0/1; an operand that is a view of a stored tensor
+//   (Step::xA / xB) starts, for batch entry b, at its base + sum_j xs[b][j] * sliceA/B[j] instead of base + b * stride.
 void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
-                   int32_t *Ce, void *Cc, int ring, cudaStream_t st);
+                   int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);
 bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
-                       int32_t *Ce, void *Cc, int ring, cudaStream_t st);   // false: shape not covered, use launch_absorb's scalar kernel
+                       int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);   // false: shape not covered, use launch_absorb's scalar kernel
 void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
-                   int32_t *Ce, void *Cc, int ring, cudaStream_t st);
+                   int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);
 
 // K3 (register/shared-memory tiled form).  C[b,g,m,n] = (+)_k A (.) B.
 //   a_kmajor = 1: A is [g][k][m] (m fastest, the engine's canonical order); 0: A is row-major [m][k].
@@ -52,10 +54,10 @@ void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kma
                         const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
                         int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, cudaStream_t st);
 
-// Local slicing: acc (+)= offset (.) slice, element-wise over n elements (first = 1: acc = offset (.) slice); the
-// zero tensor when slice_e == nullptr.  offset is one element on the device.  (+) over the assignments of a segment's
-// locally fixed indices (Eq. 3, on a sub-network; plan.h "local slicing").
-void launch_accumulate(int64_t n, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
+// Local slicing: acc (+)= (+)_b offset[b] (.) slice[b], element-wise over n elements, nb slices stored [nb][n]
+// (first = 1: acc is overwritten); the zero tensor when slice_e == nullptr.  offset[b] is one element per slice on the
+// device.  (+) over the assignments of a segment's locally fixed indices (Eq. 3, on a sub-network).
+void launch_accumulate(int64_t n, int64_t nb, const int32_t *slice_e, const void *slice_c, const int32_t *off_e, const void *off_c,
                        int32_t *acc_e, void *acc_c, int first, int ring, cudaStream_t st);
 
 // K1..K4 of a small network in ONE launch (fused_tree.cu): one CTA per leaf, every tensor in shared memory.

@@ -23,44 +23,58 @@ namespace {
 
 struct LocalRun {
   bbtn_handle *h; const Problem *P; LocalPlan *lp; cudaStream_t st;
-  DevBuf inputs, lists, assign, arena_e, arena_c, off_e, off_c, res_e, res_c, res_m;
-  std::vector<int32_t> list_host; std::vector<int64_t> var_at, sc_at;   // per segment: position of its lists in `lists`
-  int64_t gsc_at = 0; int n_gsc = 0;                                    // scalars of the run-once segments, all together
-  int64_t n_contracted = 0, n_infeasible = 0, n_pruned = 0, n_launches = 0;
+  int64_t nb_max = 1;                                                    // branches of one stretch contracted per launch sequence
+  DevBuf inputs, lists, assign, inv_e, inv_c, var_e, var_c, off_e, off_c, res_e, res_c, res_m;
+  std::vector<int32_t> list_host;
+  std::vector<int64_t> var_at, inv_at, sc_at;                            // per segment: position of its lists in `lists`
+  int64_t gsc_at = 0; int n_gsc = 0;                                     // scalars of the run-once segments, all together
+  int64_t n_contracted = 0, n_infeasible = 0, n_pruned = 0, n_launches = 0, n_sequences = 0;
+  double fma_done = 0, bytes_done = 0;
   // pruning inputs
   const int32_t *roff = nullptr, *rv = nullptr; int n_regions = 0; bool have_inc = false; int32_t inc = 0;
 
   int upload() {
     const Plan &pl = lp->plan;
+    const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;
     CUDA_TRY(h, inputs.ensure(pl.inputs.size() * sizeof(InputRec)));
     CUDA_TRY(h, cudaMemcpy(inputs.p, pl.inputs.data(), pl.inputs.size() * sizeof(InputRec), cudaMemcpyHostToDevice));
     for (const LocalSeg &s : lp->segs) {
       var_at.push_back((int64_t)list_host.size()); list_host.insert(list_host.end(), s.list_var.begin(), s.list_var.end());
+      inv_at.push_back((int64_t)list_host.size()); list_host.insert(list_host.end(), s.list_inv.begin(), s.list_inv.end());
       sc_at.push_back((int64_t)list_host.size());
       if (!s.fixed.empty()) list_host.insert(list_host.end(), s.list_scalar.begin(), s.list_scalar.end());
     }
     gsc_at = (int64_t)list_host.size();
     for (const LocalSeg &s : lp->segs) if (s.fixed.empty()) { list_host.insert(list_host.end(), s.list_scalar.begin(), s.list_scalar.end()); n_gsc += (int)s.list_scalar.size(); }
     CUDA_TRY(h, lists.upload(list_host));
-    CUDA_TRY(h, arena_e.ensure((size_t)pl.arena_variant_elems * 4));
-    CUDA_TRY(h, arena_c.ensure((h->P.flags & BBTN_SEARCH_ONLY) ? 0 : (size_t)pl.arena_variant_elems * 8));
-    CUDA_TRY(h, off_e.ensure(4 * 4)); CUDA_TRY(h, off_c.ensure(4 * 8));
+    CUDA_TRY(h, inv_e.ensure((size_t)pl.arena_invariant_elems * 4));
+    CUDA_TRY(h, inv_c.ensure(search ? 0 : (size_t)pl.arena_invariant_elems * 8));
+    CUDA_TRY(h, var_e.ensure((size_t)pl.arena_variant_elems * (size_t)nb_max * 4));
+    CUDA_TRY(h, var_c.ensure(search ? 0 : (size_t)pl.arena_variant_elems * (size_t)nb_max * 8));
+    CUDA_TRY(h, off_e.ensure((size_t)(nb_max + 2) * 4)); CUDA_TRY(h, off_c.ensure((size_t)(nb_max + 2) * 8));
     CUDA_TRY(h, res_e.ensure(4)); CUDA_TRY(h, res_c.ensure(8)); CUDA_TRY(h, res_m.ensure(8));
     return BBTN_OK;
   }
 
-  void launch_steps(const LocalSeg &s, uint32_t x, int ring) {
+  // the steps of one segment for nb branches at once; xs = their assignment rows [nb][|F|] on the device
+  void launch_steps(const LocalSeg &s, int64_t nb, const uint8_t *xs, int ring) {
     const Plan &pl = lp->plan;
-    int32_t *ve = (int32_t *)arena_e.p; char *vc = (char *)arena_c.p;
+    int32_t *ve = (int32_t *)var_e.p, *ie = (int32_t *)inv_e.p;
+    char *vc = (char *)var_c.p, *ic = (char *)inv_c.p;
     const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
-    auto pe = [&](int64_t off) { return ve + off; };
-    auto pc = [&](int64_t off) { return (void *)(vc + (size_t)off * csz); };
+    // a view (x) and an invariant tensor live in the invariant arena; a variant tensor is [nb][2^rank] at off * nb
+    auto pe = [&](int v, int x, int64_t off) { return (v && !x) ? ve + off * nb : ie + off; };
+    auto pc = [&](int v, int x, int64_t off) { return (void *)((v && !x) ? vc + (size_t)off * nb * csz : ic + (size_t)off * csz); };
     for (int q = s.step_begin; q < s.step_end; q++) {
       const Step &sp = pl.steps[q];
-      int64_t oa = sp.offA, ob = sp.offB;
-      for (int j = 0; j < sp.n_slice; j++) if ((x >> j) & 1u) { oa += sp.sliceA[j]; ob += sp.sliceB[j]; }
-      if (sp.kind == STEP_ABSORB) launch_absorb(sp, 1, pe(oa), pc(oa), pe(ob), pc(ob), pe(sp.offC), pc(sp.offC), ring, st);
-      else launch_reduce(sp, 1, pe(oa), pc(oa), pe(ob), pc(ob), pe(sp.offC), pc(sp.offC), ring, st);
+      const int64_t n = sp.variant ? nb : 1;
+      const uint8_t *x = (sp.n_slice && (sp.xA || sp.xB)) ? xs : nullptr;
+      if (sp.kind == STEP_ABSORB)
+        launch_absorb(sp, n, pe(sp.vA, sp.xA, sp.offA), pc(sp.vA, sp.xA, sp.offA), pe(sp.vB, sp.xB, sp.offB), pc(sp.vB, sp.xB, sp.offB),
+                      pe(sp.vC, 0, sp.offC), pc(sp.vC, 0, sp.offC), ring, st, x);
+      else
+        launch_reduce(sp, n, pe(sp.vA, sp.xA, sp.offA), pc(sp.vA, sp.xA, sp.offA), pe(sp.vB, sp.xB, sp.offB), pc(sp.vB, sp.xB, sp.offB),
+                      pe(sp.vC, 0, sp.offC), pc(sp.vC, 0, sp.offC), ring, st, x);
       n_launches++;
     }
   }
@@ -69,25 +83,27 @@ struct LocalRun {
     const Plan &pl = lp->plan;
     const bool first_ring = ring == RING_U64 || ring == RING_NONE;
     const int kind = P->kind;
-    int32_t *ve = (int32_t *)arena_e.p; char *vc = (char *)arena_c.p;
+    int32_t *ve = (int32_t *)var_e.p, *ie = (int32_t *)inv_e.p;
+    char *vc = (char *)var_c.p, *ic = (char *)inv_c.p;
     const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
     const InputRec *d_in = (const InputRec *)inputs.p;
     const int32_t *d_l = (const int32_t *)lists.p;
     int32_t *oe = (int32_t *)off_e.p; char *oc = (char *)off_c.p;
-    // slot 0: (.) of the scalar inputs of the run-once segments; slot 1: of the current slice; slot 2: scratch
-    launch_construct(kind, d_in, nullptr, 0, nullptr, 0, d_l + gsc_at, n_gsc, nullptr, 0, 1, ve, vc, nullptr, nullptr, oe, oc, ring, st);
+    // slot 0: (.) of the scalar inputs of the run-once segments; slot 1: scratch; slots 2 ..: one per branch in flight
+    launch_construct(kind, d_in, nullptr, 0, nullptr, 0, d_l + gsc_at, n_gsc, nullptr, 0, 1, ve, vc, ie, ic, oe, oc, ring, st);
     n_launches++;
     for (size_t si = 0; si < lp->segs.size(); si++) {
       const LocalSeg &s = lp->segs[si];
       const int f = (int)s.fixed.size();
       if (f == 0) {
-        launch_construct(kind, d_in, d_l + var_at[si], (int)s.list_var.size(), nullptr, 0, nullptr, 0, nullptr, 0, 1, ve, vc,
-                         nullptr, nullptr, oe + 2, oc + 2 * csz, ring, st);
+        launch_construct(kind, d_in, nullptr, 0, d_l + inv_at[si], (int)s.list_inv.size(), nullptr, 0, nullptr, 0, 1, ve, vc, ie, ic,
+                         oe + 1, oc + csz, ring, st);
         n_launches += 2;
-        launch_steps(s, 0, ring);
+        launch_steps(s, 1, nullptr, ring);
+        if (first_ring) { fma_done += s.fma; bytes_done += s.bytes; n_sequences++; }
         continue;
       }
-      // ---- a sliced segment: enumerate the assignments of F, prune, contract, (+)-accumulate
+      // ---- a sliced segment: enumerate the assignments of F, prune, contract the survivors in batches, (+)-accumulate
       std::vector<std::pair<int, int>> adj_pairs;            // MIS: positions in F of adjacent fixed vertices
       if (kind == BBTN_MIS) {
         std::vector<int> posF(P->n, -1);
@@ -97,6 +113,29 @@ struct LocalRun {
       const uint32_t n_x = 1u << f;
       const uint32_t chunk = std::min<uint32_t>(n_x, 1u << 14);
       bool first = true;
+      std::vector<uint8_t> live;                              // rows of the branches that survived pruning, not yet contracted
+      auto flush = [&](bool all) -> int {                     // contract the survivors, nb_max at a time
+        const int64_t n_live = (int64_t)live.size() / f;
+        int64_t done = 0;
+        while (n_live - done >= (all ? 1 : nb_max)) {
+          const int64_t nb = std::min<int64_t>(nb_max, n_live - done);
+          CUDA_TRY(h, assign.ensure((size_t)nb_max * f));
+          CUDA_TRY(h, cudaMemcpyAsync(assign.p, live.data() + (size_t)done * f, (size_t)nb * f, cudaMemcpyHostToDevice, st));
+          const uint8_t *xs = (const uint8_t *)assign.p;
+          launch_construct(kind, d_in, d_l + var_at[si], (int)s.list_var.size(), d_l + inv_at[si], (int)s.list_inv.size(),
+                           d_l + sc_at[si], (int)s.list_scalar.size(), xs, f, nb, ve, vc, ie, ic, oe + 2, oc + 2 * csz, ring, st);
+          launch_steps(s, nb, xs, ring);
+          launch_accumulate((int64_t)1 << s.acc_rank, nb, ve + s.tmp_off * nb, vc + (size_t)s.tmp_off * nb * csz, oe + 2, oc + 2 * csz,
+                            ie + s.acc_off, ic + (size_t)s.acc_off * csz, first ? 1 : 0, ring, st);
+          CUDA_TRY(h, cudaStreamSynchronize(st));             // the staging rows are reused by the next batch
+          n_launches += 4;
+          first = false;
+          done += nb;
+          if (first_ring) { n_contracted += nb; n_sequences++; fma_done += (double)nb * s.fma; bytes_done += (double)nb * s.bytes; }
+        }
+        live.erase(live.begin(), live.begin() + (size_t)done * f);
+        return BBTN_OK;
+      };
       for (uint32_t x0 = 0; x0 < n_x; x0 += chunk) {
         std::vector<uint8_t> rows((size_t)chunk * f);
         for (uint32_t i = 0; i < chunk; i++) for (int j = 0; j < f; j++) rows[(size_t)i * f + j] = (uint8_t)(((x0 + i) >> j) & 1u);
@@ -115,28 +154,18 @@ struct LocalRun {
             if (bound[i] == BBTN_NEG_INF || worse) { skip[i] = 1; if (first_ring) n_pruned++; }
           }
         }
-        CUDA_TRY(h, assign.ensure(rows.size()));
-        CUDA_TRY(h, cudaMemcpyAsync(assign.p, rows.data(), rows.size(), cudaMemcpyHostToDevice, st));
-        for (uint32_t i = 0; i < chunk; i++) {
-          if (skip[i]) continue;
-          launch_construct(kind, d_in, d_l + var_at[si], (int)s.list_var.size(), nullptr, 0, d_l + sc_at[si], (int)s.list_scalar.size(),
-                           (const uint8_t *)assign.p + (size_t)i * f, f, 1, ve, vc, nullptr, nullptr, oe + 1, oc + csz, ring, st);
-          launch_steps(s, x0 + i, ring);
-          launch_accumulate((int64_t)1 << s.acc_rank, ve + s.tmp_off, vc + (size_t)s.tmp_off * csz, oe + 1, oc + csz,
-                            ve + s.acc_off, vc + (size_t)s.acc_off * csz, first ? 1 : 0, ring, st);
-          n_launches += 3;
-          first = false;
-          if (first_ring) n_contracted++;
-        }
-        CUDA_TRY(h, cudaStreamSynchronize(st));               // `rows` is about to go out of scope
+        for (uint32_t i = 0; i < chunk; i++)
+          if (!skip[i]) live.insert(live.end(), rows.begin() + (size_t)i * f, rows.begin() + (size_t)(i + 1) * f);
+        int rc = flush(x0 + chunk >= n_x);
+        if (rc) return rc;
       }
       if (first) {                                            // every branch pruned: the boundary tensor is the zero tensor
-        launch_accumulate((int64_t)1 << s.acc_rank, nullptr, nullptr, nullptr, nullptr, ve + s.acc_off, vc + (size_t)s.acc_off * csz, 1, ring, st);
+        launch_accumulate((int64_t)1 << s.acc_rank, 0, nullptr, nullptr, nullptr, nullptr, ie + s.acc_off, ic + (size_t)s.acc_off * csz, 1, ring, st);
         n_launches++;
       }
     }
     const bool has_root = pl.result_offset >= 0;
-    launch_finalize(kind, 1, has_root ? ve + pl.result_offset : nullptr, has_root ? vc + (size_t)pl.result_offset * csz : nullptr, 0,
+    launch_finalize(kind, 1, has_root ? ie + pl.result_offset : nullptr, has_root ? ic + (size_t)pl.result_offset * csz : nullptr, 0,
                     oe, oc, d_energy, d_count, d_mod, ring, st);
     n_launches++;
     CUDA_TRY(h, cudaGetLastError());
@@ -168,12 +197,13 @@ void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out)
 
 void write_plan_stats(const LocalPlan &lp, int64_t *stats, double *work, bool search) {
   if (stats) {
-    std::memset(stats, 0, 10 * sizeof(int64_t));
+    std::memset(stats, 0, 12 * sizeof(int64_t));
     stats[0] = (int64_t)lp.segs.size(); stats[1] = lp.n_sliced_segs;
     stats[2] = lp.n_slices > 9e18 ? INT64_MAX : (int64_t)lp.n_slices;
-    stats[6] = lp.max_fixed; stats[7] = lp.plan.max_rank; stats[8] = lp.plan.arena_variant_elems * (search ? 4 : 12);
+    stats[6] = lp.max_fixed; stats[7] = lp.plan.max_rank;
+    stats[8] = (lp.plan.arena_invariant_elems + lp.plan.arena_variant_elems) * (search ? 4 : 12);      // with one branch in flight
   }
-  if (work) { work[0] = lp.fma_total; work[1] = lp.bytes_total / (search ? 3.0 : 1.0); }
+  if (work) { work[0] = lp.fma_total; work[1] = lp.bytes_total / (search ? 3.0 : 1.0); work[2] = work[3] = 0; }
 }
 
 // plan at log2_target, lowering the threshold while no candidate's arena fits the memory budget; among the
@@ -189,7 +219,7 @@ int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, Loca
       LocalPlan cur; std::string err;
       int rc = make_local_plan(*cands[i], cap, cur, err);
       if (rc) { last_rc = rc; last_err = err; continue; }
-      if (budget > 0 && cur.plan.arena_variant_elems * per_elem > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
+      if (budget > 0 && (cur.plan.arena_invariant_elems + cur.plan.arena_variant_elems) * per_elem > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
       if (best < 0 || cur.bytes_total < best_lp.bytes_total) { best = (int)i; best_lp = std::move(cur); }
     }
     if (best >= 0) { lp = std::move(best_lp); P_out = std::move(cands[best]); return BBTN_OK; }
@@ -232,6 +262,15 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
   if (rc) return rc;
   const Problem *P = Pt.get();
   LocalRun run{h, P, &lp, (cudaStream_t)stream};
+  {
+    // branches of a stretch that are small are contracted many at a time (the batch axis of the kernels): as many as fit
+    // the budget next to the invariant arena, at most 1024 and never more than the largest stretch has
+    const int64_t per_elem = (h->P.flags & BBTN_SEARCH_ONLY) ? 4 : 12;
+    const int64_t inv_b = lp.plan.arena_invariant_elems * per_elem, var_b = std::max<int64_t>(lp.plan.arena_variant_elems * per_elem, 1);
+    int64_t most = 1;
+    for (const LocalSeg &sg : lp.segs) most = std::max<int64_t>(most, (int64_t)1 << std::min<size_t>(sg.fixed.size(), 20));
+    run.nb_max = std::max<int64_t>(1, std::min<int64_t>({(mem_budget_bytes - inv_b) / var_b, (int64_t)1024, most}));
+  }
   run.roff = region_offsets; run.rv = region_vertices; run.n_regions = n_regions;
   run.have_inc = incumbent_hint != BBTN_NEG_INF; run.inc = incumbent_hint;
   if ((rc = run.upload())) return rc;
@@ -247,7 +286,12 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
   *energy = e; *count = c;
   if (count_mod) { count_mod[0] = cm[0]; count_mod[1] = cm[1]; }
   write_plan_stats(lp, stats, work, (h->P.flags & BBTN_SEARCH_ONLY) != 0);
-  if (stats) { stats[3] = run.n_contracted; stats[4] = run.n_infeasible; stats[5] = run.n_pruned; stats[9] = run.n_launches; }
+  if (stats) {
+    stats[3] = run.n_contracted; stats[4] = run.n_infeasible; stats[5] = run.n_pruned; stats[9] = run.n_launches;
+    stats[8] = (lp.plan.arena_invariant_elems + lp.plan.arena_variant_elems * run.nb_max) * (((h->P.flags & BBTN_SEARCH_ONLY) != 0) ? 4 : 12);
+    stats[10] = run.nb_max; stats[11] = run.n_sequences;
+  }
+  if (work) { work[2] = run.fma_done; work[3] = run.bytes_done / (((h->P.flags & BBTN_SEARCH_ONLY) != 0) ? 3.0 : 1.0); }
   return BBTN_OK;
 }
 

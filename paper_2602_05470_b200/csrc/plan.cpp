@@ -281,7 +281,8 @@ struct Planner {
   std::vector<char> used;
   std::vector<int32_t> tl, tr;
   // local planning: operands that must outlive the step (they are read again by the next slice)
-  std::vector<std::pair<int64_t, int64_t>> deferred;   // (offset, elements) in the variant arena
+  struct Deferred { bool variant; int64_t off, ne; };
+  std::vector<Deferred> deferred;                      // storage to give back when the sliced segment ends
 
   Planner(const Problem &P_, int force_mode_, bool enforce_cap_, bool single_arena_, bool want_labels_, Plan &out_, std::string &err_)
       : P(P_), n(P_.n), m(P_.m), n_in(P_.n + P_.m), force_mode(force_mode_), enforce_cap(enforce_cap_),
@@ -320,7 +321,7 @@ struct Planner {
   void release(TRef &x) {
     if (x.ext) return;                                  // a view: its storage belongs to the tensor it was cut from
     const int64_t ne = (int64_t)1 << x.idx.size();
-    if (x.keep) deferred.push_back({x.off, ne});
+    if (x.keep) deferred.push_back({x.variant, x.off, ne});
     else (x.variant ? av : ai).release(x.off, ne);
   }
 
@@ -443,6 +444,7 @@ struct Planner {
       st.vA = A.variant; st.vB = B.variant; st.vC = var;
       st.rA = rA; st.rB = rB;
       st.n_slice = (int32_t)std::max(A.slice.size(), B.slice.size());
+      st.xA = A.ext ? 1 : 0; st.xB = B.ext ? 1 : 0;
       for (size_t j = 0; j < A.slice.size(); j++) st.sliceA[j] = A.slice[j];
       for (size_t j = 0; j < B.slice.size(); j++) st.sliceB[j] = B.slice[j];
       st.fma = fma;
@@ -641,7 +643,9 @@ int make_local_plan(const Problem &P, int cap_rank, LocalPlan &out, std::string 
   }
 
   // ---- pass 1: the walk that emits steps and assigns storage
-  Planner pl(P, 1, false, true, false, out.plan, err);
+  // two arenas: tensors that depend on a stretch's fixed indices are leaf-variant (one copy per branch of the batch
+  // in flight), everything else -- in particular every tensor that crosses a stretch boundary -- is invariant
+  Planner pl(P, 1, false, false, false, out.plan, err);
   int rc;
   pl.cap_rank = cap_rank;
   pl.set_fixed({}); pl.count_occurrences();
@@ -651,8 +655,12 @@ int make_local_plan(const Problem &P, int cap_rank, LocalPlan &out, std::string 
   auto run_range = [&](int a, int b, LocalSeg &ls) -> int {
     ls.step_begin = (int32_t)out.plan.steps.size();
     for (int s = a; s <= b; s++)
-      for (int t : inputs_of[s]) { pl.add_input(t); (out.plan.inputs[t].rank == 0 ? ls.list_scalar : ls.list_var).push_back(t); }
-    if (n_in == 1 && a == 0) { pl.add_input(0); (out.plan.inputs[0].rank == 0 ? ls.list_scalar : ls.list_var).push_back(0); }
+      for (int t : inputs_of[s]) {
+        pl.add_input(t);
+        const InputRec &r = out.plan.inputs[t];
+        (r.rank == 0 ? ls.list_scalar : (r.variant ? ls.list_var : ls.list_inv)).push_back(t);
+      }
+    if (n_in == 1 && a == 0) { pl.add_input(0); (out.plan.inputs[0].rank == 0 ? ls.list_scalar : ls.list_inv).push_back(0); }
     for (int s = a; s <= b; s++) if ((rc = pl.do_step((size_t)s))) return rc;
     ls.step_end = (int32_t)out.plan.steps.size();
     for (int q = ls.step_begin; q < ls.step_end; q++) {
@@ -683,6 +691,7 @@ int make_local_plan(const Problem &P, int cap_rank, LocalPlan &out, std::string 
       if (cons[t] > b) continue;                              // passes the segment untouched
       bool hit = false;
       for (int v : x.idx) if (inF[v]) hit = true;
+      if (x.variant) { err = "internal: a branch-dependent tensor crosses a stretch boundary"; return ST_EINVAL; }
       if (!hit) { x.keep = true; continue; }
       bases.push_back({x.off, (int64_t)1 << x.idx.size()});
       TRef vw = x;
@@ -692,12 +701,12 @@ int make_local_plan(const Problem &P, int cap_rank, LocalPlan &out, std::string 
         if (inF[v]) { vw.slice[(size_t)pos_of(ls.fixed, v)] = Planner::bit_of(x, (int)p2); vw.sub.erase(v); }
         else { vw.idx.push_back(v); vw.phys.push_back(Planner::bit_of(x, (int)p2)); }
       }
-      vw.ext = true; vw.keep = false;
+      vw.ext = true; vw.keep = false; vw.variant = true;     // read per branch: its consumers are branch-dependent
       x = std::move(vw);
     }
     const int acc_id = sel[q].acc_id;
     ls.acc_rank = (int32_t)lab[acc_id].size();
-    ls.acc_off = pl.av.alloc((int64_t)1 << ls.acc_rank);
+    ls.acc_off = pl.ai.alloc((int64_t)1 << ls.acc_rank);
     std::vector<int32_t> F32(ls.fixed.begin(), ls.fixed.end());
     if ((rc = pl.set_fixed(F32))) return rc;
     pl.deferred.clear();
@@ -705,18 +714,19 @@ int make_local_plan(const Problem &P, int cap_rank, LocalPlan &out, std::string 
     pl.set_fixed({});
     // the per-slice result sits at tmp_off; the tensor the rest of the tree sees is the accumulator
     TRef &z = pl.T[acc_id];
-    if (z.removed || (int)z.idx.size() != ls.acc_rank || z.ext) { err = "internal: sliced segment lost its result tensor"; return ST_EINVAL; }
+    if (z.removed || (int)z.idx.size() != ls.acc_rank || z.ext || !z.variant) { err = "internal: sliced segment lost its result tensor"; return ST_EINVAL; }
     for (int v : z.idx) if (inF[v]) { err = "internal: a locally fixed index leaves its segment"; return ST_EINVAL; }
     ls.tmp_off = z.off;
     pl.av.release(z.off, (int64_t)1 << ls.acc_rank);
-    z.off = ls.acc_off;
-    for (auto &bo : bases) pl.av.release(bo.first, bo.second);
-    for (auto &d : pl.deferred) pl.av.release(d.first, d.second);
+    z.off = ls.acc_off; z.variant = false;                    // (+) over the branches: no longer branch-dependent
+    for (auto &bo : bases) pl.ai.release(bo.first, bo.second);
+    for (auto &d : pl.deferred) (d.variant ? pl.av : pl.ai).release(d.off, d.ne);
     pl.deferred.clear();
     for (int t = 0; t <= n_in + b; t++) {
       TRef &x = pl.T[t];
       if (pl.used[t] || x.removed) continue;
       x.keep = false;
+      if (x.variant) { err = "internal: a branch-dependent tensor is still live after its segment"; return ST_EINVAL; }
       for (int v : x.idx) if (inF[v]) { err = "internal: a locally fixed index is still open after its segment"; return ST_EINVAL; }
     }
     ls.bytes += 36.0 * (double)((int64_t)1 << ls.acc_rank);   // accumulation pass: read slice + read/write accumulator

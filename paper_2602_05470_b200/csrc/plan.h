@@ -64,6 +64,7 @@ struct Step {
   // local slicing (make_local_plan): an operand that is a view of a stored tensor starts at
   // off + sum_j x_j * slice[j], x = the current assignment of the segment's fixed indices
   int32_t n_slice = 0;
+  int32_t xA = 0, xB = 0;                    // operand is such a view: it lives in the invariant arena, sliced per batch entry
   uint32_t sliceA[24] = {0}, sliceB[24] = {0};
   double fma = 0;               // tropical FMAs of this launch per batch entry
   double bytes = 0;             // algorithmic bytes per batch entry (12 B per element moved)
@@ -100,10 +101,11 @@ struct Plan {
 struct LocalSeg {
   std::vector<int32_t> fixed;            // F; empty = the segment runs once
   int32_t step_begin = 0, step_end = 0;  // range in Plan::steps
-  std::vector<int32_t> list_var;         // inputs K1 builds at the start of every slice (rank > 0 under F)
+  std::vector<int32_t> list_var;         // inputs K1 builds for every slice (they touch F; rank > 0 under F)
+  std::vector<int32_t> list_inv;         // inputs of the stretch that do not depend on F: built once per launch sequence
   std::vector<int32_t> list_scalar;      // inputs that are scalars under F: their product is the slice's offset
   int32_t acc_rank = -1;                 // sliced segments: the F-dependent tensor leaving the segment ...
-  int64_t acc_off = 0, tmp_off = 0;      // ... is accumulated at acc_off from the per-slice result at tmp_off
+  int64_t acc_off = 0, tmp_off = 0;      // ... is accumulated at acc_off (invariant arena) from the per-slice results at tmp_off (variant arena)
   int32_t max_rank = 0;
   double fma = 0, bytes = 0;             // per slice (bytes include the accumulation pass)
 };

@@ -132,7 +132,8 @@ def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None):
             "n_vertices": k.n_vertices, "n_edges": k.n_edges, "seconds": dt, "plan_only_seconds": t_plan, "energy": out["energy"],
             "count_mod_2_64": out["count"], "count": str(cnt), **{key: out[key] for key in bb.Handle._LOCAL_STATS},
             "fma": out["fma"] * rings, "bytes": out["bytes"] * rings,
-            "algorithmic_gb_per_s": (out["bytes"] * 12 + out["bytes"] * 8 * (rings - 1)) / 12 / dt / 1e9}
+            "bytes_contracted": out["bytes_contracted"] * (12 + 8 * (rings - 1)) / 12,
+            "algorithmic_gb_per_s": out["bytes_contracted"] * (12 + 8 * (rings - 1)) / 12 / dt / 1e9}
 
 
 def solve_e1(L, seed=1, log2_target=32):

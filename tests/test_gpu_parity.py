@@ -658,6 +658,7 @@ def test_solve_branching_king32_seed1_rank32_leaves(bb):
     ("cube3-crt", lambda: I.ising_lattice_3d(3, 3, 3, 2), 6, 4, 1, False),
     ("cube4", lambda: I.ising_lattice_3d(4, 4, 3, 5), 13, 12, 0, True),
     ("random-mis", lambda: I.random_graph(26, 0.2, 9, "mis"), 6, 4, 1, False),
+    ("king12-many-branches", lambda: I.kings_subgraph(12, 12, 0.8, 3), 8, 7, 0, False),      # 1029 and 8197 branches planned
 ])
 def test_solve_local_matches_oracle(bb, oracle, name, make, t, t2, flags, own_tree):
     inst = make()
@@ -679,6 +680,10 @@ def test_solve_local_matches_oracle(bb, oracle, name, make, t, t2, flags, own_tr
     if t2 is not None:
         two = h.solve_local(t2)
         assert two["max_rank"] <= t2 and two["branches_planned"] > out["branches_planned"]
+        # the surviving branches of a stretch run as batches (one plan, the batch axis of K1/K3), not one by one
+        if two["branches_contracted"] >= 8:
+            assert two["branches_in_flight"] > 1
+            assert two["launch_sequences"] < two["branches_contracted"] + two["stretches"]
         assert (two["energy"], two["count"]) == (ref_e, ref_c & MASK64)
     h.close()
 
