@@ -184,7 +184,7 @@ void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmaj
                        int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, int energy_bits, cudaStream_t st) {
   // RING_U64 runs on the 128-row streaming tile of gemm_tiled.cu, except where that tile would be
   // >= 75 % padding (M, N <= 64): there the 64x64 tile below wastes nothing and many CTAs fit per SM.
-  if (ring == RING_U64 && !(M <= BM && N <= BN)) {
+  if (ring == RING_U64 && (!(M <= BM && N <= BN) || gemm_pack16_eligible(K, count_bits, energy_bits))) {
     launch_gemm_tiled_u64(batch, G, M, N, K, a_kmajor, Ae, (const uint64_t *)Ac, Be, (const uint64_t *)Bc, Ce, (uint64_t *)Cc,
                           sA, sB, sC, count_bits, energy_bits, st);
     return;

@@ -30,13 +30,18 @@ namespace {
 using namespace stage;
 
 constexpr int BIAS = 11903, FINITE2 = 15872;   // enc(e) = e + BIAS;  half >= FINITE2  <=>  finite sum
-constexpr int BN = 128;
-constexpr int PT = 512;                            // threads per CTA: 4 x 8 outputs each, 4 warps per SM sub-partition
-constexpr int P_RAW = AE_BYTES + AC_BYTES + BK * BN * 4 + BK * BN * 8;
-constexpr int P_CAE = BK * BM * 4, P_CAC = BK * BM * 4, P_CBE = BK * (BN / 2) * 4, P_CBC = BK * BN * 4;
-constexpr int P_CONV = P_CAE + P_CAC + P_CBE + P_CBC;
-constexpr int P_SMEM = RAW_STAGES * P_RAW + CONV_STAGES * P_CONV;
-static_assert(P_SMEM <= 227 * 1024, "shared memory budget");
+// tile TB x TB (128: the general case; 64: matrices with M, N <= 64, where the big tile would be mostly padding),
+// TB*TB/32 threads: 4 x 8 outputs each
+template <int TB> struct Cfg {
+  static constexpr int BM = TB, BN = TB, PT = TB * TB / 32;
+  static constexpr int AE_B = BM * AE_LD * 4, AC_B = BM * AC_LD * 8;            // raw A planes (row-major form is the larger one)
+  static constexpr int RAW = AE_B + AC_B + BK * BN * 4 + BK * BN * 8;
+  static constexpr int CAE = BK * BM * 4, CAC = BK * BM * 4, CBE = BK * (BN / 2) * 4, CBC = BK * BN * 4;
+  static constexpr int CONV = CAE + CAC + CBE + CBC;
+  static constexpr int SMEM = RAW_STAGES * RAW + CONV_STAGES * CONV;
+  static constexpr int MIN_CTAS = TB == 128 ? 1 : 2;
+  static_assert(SMEM * MIN_CTAS <= 227 * 1024, "shared memory budget");
+};
 
 __device__ __forceinline__ uint32_t enc(int32_t e) { return e < ZERO_BELOW ? 0u : (uint32_t)(e + BIAS); }
 
@@ -73,14 +78,16 @@ __device__ __forceinline__ void reset2(uint32_t &c_lo, uint32_t &c_hi, uint32_t 
 
 // raw stage (operands in their global layout) -> converted stage: encoded energies, A k-major with the value in both
 // halves, B as packed column pairs laid out [k][tx][q][p] (column = q*64 + tx*4 + 2p + half), counts narrowed to 32 bits
-template <bool A_KMAJOR>
+template <bool A_KMAJOR, int TB>
 __device__ __forceinline__ void convert_pack16(const unsigned char *raw, unsigned char *conv) {
+  using G = Cfg<TB>;
+  constexpr int BM = G::BM, BN = G::BN, PT = G::PT;
   const int t = threadIdx.x;
-  const unsigned char *rAe = raw, *rAc = raw + AE_BYTES, *rBe = raw + AE_BYTES + AC_BYTES, *rBc = rBe + BK * BN * 4;
+  const unsigned char *rAe = raw, *rAc = raw + G::AE_B, *rBe = raw + G::AE_B + G::AC_B, *rBc = rBe + BK * BN * 4;
   uint32_t *cAe = reinterpret_cast<uint32_t *>(conv);
-  uint32_t *cAc = reinterpret_cast<uint32_t *>(conv + P_CAE);
-  uint32_t *cBe = reinterpret_cast<uint32_t *>(conv + P_CAE + P_CAC);
-  uint32_t *cBc = reinterpret_cast<uint32_t *>(conv + P_CAE + P_CAC + P_CBE);
+  uint32_t *cAc = reinterpret_cast<uint32_t *>(conv + G::CAE);
+  uint32_t *cBe = reinterpret_cast<uint32_t *>(conv + G::CAE + G::CAC);
+  uint32_t *cBc = reinterpret_cast<uint32_t *>(conv + G::CAE + G::CAC + G::CBE);
   if (A_KMAJOR) {
 #pragma unroll
     for (int idx = t; idx < BK * BM / 4; idx += PT) {
@@ -93,24 +100,26 @@ __device__ __forceinline__ void convert_pack16(const unsigned char *raw, unsigne
       *reinterpret_cast<uint2 *>(cAc + 2 * idx) = make_uint2((uint32_t)v.x, (uint32_t)v.y);
     }
   } else {
-    // transpose: lane = row, so the k-major stores of a warp are contiguous; each thread moves 4 k of one row
-    const int r = t % BM, kb = (t / BM) * 4;               // PT / BM = 4 groups x 4 k = BK
-    {
-      const int4 v = *reinterpret_cast<const int4 *>(rAe + (r * AE_LD + kb) * 4);
-      cAe[(kb + 0) * BM + r] = enc(v.x) * 0x10001u; cAe[(kb + 1) * BM + r] = enc(v.y) * 0x10001u;
-      cAe[(kb + 2) * BM + r] = enc(v.z) * 0x10001u; cAe[(kb + 3) * BM + r] = enc(v.w) * 0x10001u;
+    // transpose: lane = row, so the k-major stores of a warp are contiguous; PT / BM thread groups share the BK values of k
+    constexpr int KPER = BK / (PT / BM);                   // 4 (TB = 128) or 8 (TB = 64) k per thread
+    const int r = t % BM, kb = (t / BM) * KPER;
+#pragma unroll
+    for (int q = 0; q < KPER / 4; q++) {
+      const int4 v = *reinterpret_cast<const int4 *>(rAe + (r * AE_LD + kb + 4 * q) * 4);
+      cAe[(kb + 4 * q + 0) * BM + r] = enc(v.x) * 0x10001u; cAe[(kb + 4 * q + 1) * BM + r] = enc(v.y) * 0x10001u;
+      cAe[(kb + 4 * q + 2) * BM + r] = enc(v.z) * 0x10001u; cAe[(kb + 4 * q + 3) * BM + r] = enc(v.w) * 0x10001u;
     }
 #pragma unroll
-    for (int q = 0; q < 2; q++) {
+    for (int q = 0; q < KPER / 2; q++) {
       const ulonglong2 v = *reinterpret_cast<const ulonglong2 *>(rAc + (r * AC_LD + kb + 2 * q) * 8);
       cAc[(kb + 2 * q + 0) * BM + r] = (uint32_t)v.x; cAc[(kb + 2 * q + 1) * BM + r] = (uint32_t)v.y;
     }
   }
 #pragma unroll
   for (int idx = t; idx < BK * BN / 4; idx += PT) {            // 4 consecutive columns -> two packed words
-    const int kk = idx / (BN / 4), c4 = idx % (BN / 4);       // columns 4*c4 .. 4*c4+3: q = c4 / 16, tx = c4 % 16
+    const int kk = idx / (BN / 4), c4 = idx % (BN / 4);       // columns 4*c4 .. 4*c4+3: q = c4 / (BN/8), tx = c4 % (BN/8)
     const int4 v = *reinterpret_cast<const int4 *>(rBe + 16 * idx);
-    *reinterpret_cast<uint2 *>(cBe + kk * (BN / 2) + (c4 % 16) * 4 + (c4 / 16) * 2) =
+    *reinterpret_cast<uint2 *>(cBe + kk * (BN / 2) + (c4 % (BN / 8)) * 4 + (c4 / (BN / 8)) * 2) =
         make_uint2(enc(v.x) | (enc(v.y) << 16), enc(v.z) | (enc(v.w) << 16));
   }
 #pragma unroll
@@ -125,8 +134,11 @@ __device__ __forceinline__ void lds4(const uint32_t *src, uint32_t *dst) {
   dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
 }
 
-template <bool A_KMAJOR>
-__global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
+template <bool A_KMAJOR, int TB>
+__global__ void __launch_bounds__(Cfg<TB>::PT, Cfg<TB>::MIN_CTAS) gemm_pack16_kernel(const GemmArgs p) {
+  using G = Cfg<TB>;
+  constexpr int BM = G::BM, BN = G::BN, PT = G::PT;
+  constexpr int P_RAW = G::RAW, P_CONV = G::CONV, P_CAE = G::CAE, P_CAC = G::CAC, P_CBE = G::CBE;
   extern __shared__ __align__(16) unsigned char smem[];
   unsigned char *conv_base = smem + RAW_STAGES * P_RAW;
 
@@ -140,10 +152,11 @@ __global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
   int32_t *ce = p.Ce + b * p.sC + g * (int64_t)p.M * p.N; uint64_t *cc = p.Cc + b * p.sC + g * (int64_t)p.M * p.N;
 
   // a warp covers 8 tx x 4 ty: A fetches touch 4 distinct 16-byte granules, B fetches 8; 16 warps = 2 (tx) x 8 (ty)
+  constexpr int WX = BN / 64;                               // warps side by side along the columns (8 tx each)
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tx = (w & 1) * 8 + (lane & 7), ty = (w >> 1) * 4 + (lane >> 3);      // tx 0..15, ty 0..31
+  const int tx = (w % WX) * 8 + (lane & 7), ty = (w / WX) * 4 + (lane >> 3);      // tx 0..BN/8-1, ty 0..BM/4-1
 
-  // rows: ty*4 + i (i = 0..3); columns: q*64 + tx*4 + 2p + half (q = 0,1; p = 0,1)
+  // rows: ty*4 + i (i = 0..3); columns: q*BN/2 + tx*4 + 2p + half (q = 0,1; p = 0,1)
   uint32_t E2[4][4], C[4][8];
 #pragma unroll
   for (int i = 0; i < 4; i++) {
@@ -157,13 +170,13 @@ __global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
   auto issue = [&](int c) {
     if (c < n_chunks) {
       unsigned char *s = smem + (c % RAW_STAGES) * P_RAW;
-      fill_A<A_KMAJOR, PT>(p, ae, ac, m0, c * BK, s, s + AE_BYTES);
-      fill_B<BN, PT>(p, be, bc, n0, c * BK, s + AE_BYTES + AC_BYTES, s + AE_BYTES + AC_BYTES + BK * BN * 4);
+      fill_A<A_KMAJOR, PT, BM>(p, ae, ac, m0, c * BK, s, s + G::AE_B);
+      fill_B<BN, PT>(p, be, bc, n0, c * BK, s + G::AE_B + G::AC_B, s + G::AE_B + G::AC_B + BK * BN * 4);
     }
     cp_async_commit();
   };
   auto convert = [&](int c) {
-    if (c < n_chunks) convert_pack16<A_KMAJOR>(smem + (c % RAW_STAGES) * P_RAW, conv_base + (c % CONV_STAGES) * P_CONV);
+    if (c < n_chunks) convert_pack16<A_KMAJOR, TB>(smem + (c % RAW_STAGES) * P_RAW, conv_base + (c % CONV_STAGES) * P_CONV);
   };
 
   // pass 1 of one chunk on row block rb: En2 <- max(En2, a2 + b2)
@@ -206,7 +219,7 @@ __global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
       uint32_t a2[4], ca[4], b2[4], cb[8];
       lds4(a2e + kk * BM, a2); lds4(a2c + kk * BM, ca);
       lds4(b2e + kk * (BN / 2), b2);
-      lds4(b2c + kk * BN, cb); lds4(b2c + kk * BN + 64, cb + 4);
+      lds4(b2c + kk * BN, cb); lds4(b2c + kk * BN + BN / 2, cb + 4);
       uint32_t a1[4], b1[4];
       if (P1) { lds4(a1e + kk * BM, a1); lds4(b1e + kk * (BN / 2), b1); }
 #pragma unroll
@@ -256,7 +269,7 @@ __global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
     if (gm >= p.M) continue;
 #pragma unroll
     for (int q = 0; q < 2; q++) {
-      const int gn = n0 + q * 64 + tx * 4;
+      const int gn = n0 + q * (BN / 2) + tx * 4;
       int32_t e[4]; uint64_t c[4];
 #pragma unroll
       for (int j = 0; j < 4; j++) {
@@ -281,6 +294,14 @@ __global__ void __launch_bounds__(PT, 1) gemm_pack16_kernel(const GemmArgs p) {
 
 inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
+template <bool KM, int TB>
+void launch_p16(const GemmArgs &a, int64_t batch, cudaStream_t st) {
+  using G = Cfg<TB>;
+  const int64_t n_cta = (int64_t)((a.N + G::BN - 1) / G::BN) * ((a.M + G::BM - 1) / G::BM) * batch * a.G;
+  cudaFuncSetAttribute(gemm_pack16_kernel<KM, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM);
+  gemm_pack16_kernel<KM, TB><<<dim3((unsigned)n_cta), G::PT, G::SMEM, st>>>(a);
+}
+
 }  // namespace
 
 // RING_U64, caller promises: finite |energy| <= 3967 (zero element exactly NEG_INF) and counts small enough for
@@ -293,14 +314,9 @@ void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kma
   a.vecA = (ldA % 4 == 0) && (sA % 4 == 0) && (((int64_t)M * K) % 4 == 0 || G == 1) && al16(Ae) && al16(Ac);
   a.vecB = (N % 4 == 0) && (sB % 4 == 0) && (((int64_t)K * N) % 4 == 0 || G == 1) && al16(Be) && al16(Bc);
   a.vecC = (N % 4 == 0) && (sC % 4 == 0) && (((int64_t)M * N) % 4 == 0 || G == 1) && al16(Ce) && al16(Cc);
-  const int64_t n_cta = (int64_t)((N + BN - 1) / BN) * ((M + BM - 1) / BM) * batch * G;
-  if (a_kmajor) {
-    cudaFuncSetAttribute(gemm_pack16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM);
-    gemm_pack16_kernel<true><<<dim3((unsigned)n_cta), PT, P_SMEM, st>>>(a);
-  } else {
-    cudaFuncSetAttribute(gemm_pack16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM);
-    gemm_pack16_kernel<false><<<dim3((unsigned)n_cta), PT, P_SMEM, st>>>(a);
-  }
+  const bool small = M <= 64 && N <= 64;                   // a 128-row tile would be >= 75 % padding
+  if (a_kmajor) { if (small) launch_p16<true, 64>(a, batch, st); else launch_p16<true, 128>(a, batch, st); }
+  else { if (small) launch_p16<false, 64>(a, batch, st); else launch_p16<false, 128>(a, batch, st); }
 }
 
 }  // namespace bbtn

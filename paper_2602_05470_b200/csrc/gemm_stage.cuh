@@ -31,9 +31,10 @@ struct GemmArgs {
 };
 
 // ---- global -> shared for one chunk (k0 .. k0+BK) of one operand ------------------------------
-template <bool A_KMAJOR, int NT = 256>
+template <bool A_KMAJOR, int NT = 256, int TBM = 128>
 __device__ __forceinline__ void fill_A(const GemmArgs &p, const int32_t *__restrict__ ae, const uint64_t *__restrict__ ac,
                                        int m0, int k0, unsigned char *sAe, unsigned char *sAc) {
+  constexpr int BM = TBM;                 // rows of the A tile (the 64-row packed kernel uses a smaller tile)
   const int t = threadIdx.x;
   const bool fast = p.vecA && m0 + BM <= p.M && k0 + BK <= p.K;
   if (fast) {

@@ -341,6 +341,13 @@ inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) =
 
 }  // namespace
 
+// the packed form needs 32-bit accumulators (2 * count_bits + ceil(log2 K) <= 32) and finite |energy| < 2^11
+bool gemm_pack16_eligible(int K, int count_bits, int energy_bits) {
+  int lgK = 0;
+  while (((int64_t)1 << lgK) < K) lgK++;
+  return count_bits <= 16 && 2 * count_bits + lgK <= 32 && energy_bits <= 11;
+}
+
 // RING_U64 only.  count_bits is the caller's bound on log2(count+1) of both operands.
 void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                            const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,

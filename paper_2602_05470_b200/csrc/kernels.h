@@ -49,7 +49,9 @@ void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_
                            int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, int energy_bits,
                            cudaStream_t st);
 
-// K3 packed form (gemm_pack16.cu): two outputs per integer instruction; finite |energy| < 2^11, 32-bit accumulators.
+bool gemm_pack16_eligible(int K, int count_bits, int energy_bits);
+
+// K3 packed form (gemm_pack16.cu; 128 x 128 tile, 64 x 64 for M, N <= 64): two outputs per integer instruction; finite |energy| < 2^11, 32-bit accumulators.
 void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                         const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
                         int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, cudaStream_t st);

@@ -38,6 +38,10 @@ SPARSE_CASES = [
     ("config5-shape king 32x32 p0.8 seed 2", lambda: I.kings_subgraph(32, 32, 0.8, 2)),
     ("config5-shape king 36x36 p0.8 seed 1", lambda: I.kings_subgraph(36, 36, 0.8, 1)),
     ("config5 king 40x40 p0.8 seed 1", lambda: I.kings_subgraph(40, 40, 0.8, 1)),
+    # more instances of the same ensemble (PAPER.md:95 averages over 10 instances per N)
+    ("config5-shape king 36x36 p0.8 seed 2", lambda: I.kings_subgraph(36, 36, 0.8, 2)),
+    ("config5-shape king 36x36 p0.8 seed 3", lambda: I.kings_subgraph(36, 36, 0.8, 3)),
+    ("config5 king 40x40 p0.8 seed 2", lambda: I.kings_subgraph(40, 40, 0.8, 2)),
 ]
 
 
