@@ -417,6 +417,28 @@ def test_join_over_13_summed_indices(bb, oracle, mode):
     h.close()
 
 
+@pytest.mark.parametrize("rows,cols,cuts", [(8, 3, [1]), (9, 4, [1, 2]), (7, 5, [2])])
+def test_tree_gemm_with_small_counts_takes_the_packed_kmajor_form(bb, oracle, rows, cols, cuts):
+    # FORCE_TILED on thin column blocks: the joins are GEMMs with M = 2^rows (> 64) whose operands have summed only a
+    # few vertices, so the planner's count bound allows 32-bit accumulators and the problem's energy bound the packed
+    # 16x2 form -- the k-major (engine-layout) instantiation of gemm_pack16_kernel, which the raw ABI never reaches
+    inst = I.ising_lattice_2d(rows, cols, 11 + rows, field_h=1)
+    tree = I.grouped_elimination_tree(inst.input_index_sets(), I.lattice_block_parts(rows, cols, [], cuts))
+    want = oracle.contract_tree(inst, *tree)
+    assert want == oracle.frontier_dp(inst)
+    for flags in (bb.BBTN_FORCE_TILED, bb.BBTN_FORCE_TILED | bb.BBTN_COUNT_CRT):
+        h = bb.Handle(inst, tree=tree, flags=flags)
+        assert h.plan_query()["n_gemm_tiled"] > 0
+        out = h.contract_batch()
+        assert (int(out[0][0]), int(out[1][0])) == (want[0], want[1] & MASK64)
+        h.close()
+    # the same with a sliced batch (leaf-variant operands: batch strides on A or B)
+    fixed = np.array([0, rows * cols - 1], np.int32)
+    parts = I.lattice_block_parts(rows, cols, [], cuts, exclude=fixed)
+    t2 = I.grouped_elimination_tree(inst.input_index_sets(fixed), parts)
+    _check_leaves(bb, oracle, inst, t2, fixed, I.all_assignments(2), bb.BBTN_FORCE_TILED)
+
+
 def test_batch_size_and_order_independence(bb):
     inst = I.ising_lattice_2d(8, 8, 3)
     fixed = I.slit_fixed_set_2d(8, 8, 4)
@@ -717,7 +739,7 @@ def test_solve_local_prunes_with_region_bounds(bb, oracle, kind):
     h.close()
 
 
-@pytest.mark.parametrize("L,seed,t", [(28, 1, 29), (32, 1, 31), (32, 2, 30), (36, 1, 32)])
+@pytest.mark.parametrize("L,seed,t", [(28, 1, 29), (32, 1, 31), (32, 2, 30), (36, 1, 32), (36, 2, 32), (36, 3, 32)])
 def test_solve_local_kings_large(bb, L, seed, t):
     # King's subgraphs at filling 0.8 beyond the reach of one dense contraction at the threshold: goldens by the
     # oracle's sparse frontier DP (tests/golden/config_goldens.json)
