@@ -452,19 +452,19 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
   // copies -- so the PCIe transfers of chunk c+1 / c-1 overlap the GEMM of chunk c (pinned host memory needed for
   // the overlap; pageable memory still works, serialised by the driver).  Shared operands (stride 0) go up once.
   static thread_local cudaStream_t s_in = nullptr, s_k = nullptr, s_out = nullptr;
-  static thread_local cudaEvent_t ev_start = nullptr, ev_in[8], ev_k[8], ev_done = nullptr;
+  static thread_local cudaEvent_t ev_start = nullptr, ev_in[16], ev_k[16], ev_done = nullptr;
   if (!s_in) {
     CUDA_TRY(nullptr, cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
     CUDA_TRY(nullptr, cudaStreamCreateWithFlags(&s_k, cudaStreamNonBlocking));
     CUDA_TRY(nullptr, cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
     CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
     CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming));
-    for (int i = 0; i < 8; i++) {
+    for (int i = 0; i < 16; i++) {
       CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_in[i], cudaEventDisableTiming));
       CUDA_TRY(nullptr, cudaEventCreateWithFlags(&ev_k[i], cudaEventDisableTiming));
     }
   }
-  const int n_chunks = (int)std::min<int64_t>(8, std::max<int64_t>(1, batch / 4));   // >= 4 entries per chunk
+  const int n_chunks = (int)std::min<int64_t>(16, std::max<int64_t>(1, batch / 4));   // >= 4 entries per chunk; short chunks keep the tail (last GEMM + copy-out) small
   int32_t *dAe = (int32_t *)st_e[0].p, *dBe = (int32_t *)st_e[1].p, *dCe = (int32_t *)st_e[2].p;
   uint64_t *dAc = (uint64_t *)st_c[0].p, *dBc = (uint64_t *)st_c[1].p, *dCc = (uint64_t *)st_c[2].p;
   CUDA_TRY(nullptr, cudaEventRecord(ev_start, st));
