@@ -225,6 +225,13 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
                      int32_t *energy, uint64_t *count, uint32_t *count_mod, int64_t *stats, double *work,
                      void *cuda_stream);
 
+/* A hint for the library's tree search (only used when the handle was built WITHOUT a tree): `order` [n_vertices] is
+ * a permutation of the vertices, e.g. a sweep of the caller's geometry in another direction.  bbtn_solve_local derives
+ * its candidate trees (nested-minimum-cut sweeps, reading A26) from the vertex-id order, from every hinted
+ * order and from each of them reversed, plans all of them and keeps the cheapest.  Results never depend on it.
+ * Host only.  Errors: EINVAL (not a permutation). */
+int bbtn_add_sweep_order(bbtn_handle *h, const int32_t *order);
+
 /* The plan bbtn_solve_local would run, without running it (host only, no device): stats / work as above
  * (the run-time entries 3, 4, 5, 9, 10, 11 and work[2..3] are zero).  mem_budget_bytes = 0 means no memory limit here. */
 int bbtn_local_plan_query(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t *stats, double *work);

@@ -23,7 +23,7 @@ BBTN_COUNT_CRT, BBTN_IO_DEVICE, BBTN_NO_GRAPH = 0x1, 0x2, 0x4
 BBTN_FORCE_STREAMING, BBTN_FORCE_TILED, BBTN_SEARCH_ONLY, BBTN_NO_FUSED = 0x10, 0x20, 0x40, 0x80
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
-EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query",
+EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query", "bbtn_add_sweep_order",
            "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
            "bbtn_permute_batched", "bbtn_int32_microbench", "bbtn_crt_combine", "bbtn_set_debug_checks",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
@@ -69,6 +69,7 @@ def load():
     lib.bbtn_branching_leaves.argtypes = [vp, i32, i64, i64, i64, i64, vp, vp, vp, vp, vp]
     lib.bbtn_solve_local.argtypes = [vp, i32, i64, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.bbtn_local_plan_query.argtypes = [vp, i32, i64, vp, vp]
+    lib.bbtn_add_sweep_order.argtypes = [vp, vp]
     lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, i32, vp]
     lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, i32, vp]
     lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
@@ -234,6 +235,11 @@ class Handle:
         if crt:
             out["count_mod"] = (cm[0], cm[1])
         return out
+
+    def add_sweep_order(self, order):
+        """bbtn_add_sweep_order: another base order (a permutation of the vertices) for the library's tree search."""
+        o = _np(order, np.int32)
+        _check(load().bbtn_add_sweep_order(self._h, _ptr(o)), self._h)
 
     def local_plan_query(self, log2_target: int, mem_budget_bytes: int = 0) -> dict:
         """bbtn_local_plan_query (host only)."""

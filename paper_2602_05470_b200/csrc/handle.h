@@ -72,6 +72,10 @@ struct bbtn_handle {
   std::map<std::vector<int32_t>, std::unique_ptr<bbtn::BoundPlan>> bounds;
   // branching driver (branching.cu): the unsliced tree every leaf is planned on, and one scratch plan whose
   // device buffers are reused by every leaf (leaves have different fixed sets, so they are not cached)
+  std::vector<std::vector<int>> sweep_orders;        // caller's base orders for the library's tree search (bbtn_add_sweep_order)
+  // the plan bbtn_local_plan_query / bbtn_solve_local chose last (tree search over many candidates: not repeated for the same request)
+  struct LocalChoice { int32_t log2_target = 0; int64_t budget = 0; size_t n_hints = 0; bbtn::LocalPlan lp; std::shared_ptr<bbtn::Problem> P; };
+  std::unique_ptr<LocalChoice> local_choice;
   std::unique_ptr<bbtn::Problem> Pbr;
   std::unique_ptr<bbtn::DevPlan> scratch;
 };

@@ -13,7 +13,9 @@
 // Host logic only: tensors are built, contracted and (+)-accumulated by the kernels (kernels.h).
 #include <algorithm>
 #include <cmath>
+#include <atomic>
 #include <cstring>
+#include <thread>
 
 #include "handle.h"
 
@@ -173,6 +175,16 @@ struct LocalRun {
   }
 };
 
+// run fn(i) for i in [0, n) on the host's cores (planning candidates are independent of one another)
+template <class F> void parallel_for(size_t n, F fn) {
+  const size_t nt = std::min<size_t>(n, std::max(1u, std::thread::hardware_concurrency()));
+  if (nt <= 1) { for (size_t i = 0; i < n; i++) fn(i); return; }
+  std::atomic<size_t> next{0};
+  std::vector<std::thread> th;
+  for (size_t t = 0; t < nt; t++) th.emplace_back([&] { for (size_t i; (i = next.fetch_add(1)) < n;) fn(i); });
+  for (auto &t : th) t.join();
+}
+
 // Candidate trees: the caller's tree if there is one; else elimination trees along the vertex-id order, the
 // min-degree order and nested-min-cut sweeps with several look-ahead windows (plan.cpp).  The driver plans
 // every candidate and keeps the cheapest one that fits.
@@ -186,13 +198,35 @@ void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out)
   orders.push_back(min_degree_order(P0, {}));
   int w0 = 0; double c0 = 0;
   { std::vector<int32_t> l, r; elimination_tree_for_order(P0, {}, natural, l, r, w0, c0); }
-  for (int mult : {2, 3, 4, 5, 6, 8}) orders.push_back(mincut_sweep_order(P0, 4, std::max(8, mult * w0)));
-  for (auto &o : orders) {
+  // base orders of the nested-min-cut sweeps: the vertex ids, the caller's hints (bbtn_add_sweep_order), and each reversed
+  std::vector<std::vector<int>> bases;
+  bases.push_back(natural);
+  for (auto &o : h->sweep_orders) bases.push_back(o);
+  const size_t nb0 = bases.size();
+  for (size_t i = 0; i < nb0; i++) bases.push_back(std::vector<int>(bases[i].rbegin(), bases[i].rend()));
+  struct Job { size_t base; int half; };
+  std::vector<Job> jobs;
+  std::vector<int> widths(bases.size(), w0);
+  for (size_t i = 1; i < bases.size(); i++) orders.push_back(bases[i]);
+  parallel_for(bases.size(), [&](size_t i) {                            // the look-ahead windows scale with each sweep's width
+    if (i == 0) return;
+    std::vector<int32_t> l, r; double c = 0;
+    elimination_tree_for_order(P0, {}, bases[i], l, r, widths[i], c);
+  });
+  for (size_t i = 0; i < bases.size(); i++)
+    for (int half : {4, 6, 8, 9, 10, 11, 12, 14, 16}) jobs.push_back({i, half});   // windows of 2 .. 8 sweep widths
+  const size_t first_job = orders.size();
+  orders.resize(first_job + jobs.size());
+  parallel_for(jobs.size(), [&](size_t j) {
+    orders[first_job + j] = mincut_sweep_order(P0, 4, std::max(8, jobs[j].half * widths[jobs[j].base] / 2), &bases[jobs[j].base]);
+  });
+  out.resize(orders.size());
+  parallel_for(orders.size(), [&](size_t i) {
     auto P = std::make_unique<Problem>(P0);
     int w = 0; double c = 0;
-    elimination_tree_for_order(P0, {}, o, P->tree_l, P->tree_r, w, c);
-    out.push_back(std::move(P));
-  }
+    elimination_tree_for_order(P0, {}, orders[i], P->tree_l, P->tree_r, w, c);
+    out[i] = std::move(P);
+  });
 }
 
 void write_plan_stats(const LocalPlan &lp, int64_t *stats, double *work, bool search) {
@@ -208,21 +242,36 @@ void write_plan_stats(const LocalPlan &lp, int64_t *stats, double *work, bool se
 
 // plan at log2_target, lowering the threshold while no candidate's arena fits the memory budget; among the
 // candidates that fit, the one that moves the fewest bytes
-int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, LocalPlan &lp, std::unique_ptr<Problem> &P_out) {
+int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, LocalPlan &lp, std::shared_ptr<Problem> &P_out) {
   const int64_t per_elem = (h->P.flags & BBTN_SEARCH_ONLY) ? 4 : 12;
+  if (h->local_choice && h->local_choice->log2_target == log2_target && h->local_choice->n_hints == h->sweep_orders.size() &&
+      (h->local_choice->budget == budget ||
+       (budget > 0 && (h->local_choice->lp.plan.arena_invariant_elems + h->local_choice->lp.plan.arena_variant_elems) * per_elem <= budget &&
+        h->local_choice->lp.cap_rank == log2_target))) {
+    lp = h->local_choice->lp; P_out = h->local_choice->P;       // same request (or an unconstrained choice that also fits this budget)
+    return BBTN_OK;
+  }
   std::vector<std::unique_ptr<Problem>> cands;
   candidate_trees(h, cands);
   std::string last_err; int last_rc = BBTN_ESHAPE;
   for (int cap = log2_target; cap >= 1; cap--) {
-    int best = -1; LocalPlan best_lp;
+    std::vector<LocalPlan> plans(cands.size());
+    std::vector<int> rcs(cands.size(), 0);
+    std::vector<std::string> errs(cands.size());
+    parallel_for(cands.size(), [&](size_t i) { rcs[i] = make_local_plan(*cands[i], cap, plans[i], errs[i]); });
+    int best = -1;
     for (size_t i = 0; i < cands.size(); i++) {
-      LocalPlan cur; std::string err;
-      int rc = make_local_plan(*cands[i], cap, cur, err);
-      if (rc) { last_rc = rc; last_err = err; continue; }
-      if (budget > 0 && (cur.plan.arena_invariant_elems + cur.plan.arena_variant_elems) * per_elem > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
-      if (best < 0 || cur.bytes_total < best_lp.bytes_total) { best = (int)i; best_lp = std::move(cur); }
+      if (rcs[i]) { last_rc = rcs[i]; last_err = errs[i]; continue; }
+      if (budget > 0 && (plans[i].plan.arena_invariant_elems + plans[i].plan.arena_variant_elems) * per_elem > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
+      if (best < 0 || plans[i].bytes_total < plans[best].bytes_total) best = (int)i;
     }
-    if (best >= 0) { lp = std::move(best_lp); P_out = std::move(cands[best]); return BBTN_OK; }
+    if (best >= 0) {
+      lp = std::move(plans[best]); P_out = std::move(cands[best]);
+      h->local_choice = std::make_unique<bbtn_handle::LocalChoice>();
+      h->local_choice->log2_target = log2_target; h->local_choice->budget = budget; h->local_choice->n_hints = h->sweep_orders.size();
+      h->local_choice->lp = lp; h->local_choice->P = P_out;
+      return BBTN_OK;
+    }
   }
   return fail(h, last_rc, last_err);
 }
@@ -231,10 +280,22 @@ int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, Loca
 
 extern "C" {
 
+int bbtn_add_sweep_order(bbtn_handle *h, const int32_t *order) {
+  if (!h || !order) return fail(h, BBTN_EINVAL, "null argument");
+  std::vector<int> o(order, order + h->P.n);
+  std::vector<char> seen(h->P.n, 0);
+  for (int v : o) {
+    if (v < 0 || v >= h->P.n || seen[v]) return fail(h, BBTN_EINVAL, "order is not a permutation of the vertices");
+    seen[v] = 1;
+  }
+  h->sweep_orders.push_back(std::move(o));
+  return BBTN_OK;
+}
+
 int bbtn_local_plan_query(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_bytes, int64_t *stats, double *work) {
   if (!h) return fail(nullptr, BBTN_EINVAL, "null handle");
   if (log2_target < 1 || log2_target > 32) return fail(h, BBTN_EINVAL, "log2_target must be in 1..32");
-  LocalPlan lp; std::unique_ptr<Problem> P;
+  LocalPlan lp; std::shared_ptr<Problem> P;
   int rc = plan_within_budget(h, log2_target, mem_budget_bytes, lp, P);
   if (rc) return rc;
   write_plan_stats(lp, stats, work, (h->P.flags & BBTN_SEARCH_ONLY) != 0);
@@ -257,7 +318,7 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
     CUDA_TRY(h, cudaMemGetInfo(&free_b, &total_b));
     mem_budget_bytes = (int64_t)((double)free_b * 0.94);
   }
-  LocalPlan lp; std::unique_ptr<Problem> Pt;
+  LocalPlan lp; std::shared_ptr<Problem> Pt;
   int rc = plan_within_budget(h, log2_target, mem_budget_bytes, lp, Pt);
   if (rc) return rc;
   const Problem *P = Pt.get();

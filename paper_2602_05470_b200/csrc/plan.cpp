@@ -174,10 +174,13 @@ std::vector<int> min_degree_order(const Problem &P, const std::vector<int32_t> &
 // finds the smallest separator between them; X becomes the source side closest to the source.  On a King's subgraph
 // at filling 0.8 the separators thread through the missing sites: ~30 kept sites where a straight row holds up to 39.
 // The vertices a round adds are ordered greedily (the one that enlarges the frontier least goes first).
-std::vector<int> mincut_sweep_order(const Problem &P, int delta, int window) {
+std::vector<int> mincut_sweep_order(const Problem &P, int delta, int window, const std::vector<int> *base) {
   const int n = P.n;
+  // the sweep runs on POSITIONS of a base order (the vertex ids themselves when base == nullptr); mapped back at the end
+  std::vector<int> posn(n);
+  for (int i = 0; i < n; i++) posn[base ? (*base)[i] : i] = i;
   std::vector<std::vector<int>> adj(n);
-  for (int e = 0; e < P.m; e++) { adj[P.eu[e]].push_back(P.ev[e]); adj[P.ev[e]].push_back(P.eu[e]); }
+  for (int e = 0; e < P.m; e++) { const int u = posn[P.eu[e]], v = posn[P.ev[e]]; adj[u].push_back(v); adj[v].push_back(u); }
   std::vector<char> inX(n, 0), front(n, 0);
   std::vector<int> order;
   order.reserve(n);
@@ -243,6 +246,7 @@ std::vector<int> mincut_sweep_order(const Problem &P, int delta, int window) {
     n_in_X += (int)slab.size();
     add_slab(std::move(slab));
   }
+  if (base) for (int &v : order) v = (*base)[v];
   return order;
 }
 

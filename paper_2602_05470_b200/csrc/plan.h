@@ -138,6 +138,6 @@ void derive_tree(const Problem &P, const std::vector<int32_t> &fixed,
 void elimination_tree_for_order(const Problem &P, const std::vector<int32_t> &fixed, const std::vector<int> &order,
                                 std::vector<int32_t> &tl, std::vector<int32_t> &tr, int &width, double &cost);
 std::vector<int> min_degree_order(const Problem &P, const std::vector<int32_t> &fixed);
-std::vector<int> mincut_sweep_order(const Problem &P, int delta, int window);
+std::vector<int> mincut_sweep_order(const Problem &P, int delta, int window, const std::vector<int> *base = nullptr);
 
 }  // namespace bbtn

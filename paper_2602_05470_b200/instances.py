@@ -149,6 +149,16 @@ def kings_subgraph(rows: int, cols: int, filling: float, seed: int,
                     None, w, {"shape": (rows, cols), "seed": seed, "keep": keep, "pos": pos})
 
 
+def column_major_order(inst: "Instance") -> np.ndarray:
+    """The kept sites of a King's subgraph (or the sites of a 2-D lattice) column by column: a sweep in the other
+    direction than the vertex ids (which are row-major).  Pure geometry; a hint for the library's tree search."""
+    if "pos" in inst.meta:
+        pos = inst.meta["pos"]
+        return np.lexsort((pos[:, 0], pos[:, 1])).astype(np.int32)
+    rows, cols = inst.meta["shape"]
+    return np.array([r * cols + c for c in range(cols) for r in range(rows)], np.int32)
+
+
 def random_graph(n: int, p: float, seed: int, kind: str = "ising", field_h: bool = False) -> Instance:
     """Small Erdos-Renyi graph for brute-force pins (edge (i<j) kept iff u < p)."""
     pairs = [(i, j) for i in range(n) for j in range(i + 1, n)]

@@ -117,6 +117,7 @@ def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None):
             verts += [int(ids[r][c]) for r in range(r0, min(r0 + block, L)) for c in range(c0, min(c0 + block, L)) if ids[r][c] >= 0]
             offs.append(len(verts))
     h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT if crt else 0)
+    h.add_sweep_order(I.column_major_order(k))          # the library also tries sweeps along the columns
     t0 = time.perf_counter()
     plan = h.local_plan_query(log2_target)
     t_plan = time.perf_counter() - t0

@@ -213,3 +213,23 @@ def test_block_tree_plans_use_tiled_gemm_and_trace(lib):
     info = bb.Handle(inst, tree=tree).plan_query()
     assert info["n_gemm_tiled"] == 2 and info["n_permute"] >= 2 and info["n_trace"] == 1
     assert info["n_nodes"] == inst.n_edges + inst.n_vertices - 1
+
+
+def test_local_plan_query_and_sweep_order_hints_on_host(lib):
+    # bbtn_local_plan_query / bbtn_add_sweep_order need no device: a King's subgraph whose sweep is wider than the threshold
+    # gets sliced stretches with small local fixed sets; a hinted order is validated and can only make the plan cheaper
+    k = I.kings_subgraph(14, 14, 0.8, 5)
+    h = bb.Handle(k)
+    wide = h.local_plan_query(30)
+    assert wide["sliced_stretches"] == 0 and wide["branches_planned"] == 1 and wide["max_fixed"] == 0
+    q = h.local_plan_query(wide["max_rank"] - 2)
+    assert q["sliced_stretches"] >= 1 and 1 <= q["max_fixed"] <= 24 and q["max_rank"] <= wide["max_rank"] - 2
+    assert q["branches_planned"] > q["stretches"] - q["sliced_stretches"] and q["bytes"] > 0
+    with pytest.raises(bb.BbtnError) as e:
+        h.add_sweep_order(np.zeros(k.n_vertices, np.int32))
+    assert e.value.status == bb.BBTN_EINVAL
+    h.add_sweep_order(I.column_major_order(k))
+    q2 = h.local_plan_query(wide["max_rank"] - 2)
+    assert q2["bytes"] <= q["bytes"] and q2["max_rank"] <= wide["max_rank"] - 2
+    with pytest.raises(bb.BbtnError):
+        h.local_plan_query(0)

@@ -745,7 +745,10 @@ def test_solve_local_kings_large(bb, L, seed, t):
     # oracle's sparse frontier DP (tests/golden/config_goldens.json)
     g = _goldens()[f"config5-shape king {L}x{L} p0.8 seed {seed}"]
     c = int(g["count"])
-    h = bb.Handle(I.kings_subgraph(L, L, 0.8, seed), flags=bb.BBTN_COUNT_CRT)
+    k = I.kings_subgraph(L, L, 0.8, seed)
+    h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT)
+    if seed != 1:
+        h.add_sweep_order(I.column_major_order(k))      # a hint for the tree search: sweeps along the columns as well
     out = h.solve_local(t)
     assert out["energy"] == int(g["energy"]) and out["count"] == c & MASK64, out
     assert out["count_mod"] == (c % bb.BBTN_P1, c % bb.BBTN_P2)
@@ -761,6 +764,7 @@ def test_config5_kings_40x40_exact_size_and_count(bb):
     k = I.kings_subgraph(40, 40, 0.8, 1)
     offs, verts = _grid_regions(40, 40, 4, 4, _king_ids(k, 40, 40))
     h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT)
+    h.add_sweep_order(I.column_major_order(k))
     out = h.solve_local(32, region_offsets=offs, region_vertices=verts, incumbent_hint=int(g["energy"]))
     assert out["energy"] == int(g["energy"]) and out["count"] == c & MASK64, out
     assert bb.crt_combine(out["count"], *out["count_mod"]) == c
