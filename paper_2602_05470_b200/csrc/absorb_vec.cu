@@ -28,6 +28,7 @@ struct AbsorbVecArgs {
   uint32_t addA[32], addB[32];    // per output bit
   uint32_t kA[8], kB[8];          // per summed bit
   int64_t sA, sB, sC, n_tiles;    // batch strides (elements), tiles over all batch entries
+  int b_unit;                     // B's counts are all 0/1: the product of the counts is A's count (Step::b_unit)
   const uint8_t *xs; int nF;      // local slicing: rows [nb][nF] of 0/1 and the strides of the fixed indices
   uint32_t sliceA[24], sliceB[24];
 };
@@ -133,7 +134,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
 #pragma unroll
                 for (int u = 0; u < 4; u++) {
                   const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-                  oplus<R>(acc_e[u], acc_c[u], e4[k][u] + be[ib], R::mul(c4[k].v[u], ldc<R>(bc, ib)));
+                  oplus<R>(acc_e[u], acc_c[u], e4[k][u] + be[ib], p.b_unit ? c4[k].v[u] : R::mul(c4[k].v[u], ldc<R>(bc, ib)));
                 }
               }
             }
@@ -146,7 +147,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
 #pragma unroll
               for (int u = 0; u < 4; u++) {
                 const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-                oplus<R>(acc_e[u], acc_c[u], ex[u] + be[ib], R::mul(cx.v[u], ldc<R>(bc, ib)));
+                oplus<R>(acc_e[u], acc_c[u], ex[u] + be[ib], p.b_unit ? cx.v[u] : R::mul(cx.v[u], ldc<R>(bc, ib)));
               }
             }
           }
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
               // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
               const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
               const uint32_t ib = tbo[j] + fbf + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-              oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], R::mul(c8[idx >> 2].v[idx & 3], ldc<R>(bc, ib)));
+              oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], p.b_unit ? c8[idx >> 2].v[idx & 3] : R::mul(c8[idx >> 2].v[idx & 3], ldc<R>(bc, ib)));
             }
           }
           V4<CT> oc;
@@ -227,6 +228,7 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
   p.sA = (s.vA && !s.xA) ? ((int64_t)1 << s.rA) : 0;
   p.sB = (s.vB && !s.xB) ? ((int64_t)1 << s.rB) : 0;
   p.sC = (int64_t)1 << s.rO;
+  p.b_unit = s.b_unit;
   p.xs = xs; p.nF = xs ? s.n_slice : 0;
   for (int j = 0; j < 24; j++) { p.sliceA[j] = s.sliceA[j]; p.sliceB[j] = s.sliceB[j]; }
   p.n_tiles = nb << (rOe - p.tb);

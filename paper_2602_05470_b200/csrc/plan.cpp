@@ -449,6 +449,7 @@ struct Planner {
       st.rA = rA; st.rB = rB;
       st.n_slice = (int32_t)std::max(A.slice.size(), B.slice.size());
       st.xA = A.ext ? 1 : 0; st.xB = B.ext ? 1 : 0;
+      st.b_unit = B.lc == 0 ? 1 : 0;
       for (size_t j = 0; j < A.slice.size(); j++) st.sliceA[j] = A.slice[j];
       for (size_t j = 0; j < B.slice.size(); j++) st.sliceB[j] = B.slice[j];
       st.fma = fma;

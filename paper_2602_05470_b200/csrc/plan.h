@@ -61,6 +61,10 @@ struct Step {
   // upper bound on log2(count + 1) of BOTH operands (inputs hold counts 0/1, each (.) adds the operands' bounds,
   // each (+) over 2^k terms adds k): lets K3 pick its narrow count modes inside a tree; 64 = no useful bound
   int32_t count_bits = 64;
+  // every count of operand B is 0 or 1 (B is built from input tensors only, nothing summed yet): the count product is
+  // then the count of A -- the streaming kernels skip the multiply and the load of B's counts.  (A zero element of B has
+  // energy -inf, which makes the term lose against any finite term or be canonicalised away, whatever count it carries.)
+  int32_t b_unit = 0;
   // local slicing (make_local_plan): an operand that is a view of a stored tensor starts at
   // off + sum_j x_j * slice[j], x = the current assignment of the segment's fixed indices
   int32_t n_slice = 0;
