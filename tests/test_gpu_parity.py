@@ -756,12 +756,13 @@ def test_solve_local_kings_large(bb, L, seed, t):
     h.close()
 
 
-def test_config5_kings_40x40_exact_size_and_count(bb):
-    # BASELINE configs[4]: MIS on the King's subgraph 40x40, filling 0.8, unit weights: exact size and count (1.1e32,
-    # so all three residues are needed) by local branching, with K5 region bounds on every branch
-    g = _goldens()["config5 king 40x40 p0.8 seed 1"]
+@pytest.mark.parametrize("seed", [1, 2])
+def test_config5_kings_40x40_exact_size_and_count(bb, seed):
+    # BASELINE configs[4]: MIS on the King's subgraph 40x40, filling 0.8, unit weights: exact size and count (1.1e32 for
+    # seed 1, so all three residues are needed) by local branching, with K5 region bounds on every branch
+    g = _goldens()[f"config5 king 40x40 p0.8 seed {seed}"]
     c = int(g["count"])
-    k = I.kings_subgraph(40, 40, 0.8, 1)
+    k = I.kings_subgraph(40, 40, 0.8, seed)
     offs, verts = _grid_regions(40, 40, 4, 4, _king_ids(k, 40, 40))
     h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT)
     h.add_sweep_order(I.column_major_order(k))
