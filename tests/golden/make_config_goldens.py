@@ -42,6 +42,7 @@ SPARSE_CASES = [
     ("config5-shape king 36x36 p0.8 seed 2", lambda: I.kings_subgraph(36, 36, 0.8, 2)),
     ("config5-shape king 36x36 p0.8 seed 3", lambda: I.kings_subgraph(36, 36, 0.8, 3)),
     ("config5 king 40x40 p0.8 seed 2", lambda: I.kings_subgraph(40, 40, 0.8, 2)),
+    ("config5 king 40x40 p0.8 seed 3", lambda: I.kings_subgraph(40, 40, 0.8, 3)),
 ]
 
 
