@@ -188,14 +188,13 @@ template <class F> void parallel_for(size_t n, F fn) {
 // Candidate trees: the caller's tree if there is one; else elimination trees along the vertex-id order, the
 // min-degree order and nested-min-cut sweeps with several look-ahead windows (plan.cpp).  The driver plans
 // every candidate and keeps the cheapest one that fits.
-void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out) {
+void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out, const std::vector<int> &deltas, bool plain_orders) {
   const Problem &P0 = h->P;
   if (!P0.tree_l.empty() || P0.n + P0.m <= 1) { out.push_back(std::make_unique<Problem>(P0)); return; }
   std::vector<std::vector<int>> orders;
   std::vector<int> natural(P0.n);
   for (int v = 0; v < P0.n; v++) natural[v] = v;
-  orders.push_back(natural);
-  orders.push_back(min_degree_order(P0, {}));
+  if (plain_orders) { orders.push_back(natural); orders.push_back(min_degree_order(P0, {})); }
   int w0 = 0; double c0 = 0;
   { std::vector<int32_t> l, r; elimination_tree_for_order(P0, {}, natural, l, r, w0, c0); }
   // base orders of the nested-min-cut sweeps: the vertex ids, the caller's hints (bbtn_add_sweep_order), and each reversed
@@ -204,21 +203,22 @@ void candidate_trees(bbtn_handle *h, std::vector<std::unique_ptr<Problem>> &out)
   for (auto &o : h->sweep_orders) bases.push_back(o);
   const size_t nb0 = bases.size();
   for (size_t i = 0; i < nb0; i++) bases.push_back(std::vector<int>(bases[i].rbegin(), bases[i].rend()));
-  struct Job { size_t base; int half; };
+  struct Job { size_t base; int half, delta; };
   std::vector<Job> jobs;
   std::vector<int> widths(bases.size(), w0);
-  for (size_t i = 1; i < bases.size(); i++) orders.push_back(bases[i]);
+  if (plain_orders) for (size_t i = 1; i < bases.size(); i++) orders.push_back(bases[i]);
   parallel_for(bases.size(), [&](size_t i) {                            // the look-ahead windows scale with each sweep's width
     if (i == 0) return;
     std::vector<int32_t> l, r; double c = 0;
     elimination_tree_for_order(P0, {}, bases[i], l, r, widths[i], c);
   });
   for (size_t i = 0; i < bases.size(); i++)
-    for (int half : {4, 6, 8, 9, 10, 11, 12, 14, 16}) jobs.push_back({i, half});   // windows of 2 .. 8 sweep widths
+    for (int delta : deltas)
+      for (int half : {4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 16}) jobs.push_back({i, half, delta});   // windows of 2 .. 8 sweep widths
   const size_t first_job = orders.size();
   orders.resize(first_job + jobs.size());
   parallel_for(jobs.size(), [&](size_t j) {
-    orders[first_job + j] = mincut_sweep_order(P0, 4, std::max(8, jobs[j].half * widths[jobs[j].base] / 2), &bases[jobs[j].base]);
+    orders[first_job + j] = mincut_sweep_order(P0, jobs[j].delta, std::max(8, jobs[j].half * widths[jobs[j].base] / 2), &bases[jobs[j].base]);
   });
   out.resize(orders.size());
   parallel_for(orders.size(), [&](size_t i) {
@@ -252,7 +252,8 @@ int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, Loca
     return BBTN_OK;
   }
   std::vector<std::unique_ptr<Problem>> cands;
-  candidate_trees(h, cands);
+  candidate_trees(h, cands, {4}, true);
+  bool widened = !h->P.tree_l.empty();                        // a caller's tree is the only candidate
   std::string last_err; int last_rc = BBTN_ESHAPE;
   for (int cap = log2_target; cap >= 1; cap--) {
     std::vector<LocalPlan> plans(cands.size());
@@ -264,6 +265,24 @@ int plan_within_budget(bbtn_handle *h, int32_t log2_target, int64_t budget, Loca
       if (rcs[i]) { last_rc = rcs[i]; last_err = errs[i]; continue; }
       if (budget > 0 && (plans[i].plan.arena_invariant_elems + plans[i].plan.arena_variant_elems) * per_elem > budget) { last_rc = BBTN_ENOMEM; last_err = "arena does not fit the device-memory budget"; continue; }
       if (best < 0 || plans[i].bytes_total < plans[best].bytes_total) best = (int)i;
+    }
+    if (best >= 0 && !widened && plans[best].bytes_total > 1e14) {
+      // an expensive plan (seconds of streaming): the cost of a plan is erratic in the details of the sweep, so it pays to
+      // look at more of them -- the same bases and windows with other round sizes of the min-cut sweep
+      widened = true;
+      std::vector<std::unique_ptr<Problem>> more;
+      candidate_trees(h, more, {2, 8, 16}, false);
+      std::vector<LocalPlan> plans2(more.size());
+      std::vector<int> rc2(more.size(), 0);
+      std::vector<std::string> err2(more.size());
+      parallel_for(more.size(), [&](size_t i) { rc2[i] = make_local_plan(*more[i], cap, plans2[i], err2[i]); });
+      int b2 = -1;
+      for (size_t i = 0; i < more.size(); i++) {
+        if (rc2[i] || (budget > 0 && (plans2[i].plan.arena_invariant_elems + plans2[i].plan.arena_variant_elems) * per_elem > budget)) continue;
+        if (plans2[i].bytes_total < plans[best].bytes_total && (b2 < 0 || plans2[i].bytes_total < plans2[b2].bytes_total)) b2 = (int)i;
+      }
+      if (b2 >= 0) { plans[best] = std::move(plans2[b2]); cands[best] = std::move(more[b2]); }
+      for (auto &m : more) if (m) cands.push_back(std::move(m));     // keep them for lower thresholds, should this one not be final
     }
     if (best >= 0) {
       lp = std::move(plans[best]); P_out = std::move(cands[best]);
