@@ -203,7 +203,7 @@ bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void 
   if (s.rO < 4 || s.nK > 3 || s.rA < 3) return false;
   if (xs) for (int j = 0; j < s.n_slice; j++) if (s.sliceA[j] & 3u) return false;   // a slice would break the 16-byte reads of A
   if (!al16(Ae) || !al16(Ce) || (ring != RING_NONE && (!al16(Ac) || !al16(Cc)))) return false;
-  if (ring == RING_U64 && (!al32(Ac) || !al32(Cc))) return false;       // 32-byte count vectors
+  if (ring_count_bytes(ring) == 8 && (!al32(Ac) || !al32(Cc))) return false;       // 32-byte count vectors
   int lp;
   if (s.addA[0] == 1u && s.addA[1] == 2u) {
     lp = LP_FAR;

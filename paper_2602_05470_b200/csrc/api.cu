@@ -184,7 +184,7 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
   const Plan &pl = dp->plan;
   int32_t *ve = (int32_t *)dp->var_e.p, *ie = (int32_t *)dp->inv_e.p;
   char *vc = (char *)dp->var_c.p, *ic = (char *)dp->inv_c.p;
-  const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
+  const size_t csz = ring_count_bytes(ring);
   launch_construct(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_var.p, dp->n_var,
                    (const int32_t *)dp->list_inv.p, dp->n_inv, (const int32_t *)dp->list_scalar.p, dp->n_scalar,
                    d_assign, (int)pl.fixed.size(), B, ve, vc, ie, ic, (int32_t *)dp->off_e.p, dp->off_c.p, ring, st);
@@ -356,8 +356,13 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
     }
   }
   const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;
-  const int n_rings = search ? 1 : ((crt && d_mod) ? 3 : 1);
-  const int ring0 = search ? (int)RING_NONE : (int)RING_U64;
+  // CRT mode: the two prime rings run as ONE pass (both residues in one 64-bit count) unless the plan holds a
+  // permute or tiled-GEMM step, whose kernels exist for the single-prime rings only
+  bool stream_only = true;
+  for (const Step &s : dp->plan.steps) if (s.kind == STEP_PERMUTE || s.kind == STEP_GEMM) stream_only = false;
+  int rings[3] = {search ? (int)RING_NONE : (int)RING_U64, RING_P1, RING_P2};
+  int n_rings = 1;
+  if (!search && crt && d_mod) { if (stream_only) { rings[1] = RING_P12; n_rings = 2; } else n_rings = 3; }
   const bool use_graph = allow_graph && !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
   if (dp->fused == 1) {
     const Plan &pl = dp->plan;
@@ -365,9 +370,9 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
       launch_fused_tree(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_build.p, dp->n_build,
                         (const int32_t *)dp->list_scalar.p, dp->n_scalar, d_assign, n_fixed, B, (const FusedStep *)dp->fused_steps.p,
                         (int)pl.steps.size(), dp->fused_arena, (int)pl.arena_variant_elems, (int)pl.result_offset,
-                        d_energy, d_count, d_mod, ring0 + ring, st);
+                        d_energy, d_count, d_mod, rings[ring], st);
   } else if (!use_graph) {
-    for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring0 + ring, st);
+    for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, rings[ring], st);
   } else {
     const void *io[4] = {d_assign, d_energy, d_count, d_mod};
     const bool stale = dp->graph_B != B || (int)dp->graphs.size() != n_rings || std::memcmp(io, dp->graph_io, sizeof(io)) != 0;
@@ -380,7 +385,7 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
       for (int ring = 0; ring < n_rings && ce == cudaSuccess; ring++) {
         cudaGraph_t g = nullptr; cudaGraphExec_t ge = nullptr;
         if ((ce = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal)) != cudaSuccess) break;
-        enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, ring0 + ring, cs);
+        enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, rings[ring], cs);
         ce = cudaStreamEndCapture(cs, &g);          // always ends the capture, also after a failed launch
         if (ce == cudaSuccess) ce = cudaGraphInstantiate(&ge, g, 0);
         if (g) cudaGraphDestroy(g);

@@ -123,6 +123,8 @@ __global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const Input
     } else if (ring == 0) {
       energy[b] = zero ? NEG_INF : (kind == 0 ? -e : e);
       count[b] = (uint64_t)c;
+    } else if (ring == RING_P12) {
+      if (count_mod) { count_mod[2 * b] = (uint32_t)c; count_mod[2 * b + 1] = (uint32_t)((uint64_t)c >> 32); }
     } else if (count_mod) {
       count_mod[2 * b + (ring - 1)] = (uint32_t)c;
     }
@@ -132,7 +134,7 @@ __global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const Input
 }  // namespace
 
 size_t fused_tree_smem_bytes(int arena_elems, int ring) {
-  const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
+  const size_t csz = ring_count_bytes(ring);
   return 2 * sizeof(FusedStep) + (((size_t)arena_elems * 4 + 15) & ~(size_t)15) + (size_t)arena_elems * csz + 16;
 }
 

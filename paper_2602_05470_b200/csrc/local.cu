@@ -63,7 +63,7 @@ struct LocalRun {
     const Plan &pl = lp->plan;
     int32_t *ve = (int32_t *)var_e.p, *ie = (int32_t *)inv_e.p;
     char *vc = (char *)var_c.p, *ic = (char *)inv_c.p;
-    const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
+    const size_t csz = ring_count_bytes(ring);
     // a view (x) and an invariant tensor live in the invariant arena; a variant tensor is [nb][2^rank] at off * nb
     auto pe = [&](int v, int x, int64_t off) { return (v && !x) ? ve + off * nb : ie + off; };
     auto pc = [&](int v, int x, int64_t off) { return (void *)((v && !x) ? vc + (size_t)off * nb * csz : ic + (size_t)off * csz); };
@@ -87,7 +87,7 @@ struct LocalRun {
     const int kind = P->kind;
     int32_t *ve = (int32_t *)var_e.p, *ie = (int32_t *)inv_e.p;
     char *vc = (char *)var_c.p, *ic = (char *)inv_c.p;
-    const size_t csz = ring == RING_U64 ? 8 : (ring == RING_NONE ? 0 : 4);
+    const size_t csz = ring_count_bytes(ring);
     const InputRec *d_in = (const InputRec *)inputs.p;
     const int32_t *d_l = (const int32_t *)lists.p;
     int32_t *oe = (int32_t *)off_e.p; char *oc = (char *)off_c.p;
@@ -355,13 +355,15 @@ int bbtn_solve_local(bbtn_handle *h, int32_t log2_target, int64_t mem_budget_byt
   run.have_inc = incumbent_hint != BBTN_NEG_INF; run.inc = incumbent_hint;
   if ((rc = run.upload())) return rc;
   const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;
-  const int n_rings = search ? 1 : ((crt && count_mod) ? 3 : 1);
+  // CRT mode: a second pass with both prime residues packed in one 64-bit count (the plan has streaming steps only)
+  const int n_rings = search ? 1 : ((crt && count_mod) ? 2 : 1);
+  const int rings[2] = {search ? (int)RING_NONE : (int)RING_U64, (int)RING_P12};
   for (int ring = 0; ring < n_rings; ring++)
-    if ((rc = run.run_ring(search ? (int)RING_NONE : ring, (int32_t *)run.res_e.p, (uint64_t *)run.res_c.p, (uint32_t *)run.res_m.p))) return rc;
+    if ((rc = run.run_ring(rings[ring], (int32_t *)run.res_e.p, (uint64_t *)run.res_c.p, (uint32_t *)run.res_m.p))) return rc;
   int32_t e; uint64_t c; uint32_t cm[2] = {0, 0};
   CUDA_TRY(h, cudaMemcpyAsync(&e, run.res_e.p, 4, cudaMemcpyDeviceToHost, run.st));
   CUDA_TRY(h, cudaMemcpyAsync(&c, run.res_c.p, 8, cudaMemcpyDeviceToHost, run.st));
-  if (n_rings == 3) CUDA_TRY(h, cudaMemcpyAsync(cm, run.res_m.p, 8, cudaMemcpyDeviceToHost, run.st));
+  if (n_rings == 2) CUDA_TRY(h, cudaMemcpyAsync(cm, run.res_m.p, 8, cudaMemcpyDeviceToHost, run.st));
   CUDA_TRY(h, cudaStreamSynchronize(run.st));
   *energy = e; *count = c;
   if (count_mod) { count_mod[0] = cm[0]; count_mod[1] = cm[1]; }

@@ -50,6 +50,21 @@ struct RingNone {
 using RingP1 = RingMod<2147483647u>;
 using RingP2 = RingMod<2147483629u>;
 
+// Both primes at once (CRT mode, streaming and fused kernels): the residue mod P1 in the low word and the residue
+// mod P2 in the high word of one 64-bit count, so the two prime passes share one read of the energy planes.
+struct RingP12 {
+  using T = uint64_t;
+  static constexpr bool kCounts = true;
+  static __device__ __forceinline__ T pack(uint32_t r1, uint32_t r2) { return (uint64_t)r1 | ((uint64_t)r2 << 32); }
+  static __device__ __forceinline__ T mul(T a, T b) {
+    return pack(RingP1::mul((uint32_t)a, (uint32_t)b), RingP2::mul((uint32_t)(a >> 32), (uint32_t)(b >> 32)));
+  }
+  static __device__ __forceinline__ T add(T a, T b) {
+    return pack(RingP1::add((uint32_t)a, (uint32_t)b), RingP2::add((uint32_t)(a >> 32), (uint32_t)(b >> 32)));
+  }
+  static __device__ __forceinline__ T from_small(uint32_t x) { return pack(RingP1::from_small(x), RingP2::from_small(x)); }
+};
+
 constexpr int32_t NEG_INF = -(1 << 30);
 constexpr int32_t ZERO_BELOW = -(1 << 29);
 
@@ -95,5 +110,6 @@ __device__ __forceinline__ void canonicalise(int32_t &e, typename R::T &c) {
     if ((ring) == 0) { using R = ::bbtn::RingU64; __VA_ARGS__; }        \
     else if ((ring) == 1) { using R = ::bbtn::RingP1; __VA_ARGS__; }    \
     else if ((ring) == 2) { using R = ::bbtn::RingP2; __VA_ARGS__; }    \
+    else if ((ring) == 4) { using R = ::bbtn::RingP12; __VA_ARGS__; }   \
     else { using R = ::bbtn::RingNone; __VA_ARGS__; }                   \
   } while (0)
