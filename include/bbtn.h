@@ -150,6 +150,28 @@ int bbtn_region_bound(bbtn_handle *h,
                       const uint8_t *assign, int64_t B,
                       int32_t *bound, void *cuda_stream);
 
+/* bbtn_region_bound for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same bound, same kernels (K5), but
+ *   - `assign` [B][n_fixed] and `bound` [B] are DEVICE pointers whatever the handle's flags say;
+ *   - the per-(leaf, region) maxima go to a file-scope device array of BBTN_REGION_BOUND_STATIC_MAX_ITEMS int32
+ *     (4 MiB, held by every GPU that loads the library until the process exits) instead of a handle buffer:
+ *     B * max(n_regions, 1) beyond that is refused with BBTN_ESHAPE;
+ *   - the K5 tables of (regions, fixed_vertices) must already be cached in the handle by an earlier ordinary
+ *     bbtn_region_bound call with the same regions and fixed vertices (set-up; the cache holds 64 signatures): if they
+ *     are not, the call fails with BBTN_EINVAL instead of building (and allocating) them.
+ * The call allocates and frees no device memory, copies nothing, does not synchronise: it launches the two K5 kernels
+ * on `cuda_stream` and returns.  B = 0 is the set-up call: it checks the tables and resolves the array's device address
+ * for the current device (also done by the first real call on each device) and launches nothing.
+ * Every call on a GPU shares the one array, which keeps the last call's contents (every entry a call reads it has
+ * written first, so nothing is cleared): calls that OVERLAP on the GPU (different streams) race and return garbage;
+ * calls on one stream are safe.  Errors: EINVAL, ESHAPE, ECUDA. */
+#define BBTN_REGION_BOUND_STATIC_MAX_ITEMS (1 << 20)
+int bbtn_region_bound_static(bbtn_handle *h,
+                             const int32_t *region_offsets, const int32_t *region_vertices, int32_t n_regions,
+                             const int32_t *fixed_vertices, int32_t n_fixed,
+                             const uint8_t *assign_device, int64_t B,
+                             int32_t *bound_device, void *cuda_stream);
+
 /* Host branch-and-bound driver (global pruning :67; S6): depth-first
  * over `branch_vertices` in the given order, `chunk` levels at a time; every partial assignment is
  * bounded with bbtn_region_bound and discarded iff its bound is strictly worse than the incumbent

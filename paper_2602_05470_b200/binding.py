@@ -23,7 +23,7 @@ BBTN_COUNT_CRT, BBTN_IO_DEVICE, BBTN_NO_GRAPH = 0x1, 0x2, 0x4
 BBTN_FORCE_STREAMING, BBTN_FORCE_TILED, BBTN_SEARCH_ONLY, BBTN_NO_FUSED = 0x10, 0x20, 0x40, 0x80
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
-EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query", "bbtn_add_sweep_order",
+EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_region_bound_static", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query", "bbtn_add_sweep_order",
            "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
            "bbtn_permute_batched", "bbtn_int32_microbench", "bbtn_crt_combine", "bbtn_set_debug_checks",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
@@ -64,6 +64,7 @@ def load():
     lib.bbtn_contract_batch.argtypes = [vp, vp, i32, vp, i64, vp, vp, vp, vp]
     lib.bbtn_plan_query.argtypes = [vp, vp, i32, i64, C.POINTER(_PlanInfo)]
     lib.bbtn_region_bound.argtypes = [vp, vp, vp, i32, vp, i32, vp, i64, vp, vp]
+    lib.bbtn_region_bound_static.argtypes = [vp, vp, vp, i32, vp, i32, vp, i64, vp, vp]
     lib.bbtn_solve_bb.argtypes = [vp, vp, i32, i32, vp, vp, i32, i64, i32, i32, vp, vp, vp, vp, vp]
     lib.bbtn_solve_branching.argtypes = [vp, i32, i64, i64, vp, vp, vp, vp, vp, vp]
     lib.bbtn_branching_leaves.argtypes = [vp, i32, i64, i64, i64, i64, vp, vp, vp, vp, vp]
@@ -185,6 +186,15 @@ class Handle:
         fx = np.zeros(0, np.int32) if fixed is None else _np(fixed, np.int32)
         _check(load().bbtn_region_bound(self._h, _ptr(ro), _ptr(rv), len(ro) - 1, _ptr(fx), len(fx), _ptr(assign_t),
                                         int(bound_t.shape[0]), _ptr(bound_t), _stream(stream)), self._h)
+
+    # -- bbtn_region_bound_static: no device allocation; device tensors whatever the handle's flags; B = 0 is the set-up call
+    def region_bound_static(self, region_offsets, region_vertices, fixed, assign_t, bound_t, B: int | None = None, stream=None):
+        ro, rv = _np(region_offsets, np.int32), _np(region_vertices, np.int32)
+        fx = np.zeros(0, np.int32) if fixed is None else _np(fixed, np.int32)
+        if B is None:
+            B = int(bound_t.shape[0])
+        _check(load().bbtn_region_bound_static(self._h, _ptr(ro), _ptr(rv), len(ro) - 1, _ptr(fx), len(fx), _ptr(assign_t),
+                                               B, _ptr(bound_t), _stream(stream)), self._h)
 
     def solve_bb(self, branch_vertices, chunk, region_offsets, region_vertices, max_batch=1024,
                  incumbent_hint=BBTN_NEG_INF, use_pruning=True, stream=None):

@@ -7,6 +7,7 @@
 // region u F, plus the best entry of every term no region covers, plus the fixed-fixed terms.
 // One warp per (leaf, region): the lanes enumerate the 2^nf region configurations and the
 // maximum is taken with a warp-wide integer reduction (REDUX).
+#include "../../include/bbtn.h"
 #include "kernels.h"
 #include "ring.cuh"
 
@@ -98,6 +99,32 @@ void launch_region_bound(const BoundTables &t, const uint8_t *d_assign, int64_t 
   int64_t g = (B + 127) / 128;
   if (g > 148 * 8) g = 148 * 8;
   bound_sum_kernel<<<(unsigned)g, 128, 0, st>>>(t, d_assign, B, region_scratch, bound);
+}
+
+// ---- the no-allocation variant (include/bbtn.h: bbtn_region_bound_static) ----------------------------------------
+// The per-(leaf, region) maxima go to a file-scope device array instead of a buffer the handle allocates.  Every GPU
+// that loads the library holds these 4 MiB until the process exits.  Every call shares the array and finds the last
+// call's contents in it: region_max_kernel writes all B * n_regions entries before bound_sum_kernel reads them (same
+// stream), so nothing needs clearing -- but two calls that overlap on the GPU (different streams) race on it.
+static __device__ __align__(256) int32_t g_region_scratch[BBTN_REGION_BOUND_STATIC_MAX_ITEMS];
+
+// In host code the name g_region_scratch is a stand-in, not a device address: ask the runtime, once per device, with
+// that device current.
+int launch_region_bound_static(const BoundTables &t, const uint8_t *d_assign, int64_t B, int32_t *bound, cudaStream_t st,
+                               cudaError_t *cuda_err) {
+  constexpr int MAX_DEV = 64;
+  static int32_t *addr[MAX_DEV] = {};
+  *cuda_err = cudaSuccess;
+  int dev = -1;
+  if ((*cuda_err = cudaGetDevice(&dev)) != cudaSuccess) return 1;
+  if (dev < 0 || dev >= MAX_DEV) return 2;
+  if (!addr[dev]) {
+    int32_t *ptr = nullptr;
+    if ((*cuda_err = cudaGetSymbolAddress((void **)&ptr, g_region_scratch)) != cudaSuccess || !ptr) return 1;
+    addr[dev] = ptr;
+  }
+  if (B > 0) launch_region_bound(t, d_assign, B, addr[dev], bound, st);      // B = 0: set-up only
+  return 0;
 }
 
 }  // namespace bbtn

@@ -210,6 +210,35 @@ int bbtn_region_bound(bbtn_handle *h, const int32_t *region_offsets, const int32
   return BBTN_OK;
 }
 
+int bbtn_region_bound_static(bbtn_handle *h, const int32_t *region_offsets, const int32_t *region_vertices, int32_t n_regions,
+                             const int32_t *fixed, int32_t n_fixed, const uint8_t *assign, int64_t B, int32_t *bound, void *stream) {
+  if (!h) return fail(nullptr, BBTN_EINVAL, "null handle");
+  if (B < 0 || (B > 0 && !bound) || n_regions < 0 || n_fixed < 0 || (n_regions > 0 && (!region_offsets || !region_vertices)) ||
+      (n_fixed > 0 && (!fixed || (B > 0 && !assign))))
+    return fail(h, BBTN_EINVAL, "bad region_bound_static arguments");
+  if ((double)B * (double)std::max(n_regions, 1) > (double)BBTN_REGION_BOUND_STATIC_MAX_ITEMS)
+    return fail(h, BBTN_ESHAPE, "bbtn_region_bound_static: B * n_regions = " + std::to_string(B) + " * " + std::to_string(std::max(n_regions, 1)) +
+                                    " exceeds the static scratch of " + std::to_string(BBTN_REGION_BOUND_STATIC_MAX_ITEMS) +
+                                    " entries; split the batch or use bbtn_region_bound");
+  if (!have_device()) return fail(h, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  // look the tables up, never build them (building uploads = allocates)
+  std::vector<int32_t> key;
+  key.push_back(n_regions);
+  if (n_regions > 0) { key.insert(key.end(), region_offsets, region_offsets + n_regions + 1); key.insert(key.end(), region_vertices, region_vertices + region_offsets[n_regions]); }
+  key.push_back(-1);
+  key.insert(key.end(), fixed, fixed + n_fixed);
+  auto it = h->bounds.find(key);
+  if (it == h->bounds.end())
+    return fail(h, BBTN_EINVAL, "bbtn_region_bound_static: no cached tables for these regions and fixed vertices; call bbtn_region_bound with them once first");
+  cudaError_t ce = cudaSuccess;
+  // B = 0: set-up only (the launcher resolves the array's address for this device and launches nothing)
+  const int rc = launch_region_bound_static(it->second->t, assign, B, bound, (cudaStream_t)stream, &ce);
+  if (rc == 2) return fail(h, BBTN_ECUDA, "bbtn_region_bound_static: device ordinal beyond 63");
+  if (rc) return fail(h, BBTN_ECUDA, std::string("bbtn_region_bound_static: ") + cudaGetErrorString(ce));
+  CUDA_TRY(h, cudaGetLastError());
+  return BBTN_OK;
+}
+
 int bbtn_oplus_combine(int32_t kind, int64_t n, const int32_t *energy, const uint64_t *count, const uint32_t *count_mod,
                        int32_t *out_energy, uint64_t *out_count, uint32_t *out_count_mod) {
   if ((kind != BBTN_ISING && kind != BBTN_MIS) || n < 0 || (n > 0 && (!energy || !count)) || !out_energy || !out_count ||

@@ -101,6 +101,10 @@ struct BoundTables {                 // device CSR tables built once per (region
 };
 void launch_region_bound(const BoundTables &t, const uint8_t *d_assign, int64_t B, int32_t *region_scratch,
                          int32_t *bound, cudaStream_t st);
+// the same with the region scratch in a file-scope device array (bound.cu); 0 = launched, 1 = CUDA error (*cuda_err),
+// 2 = device ordinal out of range
+int launch_region_bound_static(const BoundTables &t, const uint8_t *d_assign, int64_t B, int32_t *bound, cudaStream_t st,
+                               cudaError_t *cuda_err);
 
 // register-only integer microbenchmarks (include/bbtn.h: bbtn_int32_microbench)
 int run_microbench(int which, int iters, double *ms, double *ops, cudaStream_t st);
