@@ -70,7 +70,7 @@ typedef enum {
 #define BBTN_SEARCH_ONLY     0x40u /* ground-state SEARCH ("the tropical number inf for optimization problems",
                                       :81-91): plain max-plus, no count plane anywhere (4 B per element instead of 12);
                                       the batched calls and the solve drivers return the optimal energy only, every
-                                      count output reads 0 and `count` may be NULL.  Excludes BBTN_COUNT_CRT / FORCE_TILED */
+                                      count output reads 0 and `count` may be NULL.  Excludes BBTN_COUNT_CRT */
 
 #define BBTN_P1 2147483647u   /* 2^31 - 1  */
 #define BBTN_P2 2147483629u   /* 2^31 - 19 */
@@ -316,6 +316,22 @@ int bbtn_tropical_gemm_batched_host(int64_t batch, int32_t M, int32_t N, int32_t
                                     int32_t *Ce, uint64_t *Cc,
                                     int64_t strideA, int64_t strideB, int64_t strideC,
                                     int32_t count_bits, int32_t energy_bits, void *cuda_stream);
+
+/* K3 of the SEARCH mode alone (PAPER.md:55 "the tropical number inf for optimization problems", :81-91; Eq. 2
+ * evaluated pairwise, :51, :57, in the max-plus semiring without counts):
+ *   C[b][m][n] = max_k ( A[b][m][k] + B[b][k][n] ),   energies int32, row-major, DEVICE pointers,
+ * strides in elements between batch entries (0 = operand shared by the whole batch).  The zero element is
+ * BBTN_NEG_INF: any energy below -2^29 is read as zero, a sum that involves a zero is zero, outputs are canonical
+ * (exactly BBTN_NEG_INF).  Finite energies must lie within +-BBTN_ENERGY_LIMIT.
+ *   energy_bits  1..32, the caller's PROMISE that every finite operand energy is below 2^energy_bits in magnitude;
+ *                <= 11 selects the packed form (two 16-bit add-max per integer instruction), anything else the
+ *                32-bit form; results do not depend on it when the promise holds (checked on the device when
+ *                bbtn_set_debug_checks is on).
+ * Asynchronous on cuda_stream.  Errors: EINVAL, ESHAPE (more than 2^31-1 thread blocks), ECUDA. */
+int bbtn_maxplus_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,
+                              const int32_t *A, const int32_t *B, int32_t *C,
+                              int64_t strideA, int64_t strideB, int64_t strideC,
+                              int32_t energy_bits, void *cuda_stream);
 
 /* Raw batched bit permutation (K2 alone): dst[b][pi(i)] = src[b][i] for i in [0, 2^rank), where
  * bit j of pi(i) is bit perm[j] of i (perm is a HOST array, a permutation of 0..rank-1).

@@ -24,7 +24,7 @@ BBTN_FORCE_STREAMING, BBTN_FORCE_TILED, BBTN_SEARCH_ONLY, BBTN_NO_FUSED = 0x10, 
 BBTN_P1, BBTN_P2 = 2147483647, 2147483629
 
 EXPORTS = ["bbtn_build", "bbtn_contract_batch", "bbtn_plan_query", "bbtn_region_bound", "bbtn_region_bound_static", "bbtn_solve_bb", "bbtn_solve_branching", "bbtn_branching_leaves", "bbtn_solve_local", "bbtn_local_plan_query", "bbtn_add_sweep_order",
-           "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_oplus_combine",
+           "bbtn_tropical_gemm_batched", "bbtn_tropical_gemm_batched_host", "bbtn_maxplus_gemm_batched", "bbtn_oplus_combine",
            "bbtn_permute_batched", "bbtn_int32_microbench", "bbtn_crt_combine", "bbtn_set_debug_checks",
            "bbtn_destroy", "bbtn_last_error", "bbtn_version"]
 
@@ -72,6 +72,7 @@ def load():
     lib.bbtn_local_plan_query.argtypes = [vp, i32, i64, vp, vp]
     lib.bbtn_add_sweep_order.argtypes = [vp, vp]
     lib.bbtn_tropical_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, i32, vp]
+    lib.bbtn_maxplus_gemm_batched.argtypes = [i64, i32, i32, i32, vp, vp, vp, i64, i64, i64, i32, vp]
     lib.bbtn_tropical_gemm_batched_host.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp, i64, i64, i64, i32, i32, vp]
     lib.bbtn_oplus_combine.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
     lib.bbtn_permute_batched.argtypes = [i32, vp, i64, vp, vp, vp, vp, vp]
@@ -292,6 +293,21 @@ def tropical_gemm_batched(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64
     _check(load().bbtn_tropical_gemm_batched(batch, M, N, K, _ptr(Ae), _ptr(Ac), _ptr(Be), _ptr(Bc), _ptr(Ce), _ptr(Cc),
                                              M * K if a3 else 0, K * N if b3 else 0, M * N, count_bits, energy_bits, _stream(stream)))
     return Ce, Cc
+
+
+def maxplus_gemm_batched(A, B, C=None, energy_bits: int = 32, stream=None):
+    """bbtn_maxplus_gemm_batched on torch CUDA int32 tensors: A [B][M][K] (or [M][K] shared), B [B][K][N] (or [K][N])."""
+    import torch
+    a3, b3 = A.dim() == 3, B.dim() == 3
+    batch = A.shape[0] if a3 else (B.shape[0] if b3 else 1)
+    M, K = A.shape[-2:]
+    N = B.shape[-1]
+    assert B.shape[-2] == K
+    if C is None:
+        C = torch.empty((batch, M, N), dtype=torch.int32, device=A.device)
+    _check(load().bbtn_maxplus_gemm_batched(batch, M, N, K, _ptr(A), _ptr(B), _ptr(C), M * K if a3 else 0, K * N if b3 else 0,
+                                            M * N, energy_bits, _stream(stream)))
+    return C
 
 
 def tropical_gemm_batched_host(Ae, Ac, Be, Bc, Ce=None, Cc=None, count_bits: int = 64, energy_bits: int = 32, stream=None):

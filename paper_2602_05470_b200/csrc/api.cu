@@ -41,7 +41,7 @@ __global__ void check_operand_kernel(const int32_t *__restrict__ e, const uint64
   for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
     const int64_t r = t / row_len, i = r * row_stride + (t - r * row_len);
     const int32_t ee = e[i];
-    if (count_bits < 64 && (c[i] >> count_bits) != 0) bad |= 1;
+    if (count_bits < 64 && c && (c[i] >> count_bits) != 0) bad |= 1;
     if (ee != BBTN_NEG_INF && (ee > energy_limit || ee < -energy_limit)) bad |= 2;
   }
   if (bad) atomicOr(flags, bad);
@@ -264,8 +264,7 @@ int bbtn_build(const bbtn_problem_desc *d, bbtn_handle **out) {
   P.max_elements = d->max_elements_per_leaf > 0 ? d->max_elements_per_leaf : ((int64_t)1 << 28);
   h->force_mode = (d->flags & BBTN_FORCE_STREAMING) ? 1 : ((d->flags & BBTN_FORCE_TILED) ? 2 : 0);
   if (d->flags & BBTN_SEARCH_ONLY) {
-    if (d->flags & (BBTN_COUNT_CRT | BBTN_FORCE_TILED)) return fail(nullptr, BBTN_EINVAL, "BBTN_SEARCH_ONLY excludes BBTN_COUNT_CRT and BBTN_FORCE_TILED");
-    h->force_mode = 1;                                   // the energy-only kernels are the streaming forms
+    if (d->flags & BBTN_COUNT_CRT) return fail(nullptr, BBTN_EINVAL, "BBTN_SEARCH_ONLY excludes BBTN_COUNT_CRT");
   }
   // validate the tree once on the unsliced network
   if (!P.tree_l.empty()) {
@@ -431,6 +430,20 @@ int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, c
   if (g_debug_checks && (rc = check_gemm_operands(batch, M, N, K, Ae, Ac, Be, Bc, strideA, strideB, count_bits, energy_bits, (cudaStream_t)stream))) return rc;
   launch_gemm_tiled(batch, 1, M, N, K, 0, Ae, Ac, Be, Bc, Ce, Cc, strideA, strideB, strideC, RING_U64, count_bits, energy_bits,
                     (cudaStream_t)stream);
+  CUDA_TRY(nullptr, cudaGetLastError());
+  return BBTN_OK;
+}
+
+int bbtn_maxplus_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K, const int32_t *A, const int32_t *B, int32_t *C,
+                              int64_t strideA, int64_t strideB, int64_t strideC, int32_t energy_bits, void *stream) {
+  if (batch < 1 || M < 1 || N < 1 || K < 1 || !A || !B || !C || strideA < 0 || strideB < 0 || strideC < 0)
+    return fail(nullptr, BBTN_EINVAL, "bad GEMM arguments");
+  if (batch > 1 && strideC < (int64_t)M * N) return fail(nullptr, BBTN_EINVAL, "strideC overlaps outputs");
+  int rc = check_gemm_shape(batch, M, N, 1, energy_bits);
+  if (rc) return rc;
+  if (!have_device()) return fail(nullptr, BBTN_ECUDA, "no CUDA device (there is no CPU fallback)");
+  if (g_debug_checks && (rc = check_gemm_operands(batch, M, N, K, A, nullptr, B, nullptr, strideA, strideB, 64, energy_bits, (cudaStream_t)stream))) return rc;
+  launch_gemm_maxplus(batch, 1, M, N, K, 0, A, B, C, strideA, strideB, strideC, energy_bits, (cudaStream_t)stream);
   CUDA_TRY(nullptr, cudaGetLastError());
   return BBTN_OK;
 }

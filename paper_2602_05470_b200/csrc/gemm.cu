@@ -182,6 +182,10 @@ void launch_v1(dim3 grid, cudaStream_t st, int64_t G, int M, int N, int K, const
 void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                        const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc, int32_t *Ce, void *Cc,
                        int64_t sA, int64_t sB, int64_t sC, int ring, int count_bits, int energy_bits, cudaStream_t st) {
+  if (ring == RING_NONE) {                                 // search mode: the energy plane alone (gemm_maxplus.cu)
+    launch_gemm_maxplus(batch, G, M, N, K, a_kmajor, Ae, Be, Ce, sA, sB, sC, energy_bits, st);
+    return;
+  }
   // RING_U64 runs on the 128-row streaming tile of gemm_tiled.cu, except where that tile would be
   // >= 75 % padding (M, N <= 64): there the 64x64 tile below wastes nothing and many CTAs fit per SM.
   if (ring == RING_U64 && (!(M <= BM && N <= BN) || gemm_pack16_eligible(K, count_bits, energy_bits))) {

@@ -58,6 +58,11 @@ void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kma
                         const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
                         int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, cudaStream_t st);
 
+// K3 in search mode (gemm_maxplus.cu): max-plus on the energy planes alone, one fused add-max per FMA (two with
+// energy_bits <= 11: packed 16-bit halves); layout arguments as launch_gemm_tiled.
+void launch_gemm_maxplus(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor, const int32_t *A, const int32_t *B,
+                         int32_t *C, int64_t sA, int64_t sB, int64_t sC, int energy_bits, cudaStream_t st);
+
 // Local slicing: acc (+)= (+)_b offset[b] (.) slice[b], element-wise over n elements, nb slices stored [nb][n]
 // (first = 1: acc is overwritten); the zero tensor when slice_e == nullptr.  offset[b] is one element per slice on the
 // device.  (+) over the assignments of a segment's locally fixed indices (Eq. 3, on a sub-network).

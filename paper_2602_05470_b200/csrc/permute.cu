@@ -10,6 +10,8 @@
 // A CTA gathers the tile spanned by (source-low u destination-low) bits with coalesced,
 // vectorised reads along the source-low bits, stages it in shared memory and writes it with
 // coalesced stores along the destination-low bits.  HBM-bound: 24 B per element (12 in + 12 out).
+#include <type_traits>
+
 #include "kernels.h"
 #include "ring.cuh"
 
@@ -35,8 +37,9 @@ __global__ void __launch_bounds__(256) permute_kernel(PermArgs p, const int32_t 
                                                       CT *__restrict__ dst_c) {
   extern __shared__ __align__(16) unsigned char smem[];
   const int tile = 1 << p.nt;
+  constexpr bool HC = !std::is_same<CT, NoCount>::value;            // search mode moves the energy plane alone
   CT *sh_c = reinterpret_cast<CT *>(smem);
-  int32_t *sh_e = reinterpret_cast<int32_t *>(smem + sizeof(CT) * tile);
+  int32_t *sh_e = reinterpret_cast<int32_t *>(smem + (HC ? sizeof(CT) : 0) * tile);
   const int64_t n_tiles = ((int64_t)1 << p.n_outer) * p.batch;
   for (int64_t t = blockIdx.x; t < n_tiles; t += gridDim.x) {
     const int64_t b = t >> p.n_outer;
@@ -49,7 +52,7 @@ __global__ void __launch_bounds__(256) permute_kernel(PermArgs p, const int32_t 
       uint32_t s = 0;
       for (int q = 0; q < p.nt; q++) if ((i >> q) & 1) s += p.tile_src[q];
       sh_e[i] = src_e[sbase + s];
-      sh_c[i] = src_c[sbase + s];
+      if constexpr (HC) sh_c[i] = src_c[sbase + s];
     }
     __syncthreads();
     // scatter: thread index bits enumerate the tile in destination order
@@ -57,7 +60,7 @@ __global__ void __launch_bounds__(256) permute_kernel(PermArgs p, const int32_t 
       uint32_t d = 0; int j = 0;
       for (int q = 0; q < p.nt; q++) if ((i >> q) & 1) { int tb = p.dperm[q]; j |= 1 << tb; d += p.tile_dst[tb]; }
       dst_e[dbase + d] = sh_e[j];
-      dst_c[dbase + d] = sh_c[j];
+      if constexpr (HC) dst_c[dbase + d] = sh_c[j];
     }
     __syncthreads();
   }
@@ -103,14 +106,22 @@ template <> struct Vec4<uint32_t> {
   __device__ __forceinline__ void set(int u, uint32_t v) { if (u == 0) a.x = v; else if (u == 1) a.y = v; else if (u == 2) a.z = v; else a.w = v; }
 };
 
+template <> struct Vec4<NoCount> {
+  __device__ __forceinline__ void load(const NoCount *) {}
+  __device__ __forceinline__ void store(NoCount *) const {}
+  __device__ __forceinline__ void gload(const NoCount *) {}
+  __device__ __forceinline__ void gstore(NoCount *) const {}
+};
+
 template <class CT>
 __global__ void __launch_bounds__(256, 2) permute_vec_kernel(PermVecArgs p, const int32_t *__restrict__ src_e,
                                                           const CT *__restrict__ src_c, int32_t *__restrict__ dst_e,
                                                           CT *__restrict__ dst_c) {
   extern __shared__ __align__(16) unsigned char smem[];
   const int tile = 1 << p.nt, nvec = tile >> 2;
+  constexpr bool HC = !std::is_same<CT, NoCount>::value;
   CT *sh_c = reinterpret_cast<CT *>(smem);
-  int32_t *sh_e = reinterpret_cast<int32_t *>(smem + sizeof(CT) * tile);
+  int32_t *sh_e = reinterpret_cast<int32_t *>(smem + (HC ? sizeof(CT) : 0) * tile);
   constexpr int VPT = 4;                               // vectors per thread at nt = 12
   // per-thread tables: vector v = threadIdx.x + 256*k
   uint32_t s_off[VPT], s_adr[VPT], d_off[VPT], d_adr[VPT], u_adr[4];
@@ -157,7 +168,7 @@ __global__ void __launch_bounds__(256, 2) permute_vec_kernel(PermVecArgs p, cons
       if (threadIdx.x + 256 * k < nvec) {
         int32_t e[4]; Vec4<CT> c;
 #pragma unroll
-        for (int u = 0; u < 4; u++) { const uint32_t a = d_adr[k] ^ u_adr[u]; e[u] = sh_e[a]; c.set(u, sh_c[a]); }
+        for (int u = 0; u < 4; u++) { const uint32_t a = d_adr[k] ^ u_adr[u]; e[u] = sh_e[a]; if constexpr (HC) c.set(u, sh_c[a]); }
         *reinterpret_cast<int4 *>(dst_e + dbase + d_off[k]) = make_int4(e[0], e[1], e[2], e[3]);
         c.gstore(dst_c + dbase + d_off[k]);
       }
@@ -174,7 +185,7 @@ inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 
 bool launch_permute_vec(int rank, const int32_t *perm, const int *inv, int64_t batch, const int32_t *src_e, const void *src_c,
                         int32_t *dst_e, void *dst_c, int ring, cudaStream_t st) {
   if (rank < 4 || !aligned16(src_e) || !aligned16(src_c) || !aligned16(dst_e) || !aligned16(dst_c)) return false;
-  if (ring == 0 && ((reinterpret_cast<uintptr_t>(src_c) | reinterpret_cast<uintptr_t>(dst_c)) & 31)) return false;   // 32-byte count vectors
+  if (ring_count_bytes(ring) == 8 && ((reinterpret_cast<uintptr_t>(src_c) | reinterpret_cast<uintptr_t>(dst_c)) & 31)) return false;   // 32-byte count vectors
   PermVecArgs p;
   p.rank = rank; p.batch = batch;
   const int LOW = rank < 5 ? rank : 5;
@@ -213,10 +224,12 @@ bool launch_permute_vec(int rank, const int32_t *perm, const int *inv, int64_t b
   const int64_t n_tiles = ((int64_t)1 << p.n_outer) * batch;
   const int64_t cap = 148 * 8;
   const int grid = (int)(n_tiles < cap ? n_tiles : cap);
-  const size_t csz = ring == 0 ? 8 : 4;
+  const size_t csz = ring_count_bytes(ring);
   const size_t smem = ((size_t)1 << nt) * (csz + 4);
-  if (ring == 0)
+  if (csz == 8)                                           // mod 2^64, or both prime residues packed: pure data movement
     permute_vec_kernel<uint64_t><<<grid, 256, smem, st>>>(p, src_e, (const uint64_t *)src_c, dst_e, (uint64_t *)dst_c);
+  else if (csz == 0)
+    permute_vec_kernel<NoCount><<<grid, 256, smem, st>>>(p, src_e, (const NoCount *)src_c, dst_e, (NoCount *)dst_c);
   else
     permute_vec_kernel<uint32_t><<<grid, 256, smem, st>>>(p, src_e, (const uint32_t *)src_c, dst_e, (uint32_t *)dst_c);
   return true;
@@ -253,10 +266,12 @@ void launch_permute(int rank, const int32_t *perm, int64_t batch, const int32_t 
   const int64_t n_tiles = ((int64_t)1 << p.n_outer) * batch;
   const int64_t cap = 148 * 8;
   const int grid = (int)(n_tiles < cap ? n_tiles : cap);
-  const size_t csz = ring == 0 ? 8 : 4;
+  const size_t csz = ring_count_bytes(ring);
   const size_t smem = ((size_t)1 << nt) * (csz + 4);
-  if (ring == 0)
+  if (csz == 8)
     permute_kernel<uint64_t><<<grid, 256, smem, st>>>(p, src_e, (const uint64_t *)src_c, dst_e, (uint64_t *)dst_c);
+  else if (csz == 0)
+    permute_kernel<NoCount><<<grid, 256, smem, st>>>(p, src_e, (const NoCount *)src_c, dst_e, (NoCount *)dst_c);
   else
     permute_kernel<uint32_t><<<grid, 256, smem, st>>>(p, src_e, (const uint32_t *)src_c, dst_e, (uint32_t *)dst_c);
 }

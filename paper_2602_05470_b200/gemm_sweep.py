@@ -8,6 +8,8 @@ median of --repeat after 2 warm-ups), GFMA/s (1 tropical FMA = one (b, m, n, k) 
 A mode is count_bits:energy_bits, the caller's promises on the operands (include/bbtn.h): 3:7 selects the packed
 16x2 form (small counts and |energy| < 2^7), 3:32 32-bit energies with 32-bit accumulators, 14:32 chunk-local
 32-bit tie sums with 64-bit accumulators, 32:32 32-bit operands with 64-bit accumulators, 64:32 the full 64x64 multiply.
+count_bits 0 is the search mode's K3 (bbtn_maxplus_gemm_batched: energy planes alone, 4 B per element): 0:7 its packed
+16-bit form, 0:32 its 32-bit form.
 """
 from __future__ import annotations
 
@@ -43,20 +45,24 @@ def main():
             dCe = torch.empty((B, n, n), dtype=torch.int32, device="cuda"); dCc = torch.empty((B, n, n), dtype=torch.int64, device="cuda")
             for mode in a.modes:
                 bits, ebits = (int(x) for x in mode.split(":"))
+                if bits == 0:
+                    run = lambda: bb.maxplus_gemm_batched(dAe, dBe, dCe, energy_bits=ebits, stream=st.cuda_stream)
+                else:
+                    run = lambda: bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, energy_bits=ebits, stream=st.cuda_stream)
                 with torch.cuda.stream(st):
                     for _ in range(2):
-                        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, energy_bits=ebits, stream=st.cuda_stream)
+                        run()
                     ts = []
                     for _ in range(a.repeat):
                         e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
                         e0.record(st)
-                        bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, dCe, dCc, count_bits=bits, energy_bits=ebits, stream=st.cuda_stream)
+                        run()
                         e1.record(st); e1.synchronize()
                         ts.append(e0.elapsed_time(e1))
                 ms = float(np.median(ts))
                 fma = float(B) * n * n * n
                 print(json.dumps({"n": n, "batch": B, "count_bits": bits, "energy_bits": ebits, "ms": ms, "gfma_per_s": fma / ms / 1e6,
-                                  "gop_per_s": 2 * fma / ms / 1e6, "bytes": B * 3 * n * n * 12}), flush=True)
+                                  "gop_per_s": 2 * fma / ms / 1e6, "bytes": B * 3 * n * n * (12 if bits else 4)}), flush=True)
             del dAe, dAc, dBe, dBc, dCe, dCc
 
 

@@ -790,8 +790,9 @@ def test_search_mode_energies_match_oracle(bb, oracle, case):
     n = inst.n_vertices
     fixed = np.array([0, 1, 5], np.int32) if case == 4 else I.random_order(n, 70 + case)[:4]
     assign = I.all_assignments(len(fixed))
-    for tree in (None, I.elimination_tree(inst.input_index_sets(), I.natural_order(n))):
-        h = bb.Handle(inst, tree=tree, flags=bb.BBTN_SEARCH_ONLY)
+    for tree, extra in ((None, 0), (I.elimination_tree(inst.input_index_sets(), I.natural_order(n)), 0),
+                        (None, bb.BBTN_FORCE_TILED | bb.BBTN_NO_FUSED)):       # permute + max-plus GEMM wherever an index is summed
+        h = bb.Handle(inst, tree=tree, flags=bb.BBTN_SEARCH_ONLY | extra)
         energy, count = h.contract_batch(fixed, assign)
         assert (count == 0).all()
         for b in range(len(assign)):
@@ -822,6 +823,83 @@ def test_search_mode_drivers_and_large_kings(bb, oracle):
         h = bb.Handle(I.kings_subgraph(L, L, 0.8, 1), flags=bb.BBTN_SEARCH_ONLY)
         out = h.solve_local(32)
         assert out["energy"] == int(_goldens()[name]["energy"]) and out["count"] == 0, out
+        h.close()
+
+
+@pytest.mark.parametrize("B,M,N,K,seed,frac", [
+    (1, 64, 64, 64, 61, 0.0),
+    (3, 256, 256, 256, 62, 0.0),
+    (2, 131, 197, 100, 63, 0.2),          # ragged in every dimension, zero elements
+    (5, 1, 1, 1, 64, 0.0),
+    (1, 129, 65, 513, 65, 0.05),
+    (4, 17, 201, 3, 66, 0.5),             # odd leading dimension: the scalar load/store paths
+    (1, 1, 300, 1000, 67, 0.0),
+    (2, 333, 1, 129, 68, 0.3),
+    (7, 48, 64, 33, 69, 0.2),             # M, N <= 64: the 64x64 tile, ragged, batched
+    (3, 64, 37, 70, 70, 0.0),
+    (1, 300, 129, 17, 71, 0.9),           # mostly zero elements: whole rows / columns of -inf
+])
+def test_maxplus_gemm_matches_oracle(bb, oracle, B, M, N, K, seed, frac):
+    # K3 of the search mode alone: max-plus on the energy plane = the energy half of the counting oracle's GEMM
+    import torch
+    Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed, neg_inf_frac=frac)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    prev = bb.set_debug_checks(True)
+    try:
+        want_e, _ = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
+        for ebits in (7, 32):                                          # packed 16-bit halves / 32-bit
+            assert (bb.maxplus_gemm_batched(dev(Ae), dev(Be), energy_bits=ebits).cpu().numpy() == want_e).all(), ebits
+        # the whole range of the packed form (-2047..2047) and the zero element
+        spread = lambda e, sft: np.where(e <= -(1 << 29), e, ((e.astype(np.int64) * 31 + sft) % 4095 - 2047)).astype(np.int32)
+        A2, B2 = spread(Ae, 7), spread(Be, 1900)
+        want2, _ = _oracle_gemm(oracle, A2, Ac, B2, Bc)
+        for ebits in (11, 12, 32):
+            assert (bb.maxplus_gemm_batched(dev(A2), dev(B2), energy_bits=ebits).cpu().numpy() == want2).all(), ebits
+        if A2.size > 100 and frac < 0.5:
+            with pytest.raises(bb.BbtnError):                          # |e| up to 2047 is not below 2^10
+                bb.maxplus_gemm_batched(dev(A2), dev(B2), energy_bits=10)
+        # energies up to +-2^27 (sums within the finite range): the 32-bit form
+        big = lambda e: np.where(e <= -(1 << 29), e, e.astype(np.int64) * (1 << 15)).astype(np.int32)
+        A3, B3 = big(A2), big(B2)
+        want3, _ = _oracle_gemm(oracle, A3, Ac, B3, Bc)
+        assert (bb.maxplus_gemm_batched(dev(A3), dev(B3), energy_bits=27).cpu().numpy() == want3).all()
+    finally:
+        bb.set_debug_checks(prev)
+    # a shared operand (stride 0) holding non-canonical zero elements (anything below -2^29 reads as zero)
+    if B > 1:
+        Bz = Be[0].copy(); Bz[Bz <= -(1 << 29)] = -(1 << 29) - 5
+        wants, _ = _oracle_gemm(oracle, Ae, Ac, np.broadcast_to(Be[0], Be.shape).copy(), np.broadcast_to(Bc[0], Bc.shape).copy())
+        for ebits in (7, 32):
+            assert (bb.maxplus_gemm_batched(dev(Ae), dev(Bz), energy_bits=ebits).cpu().numpy() == wants).all(), ebits
+
+
+@pytest.mark.parametrize("case", ["ising12", "king12", "ising12-sliced", "king12-sliced"])
+def test_search_mode_block_tree_runs_permute_and_maxplus_gemm(bb, oracle, case):
+    # the divide-and-conquer trees of test_block_tree_runs_tiled_gemm_and_trace_kernels in search mode: the joins are
+    # energy-only K2 + the max-plus K3 (automatic mode); every leaf energy equals the counting oracle's
+    L = 12
+    if case.startswith("ising"):
+        inst = I.ising_lattice_2d(L, L, 3)
+        ids = None
+    else:
+        inst = I.kings_subgraph(L, L, 1.0, 6, weights="rand")
+        ids = _king_ids(inst, L, L)
+    fixed, assign = None, None
+    if case.endswith("sliced"):
+        v = lambda r, c: r * L + c if ids is None else int(ids[r][c])
+        fixed = np.array([v(2, 2), v(2, L - 3), v(L - 3, 3)], np.int32)
+        assign = I.all_assignments(3)
+    parts = I.lattice_block_parts(L, L, [L // 2], [L // 2], ids, exclude=() if fixed is None else fixed)
+    tree = I.grouped_elimination_tree(inst.input_index_sets(() if fixed is None else fixed), parts)
+    for flags in (bb.BBTN_SEARCH_ONLY, bb.BBTN_SEARCH_ONLY | bb.BBTN_FORCE_TILED | bb.BBTN_NO_GRAPH):
+        h = bb.Handle(inst, tree=tree, flags=flags)
+        info = h.plan_query(fixed, 1 if assign is None else len(assign))
+        assert info["n_gemm_tiled"] > 0 and info["n_permute"] > 0, info
+        energy, count = h.contract_batch(fixed, assign)
+        assert (count == 0).all()
+        for b in range(len(energy)):
+            we, _ = oracle.contract_tree(inst, tree[0], tree[1], fixed, None if assign is None else assign[b])
+            assert int(energy[b]) == we, (case, flags, b)
         h.close()
 
 
