@@ -44,12 +44,16 @@ template <bool P16, int TB> struct Cfg {
   static_assert(2 * STAGE_WORDS * 4 <= 48 * 1024, "static shared memory");
 };
 
+// enc(e) = max(e + BIAS, 0): a finite e >= -3967 gives e + BIAS > 0, any zero element (e < -2^29) a negative sum -> 0;
+// one VIADDMNMX instead of compare + add + select (the encoders run on the same ALU pipe as the FMAs)
+__device__ __forceinline__ uint32_t enc16(int32_t e) { return (uint32_t)__viaddmax_s32(e, BIAS, 0); }
+__device__ __forceinline__ uint32_t canon32(int32_t e) { return (uint32_t)(e < ZERO_BELOW ? NEG_INF : e); }   // non-canonical zero -> canonical
 template <bool P16> __device__ __forceinline__ uint32_t enc_a(int32_t e) {
-  if (P16) return e < ZERO_BELOW ? 0u : (uint32_t)(e + BIAS) * 0x10001u;      // the value in both halves
-  return (uint32_t)(e < ZERO_BELOW ? NEG_INF : e);                            // a non-canonical zero becomes the canonical one
+  if (P16) return enc16(e) * 0x10001u;                                        // the value in both halves
+  return canon32(e);
 }
-__device__ __forceinline__ uint32_t canon32(int32_t e) { return (uint32_t)(e < ZERO_BELOW ? NEG_INF : e); }
-__device__ __forceinline__ uint32_t enc16(int32_t e) { return e < ZERO_BELOW ? 0u : (uint32_t)(e + BIAS); }
+// two encoded halves in one word; written as a multiply-add so that it issues on the FMA pipe (IMAD), not the ALU pipe
+__device__ __forceinline__ uint32_t pack2(int32_t lo, int32_t hi) { return enc16(hi) * 0x10000u + enc16(lo); }
 
 __device__ __forceinline__ void lds4(const uint32_t *src, uint32_t *dst) {
   const uint4 v = *reinterpret_cast<const uint4 *>(src);
@@ -119,6 +123,30 @@ __global__ void __launch_bounds__(Cfg<P16, TB>::NT, TB == 128 ? 2 : 8) gemm_maxp
       }
     }
   };
+  // interior tile with 16-byte access: element offsets of this thread's units are fixed, only the chunk base moves
+  const bool interior = p.vecA && p.vecB && m0 + TB <= p.M && n0 + TB <= p.N &&
+                        (int64_t)p.M * p.K < (1ll << 31) && (int64_t)p.K * p.N < (1ll << 31);      // 32-bit element offsets
+  int offA[UNITS], offB[UNITS];
+#pragma unroll
+  for (int u = 0; u < UNITS; u++) {
+    const int idx = t + u * NT;
+    offA[u] = A_KMAJOR ? (idx / (TB / 4)) * p.M + m0 + 4 * (idx % (TB / 4)) : (m0 + idx / (BK / 4)) * p.K + 4 * (idx % (BK / 4));
+    offB[u] = (idx / (TB / 4)) * p.N + n0 + 4 * (idx % (TB / 4));
+  }
+  auto load_fast = [&](int c) {
+    const int32_t *Ac = A + (A_KMAJOR ? (int64_t)c * BK * p.M : (int64_t)c * BK);
+    const int32_t *Bc = B + (int64_t)c * BK * p.N;
+#pragma unroll
+    for (int u = 0; u < UNITS; u++) {
+      const int4 v = __ldg(reinterpret_cast<const int4 *>(Ac + offA[u]));
+      ra[u][0] = v.x; ra[u][1] = v.y; ra[u][2] = v.z; ra[u][3] = v.w;
+    }
+#pragma unroll
+    for (int u = 0; u < UNITS; u++) {
+      const int4 v = __ldg(reinterpret_cast<const int4 *>(Bc + offB[u]));
+      rb[u][0] = v.x; rb[u][1] = v.y; rb[u][2] = v.z; rb[u][3] = v.w;
+    }
+  };
   auto store = [&](int buf) {
     uint32_t *sA = smem + buf * G::STAGE_WORDS, *sB = sA + BK * TB;
 #pragma unroll
@@ -141,7 +169,7 @@ __global__ void __launch_bounds__(Cfg<P16, TB>::NT, TB == 128 ? 2 : 8) gemm_maxp
       const int kk = idx / (TB / 4), q = idx % (TB / 4);
       if (P16)
         *reinterpret_cast<uint2 *>(sB + kk * BW + 2 * q) =
-            make_uint2(enc16(rb[u][0]) | (enc16(rb[u][1]) << 16), enc16(rb[u][2]) | (enc16(rb[u][3]) << 16));
+            make_uint2(pack2(rb[u][0], rb[u][1]), pack2(rb[u][2], rb[u][3]));
       else
         *reinterpret_cast<uint4 *>(sB + kk * BW + 4 * q) =
             make_uint4(canon32(rb[u][0]), canon32(rb[u][1]), canon32(rb[u][2]), canon32(rb[u][3]));
@@ -167,12 +195,14 @@ __global__ void __launch_bounds__(Cfg<P16, TB>::NT, TB == 128 ? 2 : 8) gemm_maxp
   };
 
   const int n_chunks = (p.K + BK - 1) / BK;
-  load(0);
+  const int n_fast = interior ? p.K / BK : 0;                    // chunks 0 .. n_fast-1 need no bounds checks
+  if (n_fast > 0) load_fast(0); else load(0);
   store(0);
   __syncthreads();
   for (int c = 0; c < n_chunks; c++) {
     const bool more = c + 1 < n_chunks;
-    if (more) load(c + 1);
+    if (c + 1 < n_fast) load_fast(c + 1);
+    else if (more) load(c + 1);
     compute(c & 1);
     if (more) store((c + 1) & 1);        // the other buffer: last read in compute(c - 1), before the barrier that ended it
     __syncthreads();
