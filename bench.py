@@ -208,9 +208,11 @@ def _goldens():
         return json.load(f)["cases"]
 
 
-def gemm_sweep_block(bb, torch, stream, int_peak, repeat=3):
+def gemm_sweep_block(bb, torch, stream, int_peak, viaddmnmx_peak, repeat=3):
     """Corners of the config-4a sweep (n, batch) in every count/energy mode: GFMA/s and the fraction of the int32 roof
-    (4 algorithmic int32 lane-instructions per FMA; 6 for the full 64x64 count product)."""
+    (4 algorithmic int32 lane-instructions per FMA; 6 for the full 64x64 count product).  Then the search mode's K3
+    (max-plus on the energy planes, bbtn_maxplus_gemm_batched) on the same operands: its one instruction per FMA
+    (per two FMAs in the packed form) is VIADDMNMX, so its roof is the measured VIADDMNMX issue rate."""
     out = []
     ev = lambda: torch.cuda.Event(enable_timing=True)
     for n, B in SWEEP:
@@ -238,7 +240,23 @@ def gemm_sweep_block(bb, torch, stream, int_peak, repeat=3):
             gfma = float(B) * n ** 3 / ms / 1e6
             out.append({"n": n, "batch": B, "mode": mode, "what": what, "ms": ms, "gfma_per_s": gfma,
                         "frac_of_int32_peak": INT_OPS_PER_FMA[acc_bits] * gfma / int_peak})
-        del dAe, dAc, dBe, dBc, dCe, dCc
+        dCm = torch.empty_like(dCe)
+        for ebits, what, fma_per_instr in ((7, "search mode: max-plus, packed 16-bit energies", 2), (32, "search mode: max-plus, 32-bit energies", 1)):
+            ts = []
+            with torch.cuda.stream(stream):
+                for it in range(repeat + 1):
+                    a, b = ev(), ev()
+                    a.record(stream)
+                    bb.maxplus_gemm_batched(dAe, dBe, dCm, energy_bits=ebits, stream=stream.cuda_stream)
+                    b.record(stream); b.synchronize()
+                    if it:
+                        ts.append(a.elapsed_time(b))
+            assert bool((dCm == dCe).all().item()), f"max-plus GEMM disagrees with the energies of the counting GEMM at n={n}"
+            ms = float(np.median(ts))
+            gfma = float(B) * n ** 3 / ms / 1e6
+            out.append({"n": n, "batch": B, "mode": f"0:{ebits}", "what": what, "ms": ms, "gfma_per_s": gfma,
+                        "frac_of_viaddmnmx_peak": gfma / fma_per_instr / viaddmnmx_peak})
+        del dAe, dAc, dBe, dBc, dCe, dCc, dCm
     return out
 
 
@@ -514,7 +532,7 @@ def run_ours(args):
         cpu = cpu_baseline_both(args)
     sweep = tts = None
     if world == 1 and not args.no_extras:
-        sweep = gemm_sweep_block(bb, torch, stream, int_peak)
+        sweep = gemm_sweep_block(bb, torch, stream, int_peak, mb["viaddmnmx"])
         h_dev.close(); h_host.close()
         del dAe, dAc, dBe, dBc, dCe, dCc, dPe, dPc
         torch.cuda.empty_cache()
