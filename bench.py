@@ -297,7 +297,7 @@ def time_to_solve_block(bb, skip_king40=False):
             continue
         r = T.solve_king_local(L, 1, 32, crt=True, hint=int(g[name]["energy"]))
         check(name, {"config": 5, "king": L, "seconds": r["seconds"], "plan_seconds": r["plan_only_seconds"],
-                     "mode": "bbtn_solve_local, T_target 2^32, three count rings, K5 bounds vs the golden optimum as incumbent",
+                     "mode": "bbtn_solve_local, T_target 2^32, three count residues in two passes (mod 2^64; p1 and p2 packed), K5 bounds vs the golden optimum as incumbent",
                      **{k: r[k] for k in ("stretches", "sliced_stretches", "branches_planned", "branches_contracted", "branches_infeasible",
                                           "branches_pruned", "max_fixed", "max_rank", "arena_bytes", "kernel_launches")},
                      "algorithmic_gb_per_s": r["algorithmic_gb_per_s"], "count": r["count"]}, r["energy"], r["count_mod_2_64"], r["count"])
