@@ -54,7 +54,9 @@ INT_OPS_PER_FMA = {32: 4, 64: 6}
 # object (profiles/r2_k3_pack16_sass.md): per 128 FMAs 64 VIADDMNMX.S16x2 + 64 adds + 64 HSETP2 + 128 IMAD + 28 LDS.128 + 16 others
 PACK16_INSTR_PER_FMA = 364.0 / 128.0
 SWEEP = [(64, 1024), (256, 256), (1024, 64), (4096, 2)]                # (n, batch) corners of config 4a
-SWEEP_MODES = [("3:7", "packed 16x2 energies, 32-bit accumulators", 32), ("3:32", "32-bit accumulators", 32),
+SWEEP_MODES = [("3:7", "packed 16x2 energies, 32-bit accumulators", 32),
+               ("13:7", "packed 16x2 energies, carry form (31-bit running sum + carry register), 64-bit totals", 32),
+               ("32:7", "packed 16x2 energies, 32-bit operands, 64-bit accumulators", 32), ("3:32", "32-bit accumulators", 32),
                ("14:32", "chunk-local 32-bit tie sums, 64-bit accumulators", 32),
                ("32:32", "32-bit operands, 64-bit accumulators", 32), ("64:32", "full 64x64 count product", 64)]
 

@@ -294,8 +294,9 @@ int bbtn_set_debug_checks(int32_t on);
  * count_bits in 1..64: upper bound on log2(count+1) of BOTH operands that the caller guarantees (64 = no
  * promise; <= 32 selects the 32x32->64 multiply path, small values 32-bit accumulators).
  * energy_bits in 1..32: the caller guarantees |e| < 2^energy_bits for every FINITE operand energy (32 = no promise
- * beyond BBTN_ENERGY_LIMIT).  energy_bits <= 11 together with counts small enough for 32-bit accumulators
- * (2 * count_bits + ceil(log2 K) <= 32) selects the packed form: 16-bit energies, two outputs per instruction.
+ * beyond BBTN_ENERGY_LIMIT).  energy_bits <= 11 together with count_bits <= 32 selects the packed form: 16-bit
+ * energies, two outputs per instruction, with 32-bit accumulators where 2 * count_bits + ceil(log2 K) <= 32, a
+ * 31-bit running sum plus carry register for count_bits <= 13, and 64-bit accumulators otherwise.
  * A broken promise gives wrong results silently unless bbtn_set_debug_checks is on.  The result never depends on
  * which form ran.  Asynchronous on cuda_stream. */
 int bbtn_tropical_gemm_batched(int64_t batch, int32_t M, int32_t N, int32_t K,

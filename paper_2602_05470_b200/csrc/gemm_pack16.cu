@@ -30,6 +30,13 @@ namespace {
 using namespace stage;
 
 constexpr int BIAS = 11903, FINITE2 = 15872;   // enc(e) = e + BIAS;  half >= FINITE2  <=>  finite sum
+// count accumulators:
+//   CM_ACC32    32-bit (2 * count_bits + ceil(log2 K) <= 32)
+//   CM_CARRY31  operand counts < 2^13, any K: the 32-bit accumulator is kept below 2^31 at chunk boundaries (a chunk adds
+//               16 products < 2^26, so it cannot wrap inside a chunk) and its bit 31 is moved into a second 32-bit register
+//               after every chunk: total = hi * 2^31 + lo < 2^63.  Inner loop = CM_ACC32's.
+//   CM_WIDE64   operand counts < 2^32: 64-bit accumulators, SEL + IMAD.WIDE per FMA
+enum CountMode : int { CM_ACC32 = 0, CM_CARRY31 = 1, CM_WIDE64 = 2 };
 // tile TB x TB (128: the general case; 64: matrices with M, N <= 64, where the big tile would be mostly padding),
 // TB*TB/32 threads: 4 x 8 outputs each
 template <int TB> struct Cfg {
@@ -66,6 +73,26 @@ __device__ __forceinline__ void tie2(uint32_t &c_lo, uint32_t &c_hi, uint32_t a2
         "@p mad.lo.u32 %0, %5, %6, %0;\n\t"
         "@q mad.lo.u32 %1, %5, %7, %1;\n\t}"
         : "+r"(c_lo), "+r"(c_hi) : "r"(a2), "r"(b2), "r"(E2), "r"(ca), "r"(cb_lo), "r"(cb_hi));
+}
+// the same with 64-bit accumulators and 32-bit operand counts (CM_WIDE64): ptxas turns a predicated mad.wide into
+// multiply + add + add-with-carry + two selects, so the predicate selects the multiplicand instead (SEL + IMAD.WIDE)
+__device__ __forceinline__ void tie2w(uint64_t &c_lo, uint64_t &c_hi, uint32_t a2, uint32_t b2, uint32_t E2, uint32_t ca,
+                                      uint32_t cb_lo, uint32_t cb_hi) {
+  asm("{\n\t.reg .pred p, q;\n\t.reg .b32 s, t0, t1;\n\t"
+      "add.u32 s, %2, %3;\n\t"
+      "setp.eq.f16x2 p|q, s, %4;\n\t"
+      "selp.u32 t0, %6, 0, p;\n\t"
+      "selp.u32 t1, %7, 0, q;\n\t"
+      "mad.wide.u32 %0, %5, t0, %0;\n\t"
+      "mad.wide.u32 %1, %5, t1, %1;\n\t}"
+      : "+l"(c_lo), "+l"(c_hi) : "r"(a2), "r"(b2), "r"(E2), "r"(ca), "r"(cb_lo), "r"(cb_hi));
+}
+__device__ __forceinline__ void reset2w(uint64_t &c_lo, uint64_t &c_hi, uint32_t En2, uint32_t E2) {
+  asm("{\n\t.reg .pred p, q;\n\t"
+      "setp.ne.f16x2 p|q, %2, %3;\n\t"
+      "@p mov.u64 %0, 0;\n\t"
+      "@q mov.u64 %1, 0;\n\t}"
+      : "+l"(c_lo), "+l"(c_hi) : "r"(En2), "r"(E2));
 }
 // a new maximum in a half drops the count of the old one
 __device__ __forceinline__ void reset2(uint32_t &c_lo, uint32_t &c_hi, uint32_t En2, uint32_t E2) {
@@ -134,8 +161,9 @@ __device__ __forceinline__ void lds4(const uint32_t *src, uint32_t *dst) {
   dst[0] = v.x; dst[1] = v.y; dst[2] = v.z; dst[3] = v.w;
 }
 
-template <bool A_KMAJOR, int TB>
+template <bool A_KMAJOR, int TB, int CM>
 __global__ void __launch_bounds__(Cfg<TB>::PT, Cfg<TB>::MIN_CTAS) gemm_pack16_kernel(const GemmArgs p) {
+  static_assert(CM == CM_ACC32 || TB == 64, "the 64-bit count modes need more than the 128 registers of the 512-thread tile");
   using G = Cfg<TB>;
   constexpr int BM = G::BM, BN = G::BN, PT = G::PT;
   constexpr int P_RAW = G::RAW, P_CONV = G::CONV, P_CAE = G::CAE, P_CAC = G::CAC, P_CBE = G::CBE;
@@ -157,13 +185,15 @@ __global__ void __launch_bounds__(Cfg<TB>::PT, Cfg<TB>::MIN_CTAS) gemm_pack16_ke
   const int tx = (w % WX) * 8 + (lane & 7), ty = (w / WX) * 4 + (lane >> 3);      // tx 0..BN/8-1, ty 0..BM/4-1
 
   // rows: ty*4 + i (i = 0..3); columns: q*BN/2 + tx*4 + 2p + half (q = 0,1; p = 0,1)
-  uint32_t E2[4][4], C[4][8];
+  using AccC = typename std::conditional<CM == CM_WIDE64, uint64_t, uint32_t>::type;
+  uint32_t E2[4][4]; AccC C[4][8];
+  uint32_t H[CM == CM_CARRY31 ? 4 : 1][8];                  // CM_CARRY31: carries out of bit 31 of C
 #pragma unroll
   for (int i = 0; i < 4; i++) {
 #pragma unroll
     for (int j = 0; j < 4; j++) E2[i][j] = 0u;
 #pragma unroll
-    for (int j = 0; j < 8; j++) C[i][j] = 0u;
+    for (int j = 0; j < 8; j++) { C[i][j] = 0; if (CM == CM_CARRY31) H[i][j] = 0u; }
   }
 
   const int n_chunks = (p.K + BK - 1) / BK;
@@ -227,18 +257,30 @@ __global__ void __launch_bounds__(Cfg<TB>::PT, Cfg<TB>::MIN_CTAS) gemm_pack16_ke
 #pragma unroll
         for (int j = 0; j < 4; j++) {                        // j = q*2 + p: columns q*64 + tx*4 + 2p, +1
           if (P1) En[i][j] = __viaddmax_s16x2(a1[i], b1[j], En[i][j]);
-          if ((i * 4 + j) % 8 < 5)                       // 10 of 16 adds on the ALU pipe: ALU 42 / FMA 38 instructions per kk
+          if constexpr (CM == CM_WIDE64)
+            tie2w(C[i][2 * j], C[i][2 * j + 1], a2[i], b2[j], E2[i][j], ca[i], cb[2 * j], cb[2 * j + 1]);
+          else if ((i * 4 + j) % 8 < 5)                  // 10 of 16 adds on the ALU pipe: ALU 42 / FMA 38 instructions per kk
             tie2<true>(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], a2[i], b2[j], E2[rb * 4 + i][j], ca[i], cb[2 * j], cb[2 * j + 1]);
           else
             tie2<false>(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], a2[i], b2[j], E2[rb * 4 + i][j], ca[i], cb[2 * j], cb[2 * j + 1]);
         }
+    }
+    if constexpr (CM == CM_CARRY31) {                    // once per chunk: move bit 31 of the running sum into the carry register
+#pragma unroll
+      for (int i = 0; i < 4; i++)
+#pragma unroll
+        for (int j = 0; j < 8; j++) { H[i][j] += C[i][j] >> 31; C[i][j] &= 0x7fffffffu; }
     }
     if (P1) {
 #pragma unroll
       for (int i = 0; i < 4; i++)
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-          reset2(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], En[i][j], E2[rb * 4 + i][j]);
+          if constexpr (CM == CM_WIDE64) reset2w(C[i][2 * j], C[i][2 * j + 1], En[i][j], E2[i][j]);
+          else {
+            reset2(C[rb * 4 + i][2 * j], C[rb * 4 + i][2 * j + 1], En[i][j], E2[rb * 4 + i][j]);
+            if constexpr (CM == CM_CARRY31) reset2(H[i][2 * j], H[i][2 * j + 1], En[i][j], E2[i][j]);
+          }
           E2[rb * 4 + i][j] = En[i][j];
         }
     }
@@ -276,7 +318,9 @@ __global__ void __launch_bounds__(Cfg<TB>::PT, Cfg<TB>::MIN_CTAS) gemm_pack16_ke
         const uint32_t h = (E2[i][q * 2 + (j >> 1)] >> ((j & 1) * 16)) & 0xffffu;
         const bool fin = h >= (uint32_t)FINITE2;
         e[j] = fin ? (int32_t)h - 2 * BIAS : NEG_INF;
-        c[j] = fin ? (uint64_t)C[i][q * 4 + j] : 0ull;
+        uint64_t tot = (uint64_t)C[i][q * 4 + j];
+        if constexpr (CM == CM_CARRY31) tot += (uint64_t)H[i][q * 4 + j] << 31;
+        c[j] = fin ? tot : 0ull;
       }
       const int64_t o = (int64_t)gm * p.N + gn;
       if (p.vecC && gn + 4 <= p.N) {
@@ -294,29 +338,39 @@ __global__ void __launch_bounds__(Cfg<TB>::PT, Cfg<TB>::MIN_CTAS) gemm_pack16_ke
 
 inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
-template <bool KM, int TB>
+template <bool KM, int TB, int CM>
 void launch_p16(const GemmArgs &a, int64_t batch, cudaStream_t st) {
   using G = Cfg<TB>;
   const int64_t n_cta = (int64_t)((a.N + G::BN - 1) / G::BN) * ((a.M + G::BM - 1) / G::BM) * batch * a.G;
-  cudaFuncSetAttribute(gemm_pack16_kernel<KM, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM);
-  gemm_pack16_kernel<KM, TB><<<dim3((unsigned)n_cta), G::PT, G::SMEM, st>>>(a);
+  cudaFuncSetAttribute(gemm_pack16_kernel<KM, TB, CM>, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM);
+  gemm_pack16_kernel<KM, TB, CM><<<dim3((unsigned)n_cta), G::PT, G::SMEM, st>>>(a);
 }
 
 }  // namespace
 
-// RING_U64, caller promises: finite |energy| <= 3967 (zero element exactly NEG_INF) and counts small enough for
-// 32-bit accumulators (2 * count_bits + ceil(log2 K) <= 32).
+// RING_U64, caller promises: finite |energy| <= 3967 (zero element exactly NEG_INF) and operand counts below
+// 2^count_bits, count_bits <= 32.  32-bit accumulators when 2 * count_bits + ceil(log2 K) <= 32, else the carry form
+// (count_bits <= 13) or 64-bit accumulators, both on the 64 x 64 tile.
 void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                         const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
-                        int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, cudaStream_t st) {
+                        int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, cudaStream_t st) {
   GemmArgs a{G, M, N, K, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC, 0, 0, 0};
   const int ldA = a_kmajor ? M : K;
   a.vecA = (ldA % 4 == 0) && (sA % 4 == 0) && (((int64_t)M * K) % 4 == 0 || G == 1) && al16(Ae) && al16(Ac);
   a.vecB = (N % 4 == 0) && (sB % 4 == 0) && (((int64_t)K * N) % 4 == 0 || G == 1) && al16(Be) && al16(Bc);
   a.vecC = (N % 4 == 0) && (sC % 4 == 0) && (((int64_t)M * N) % 4 == 0 || G == 1) && al16(Ce) && al16(Cc);
   const bool small = M <= 64 && N <= 64;                   // a 128-row tile would be >= 75 % padding
-  if (a_kmajor) { if (small) launch_p16<true, 64>(a, batch, st); else launch_p16<true, 128>(a, batch, st); }
-  else { if (small) launch_p16<false, 64>(a, batch, st); else launch_p16<false, 128>(a, batch, st); }
+  int lgK = 0;
+  while (((int64_t)1 << lgK) < K) lgK++;
+  const int cm = (count_bits <= 16 && 2 * count_bits + lgK <= 32) ? CM_ACC32 : (count_bits <= 13 ? CM_CARRY31 : CM_WIDE64);
+  if (cm == CM_ACC32) {
+    if (a_kmajor) { if (small) launch_p16<true, 64, CM_ACC32>(a, batch, st); else launch_p16<true, 128, CM_ACC32>(a, batch, st); }
+    else { if (small) launch_p16<false, 64, CM_ACC32>(a, batch, st); else launch_p16<false, 128, CM_ACC32>(a, batch, st); }
+  } else if (cm == CM_CARRY31) {
+    if (a_kmajor) launch_p16<true, 64, CM_CARRY31>(a, batch, st); else launch_p16<false, 64, CM_CARRY31>(a, batch, st);
+  } else {
+    if (a_kmajor) launch_p16<true, 64, CM_WIDE64>(a, batch, st); else launch_p16<false, 64, CM_WIDE64>(a, batch, st);
+  }
 }
 
 }  // namespace bbtn

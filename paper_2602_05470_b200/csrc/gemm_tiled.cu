@@ -341,11 +341,11 @@ inline bool al16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) =
 
 }  // namespace
 
-// the packed form needs 32-bit accumulators (2 * count_bits + ceil(log2 K) <= 32) and finite |energy| < 2^11
+// the packed form needs finite |energy| < 2^11 and operand counts below 2^32 (32-bit accumulators where
+// 2 * count_bits + ceil(log2 K) <= 32, else the carry form or 64-bit accumulators: gemm_pack16.cu)
 bool gemm_pack16_eligible(int K, int count_bits, int energy_bits) {
-  int lgK = 0;
-  while (((int64_t)1 << lgK) < K) lgK++;
-  return count_bits <= 16 && 2 * count_bits + lgK <= 32 && energy_bits <= 11;
+  (void)K;
+  return count_bits <= 32 && energy_bits <= 11;
 }
 
 // RING_U64 only.  count_bits is the caller's bound on log2(count+1) of both operands.
@@ -362,8 +362,8 @@ void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_
   while (((int64_t)1 << lgK) < K) lgK++;
   const int mode = (count_bits <= 16 && 2 * count_bits + lgK <= 32) ? ACC32
                    : (count_bits <= 14 ? NARROW64 : (count_bits <= 32 ? ACC64N : WIDE));
-  if (mode == ACC32 && energy_bits <= 11) {
-    launch_gemm_pack16(batch, G, M, N, K, a_kmajor, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC, st);
+  if (mode != WIDE && energy_bits <= 11) {
+    launch_gemm_pack16(batch, G, M, N, K, a_kmajor, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC, count_bits, st);
   } else if (mode == ACC32) {
     if (a_kmajor) launch_one<ACC32, true, 2>(a, batch, st); else launch_one<ACC32, false, 2>(a, batch, st);
   } else if (mode == NARROW64) {

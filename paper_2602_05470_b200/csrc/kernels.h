@@ -56,7 +56,7 @@ bool gemm_pack16_eligible(int K, int count_bits, int energy_bits);
 // K3 packed form (gemm_pack16.cu; 128 x 128 tile, 64 x 64 for M, N <= 64): two outputs per integer instruction; finite |energy| < 2^11, 32-bit accumulators.
 void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kmajor,
                         const int32_t *Ae, const uint64_t *Ac, const int32_t *Be, const uint64_t *Bc,
-                        int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, cudaStream_t st);
+                        int32_t *Ce, uint64_t *Cc, int64_t sA, int64_t sB, int64_t sC, int count_bits, cudaStream_t st);
 
 // K3 in search mode (gemm_maxplus.cu): max-plus on the energy planes alone, one fused add-max per FMA (two with
 // energy_bits <= 11: packed 16-bit halves); layout arguments as launch_gemm_tiled.

@@ -8,6 +8,7 @@ median of --repeat after 2 warm-ups), GFMA/s (1 tropical FMA = one (b, m, n, k) 
 A mode is count_bits:energy_bits, the caller's promises on the operands (include/bbtn.h): 3:7 selects the packed
 16x2 form (small counts and |energy| < 2^7), 3:32 32-bit energies with 32-bit accumulators, 14:32 chunk-local
 32-bit tie sums with 64-bit accumulators, 32:32 32-bit operands with 64-bit accumulators, 64:32 the full 64x64 multiply.
+13:7 and 32:7 are the packed form with 64-bit totals (carry form for counts < 2^13; 64-bit accumulators for counts < 2^32).
 count_bits 0 is the search mode's K3 (bbtn_maxplus_gemm_batched: energy planes alone, 4 B per element): 0:7 its packed
 16-bit form, 0:32 its 32-bit form.
 """

@@ -55,7 +55,8 @@ def test_gemm_matches_oracle(bb, oracle, B, M, N, K, seed, frac, wide):
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
     # 64: full 64x64 multiply; 32: 32-bit operands, 64-bit accumulators; 3: counts <= 4, 32-bit accumulators;
     # (3, 7): also |energy| < 2^7 promised -> the packed 16x2 form
-    for bits, ebits in ((64, 32), (32, 32), (14, 32), (3, 32), (3, 7)) if not wide else ((64, 32),):
+    # (13, 7) / (32, 7): packed energies with the carry form / with 64-bit accumulators (64x64 tile)
+    for bits, ebits in ((64, 32), (32, 32), (14, 32), (3, 32), (3, 7), (13, 7), (32, 7)) if not wide else ((64, 32),):
         Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits, energy_bits=ebits)
         got_e = Ce.cpu().numpy(); got_c = Cc.cpu().numpy().view(np.uint64)
         assert (got_e == want_e).all(), (bits, ebits)
@@ -79,10 +80,10 @@ def test_gemm_packed_form_full_energy_range(bb, oracle, B, M, N, K, seed, frac):
     dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
     prev = bb.set_debug_checks(True)
     try:
-        for ebits in (11, 32):
-            Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=3, energy_bits=ebits)
-            assert (Ce.cpu().numpy() == want_e).all(), ebits
-            assert (Cc.cpu().numpy().view(np.uint64) == want_c).all(), ebits
+        for ebits, bits in ((11, 3), (32, 3), (11, 13), (11, 32)):       # 32-bit, carry-form and 64-bit accumulators
+            Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits, energy_bits=ebits)
+            assert (Ce.cpu().numpy() == want_e).all(), (ebits, bits)
+            assert (Cc.cpu().numpy().view(np.uint64) == want_c).all(), (ebits, bits)
         with pytest.raises(bb.BbtnError):                              # |e| up to 2047 is not below 2^10
             bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=3, energy_bits=10)
     finally:
@@ -103,6 +104,34 @@ def test_gemm_narrow_counts_long_sums(bb, oracle):
     for bits in (14, 32, 64):
         Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=bits)
         assert (Ce.cpu().numpy() == want_e).all() and (Cc.cpu().numpy().view(np.uint64) == want_c).all(), bits
+
+
+@pytest.mark.parametrize("bits,kmod", [(13, 1), (13, 3), (32, 1), (32, 5), (20, 2)])
+def test_gemm_packed_form_wide_counts_long_tie_sums(bb, oracle, bits, kmod):
+    # the packed form beyond 32-bit totals: the carry form (operand counts < 2^13: bit 31 of the running sum moves into
+    # a second register after every chunk) and 64-bit accumulators (operand counts < 2^32, totals wrap mod 2^64).
+    # Energies take kmod distinct values per operand so that a large share of the K terms tie (kmod = 1: all of them),
+    # and the maximum keeps rising along k for kmod > 1 (resets of both accumulator halves)
+    B, M, N, K = 2, 130, 70, 1500
+    Ae, Ac, Be, Bc = I.gemm_operands(B, M, N, K, seed=300 + bits + kmod, neg_inf_frac=0.02 if kmod > 1 else 0.0)
+    fin_a, fin_b = Ae > -(1 << 29), Be > -(1 << 29)
+    ramp_a = (np.arange(K)[None, None, :] * kmod // K).astype(np.int32)           # rises along k: later chunks beat earlier ones
+    Ae = np.where(fin_a, (Ae % kmod) + ramp_a, Ae).astype(np.int32)
+    Be = np.where(fin_b, Be % kmod, Be).astype(np.int32)
+    Ac = np.where(fin_a, I.splitmix64(7, Ac.size, 40).reshape(Ac.shape) % np.uint64(1 << bits), 0).astype(np.uint64)
+    Bc = np.where(fin_b, I.splitmix64(7, Bc.size, 41).reshape(Bc.shape) % np.uint64(1 << bits), 0).astype(np.uint64)
+    want_e, want_c = _oracle_gemm(oracle, Ae, Ac, Be, Bc)
+    if bits == 13 and kmod == 1:
+        assert int(want_c.max()) > 1 << 33                                      # carries out of bit 31 happened
+    dAe, dAc = _to_dev(Ae, Ac); dBe, dBc = _to_dev(Be, Bc)
+    prev = bb.set_debug_checks(True)
+    try:
+        for cb, eb in ((bits, 7), (bits, 32), (64, 32)):
+            Ce, Cc = bb.tropical_gemm_batched(dAe, dAc, dBe, dBc, count_bits=cb, energy_bits=eb)
+            assert (Ce.cpu().numpy() == want_e).all(), (cb, eb)
+            assert (Cc.cpu().numpy().view(np.uint64) == want_c).all(), (cb, eb)
+    finally:
+        bb.set_debug_checks(prev)
 
 
 def test_gemm_shared_operand_stride0(bb, oracle):
