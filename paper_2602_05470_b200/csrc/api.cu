@@ -369,7 +369,7 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
       launch_fused_tree(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)dp->list_build.p, dp->n_build,
                         (const int32_t *)dp->list_scalar.p, dp->n_scalar, d_assign, n_fixed, B, (const FusedStep *)dp->fused_steps.p,
                         (int)pl.steps.size(), dp->fused_arena, (int)pl.arena_variant_elems, (int)pl.result_offset,
-                        d_energy, d_count, d_mod, rings[ring], st);
+                        d_energy, d_count, d_mod, rings[ring], pl.max_rank, st);
   } else if (!use_graph) {
     for (int ring = 0; ring < n_rings; ring++) enqueue_ring(h, dp, B, d_assign, d_energy, d_count, d_mod, rings[ring], st);
   } else {

@@ -14,10 +14,11 @@
 namespace bbtn {
 namespace {
 
-constexpr int FT = 512;               // threads per CTA
+// threads per CTA = 2^FTB: 256 in general; 128 for the smallest networks (every tensor <= 2^8 elements), where the
+// block barrier between steps is most of a step's time
 
-template <class R>
-__global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const InputRec *__restrict__ inputs,
+template <class R, int FTB>
+__global__ void __launch_bounds__(1 << FTB, 1) fused_tree_kernel(int kind, const InputRec *__restrict__ inputs,
                                                            const int32_t *__restrict__ list_build, int n_build,
                                                            const int32_t *__restrict__ list_scalar, int n_scalar,
                                                            const uint8_t *__restrict__ assign, int n_fixed,
@@ -26,6 +27,7 @@ __global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const Input
                                                            int32_t *__restrict__ energy, uint64_t *__restrict__ count,
                                                            uint32_t *__restrict__ count_mod, int ring) {
   using CT = typename R::T;
+  constexpr int FT = 1 << FTB;
   extern __shared__ __align__(16) unsigned char smem[];
   FusedStep *desc = reinterpret_cast<FusedStep *>(smem);                          // two descriptors, double-buffered
   int32_t *te = reinterpret_cast<int32_t *>(smem + 2 * sizeof(FusedStep));
@@ -81,15 +83,15 @@ __global__ void __launch_bounds__(FT, 1) fused_tree_kernel(int kind, const Input
     const int rO = d.rO, nK = d.nK;
     const int32_t *ae = te + d.offA, *be = te + d.offB;
     const CT *ac = tc + d.offA, *bc = tc + d.offB;
-    // a thread's outputs are o = t + j * FT: the low 9 bits of o never change, their address part is computed once
+    // a thread's outputs are o = t + j * FT: the low log2(FT) bits of o never change, their address part is computed once
     // (unused table entries are 0, so the loops below need no rank tests and unroll into independent loads)
     uint32_t a_lo = 0, b_lo = 0;
 #pragma unroll
-    for (int q = 0; q < 9; q++) { const uint32_t m = 0u - ((t >> q) & 1u); a_lo += d.addA[q] & m; b_lo += d.addB[q] & m; }
+    for (int q = 0; q < FTB; q++) { const uint32_t m = 0u - ((t >> q) & 1u); a_lo += d.addA[q] & m; b_lo += d.addB[q] & m; }
     for (int o = t; o < (1 << rO); o += FT) {
       uint32_t a0 = a_lo, b0 = b_lo;
 #pragma unroll
-      for (int q = 9; q < 13; q++) { const uint32_t m = 0u - ((o >> q) & 1u); a0 += d.addA[q] & m; b0 += d.addB[q] & m; }
+      for (int q = FTB; q < 13; q++) { const uint32_t m = 0u - ((o >> q) & 1u); a0 += d.addA[q] & m; b0 += d.addB[q] & m; }
       int32_t acc_e = NEG_INF; CT acc_c = czero<R>();
       if (nK <= 3) {
 #pragma unroll 4
@@ -141,13 +143,20 @@ size_t fused_tree_smem_bytes(int arena_elems, int ring) {
 void launch_fused_tree(int kind, const InputRec *d_inputs, const int32_t *d_list_build, int n_build,
                        const int32_t *d_list_scalar, int n_scalar, const uint8_t *d_assign, int n_fixed, int64_t B,
                        const FusedStep *d_steps, int n_steps, int arena_elems, int inv_base, int result_off,
-                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, cudaStream_t st) {
+                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, int max_rank, cudaStream_t st) {
   const size_t smem = fused_tree_smem_bytes(arena_elems, ring);
   BBTN_RING_DISPATCH(ring, {
-    cudaFuncSetAttribute(fused_tree_kernel<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    fused_tree_kernel<R><<<(unsigned)B, FT, smem, st>>>(kind, d_inputs, d_list_build, n_build, d_list_scalar, n_scalar, d_assign,
-                                                        n_fixed, d_steps, n_steps, arena_elems, inv_base, result_off, energy,
-                                                        count, count_mod, ring);
+    if (max_rank <= 8) {
+      cudaFuncSetAttribute(fused_tree_kernel<R, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      fused_tree_kernel<R, 7><<<(unsigned)B, 128, smem, st>>>(kind, d_inputs, d_list_build, n_build, d_list_scalar, n_scalar, d_assign,
+                                                              n_fixed, d_steps, n_steps, arena_elems, inv_base, result_off, energy,
+                                                              count, count_mod, ring);
+    } else {
+      cudaFuncSetAttribute(fused_tree_kernel<R, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      fused_tree_kernel<R, 8><<<(unsigned)B, 256, smem, st>>>(kind, d_inputs, d_list_build, n_build, d_list_scalar, n_scalar, d_assign,
+                                                              n_fixed, d_steps, n_steps, arena_elems, inv_base, result_off, energy,
+                                                              count, count_mod, ring);
+    }
   });
 }
 

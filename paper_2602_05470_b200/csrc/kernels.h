@@ -80,7 +80,7 @@ size_t fused_tree_smem_bytes(int arena_elems, int ring);
 void launch_fused_tree(int kind, const InputRec *d_inputs, const int32_t *d_list_build, int n_build,
                        const int32_t *d_list_scalar, int n_scalar, const uint8_t *d_assign, int n_fixed, int64_t B,
                        const FusedStep *d_steps, int n_steps, int arena_elems, int inv_base, int result_off,
-                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, cudaStream_t st);
+                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, int max_rank, cudaStream_t st);
 
 // K4: (E[b], c[b]) = offset[b] (.) root[b]; canonicalise; convert to reported units.
 //   root_e == nullptr: the network is all scalars.  root_stride 0: root is leaf-invariant.
