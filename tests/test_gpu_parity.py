@@ -848,8 +848,12 @@ def test_search_mode_drivers_and_large_kings(bb, oracle):
         bb.Handle(k, flags=bb.BBTN_SEARCH_ONLY | bb.BBTN_COUNT_CRT)
     h.close()
     # MIS size of the 36x36 and 40x40 King's subgraphs (goldens by the oracle's sparse DP): 4 B per element
-    for L, name in ((36, "config5-shape king 36x36 p0.8 seed 1"), (40, "config5 king 40x40 p0.8 seed 1")):
-        h = bb.Handle(I.kings_subgraph(L, L, 0.8, 1), flags=bb.BBTN_SEARCH_ONLY)
+    for L, seed, name in ((36, 1, "config5-shape king 36x36 p0.8 seed 1"), (40, 1, "config5 king 40x40 p0.8 seed 1"),
+                          (40, 3, "config5 king 40x40 p0.8 seed 3")):
+        k = I.kings_subgraph(L, L, 0.8, seed)
+        h = bb.Handle(k, flags=bb.BBTN_SEARCH_ONLY)
+        if seed != 1:
+            h.add_sweep_order(I.column_major_order(k))
         out = h.solve_local(32)
         assert out["energy"] == int(_goldens()[name]["energy"]) and out["count"] == 0, out
         h.close()
