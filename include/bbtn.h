@@ -66,7 +66,7 @@ typedef enum {
 #define BBTN_NO_GRAPH  0x4u   /* launch kernels one by one instead of replaying a CUDA graph       */
 #define BBTN_FORCE_STREAMING 0x10u /* tuning/testing: never use the tiled GEMM + permute path          */
 #define BBTN_FORCE_TILED     0x20u /* tuning/testing: permute + tiled GEMM wherever an index is summed */
-#define BBTN_NO_FUSED        0x80u /* tuning/testing: never run a small network as one shared-memory launch (one CTA per leaf) */
+#define BBTN_NO_FUSED        0x80u /* tuning/testing: never run a small network, or the small subtrees of a larger one, as a shared-memory launch (one CTA per leaf) */
 #define BBTN_SEARCH_ONLY     0x40u /* ground-state SEARCH ("the tropical number inf for optimization problems",
                                       :81-91): plain max-plus, no count plane anywhere (4 B per element instead of 12);
                                       the batched calls and the solve drivers return the optimal energy only, every

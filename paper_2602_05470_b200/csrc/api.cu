@@ -73,6 +73,8 @@ int check_gemm_shape(int64_t batch, int32_t M, int32_t N, int32_t count_bits, in
   return BBTN_OK;
 }
 
+void prepare_hybrid(bbtn_handle *h, DevPlan *dp);
+
 int get_plan(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, bool enforce, DevPlan **out) {
   if (n_fixed < 0 || (n_fixed > 0 && !fixed)) return fail(h, BBTN_EINVAL, "bad fixed set");
   std::vector<int32_t> key(fixed, fixed + n_fixed);
@@ -82,6 +84,7 @@ int get_plan(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, bool enforce
     std::string err;
     int rc = make_plan(h->P, key, h->force_mode, false, dp->plan, err);
     if (rc) return fail(h, rc, err);
+    prepare_hybrid(h, dp.get());
     it = h->plans.emplace(key, std::move(dp)).first;
   }
   DevPlan *dp = it->second.get();
@@ -112,8 +115,30 @@ int upload_tables(bbtn_handle *h, DevPlan *dp) {
     CUDA_TRY(h, cudaMemcpy(dp->list_scalar.p, pl.scalar_inputs.data(), pl.scalar_inputs.size() * 4, cudaMemcpyHostToDevice));
   CUDA_TRY(h, dp->inv_e.ensure((size_t)pl.arena_invariant_elems * 4));
   CUDA_TRY(h, dp->inv_c.ensure((h->P.flags & BBTN_SEARCH_ONLY) ? 0 : (size_t)pl.arena_invariant_elems * 8));
+  if (dp->hybrid == 1)
+    for (auto &g : dp->hyb) {
+      if (g.steps.empty()) continue;
+      CUDA_TRY(h, g.d_steps.ensure(g.steps.size() * sizeof(FusedStep)));
+      CUDA_TRY(h, cudaMemcpy(g.d_steps.p, g.steps.data(), g.steps.size() * sizeof(FusedStep), cudaMemcpyHostToDevice));
+      CUDA_TRY(h, g.d_build.upload(g.build));
+      CUDA_TRY(h, g.d_build_off.upload(g.build_off));
+    }
   dp->tables_ready = true;
   return BBTN_OK;
+}
+
+// descriptor of one streaming step with shared-memory operand offsets (fused_tree.cu)
+FusedStep make_fused_step(const Step &s, int64_t offA, int64_t offB, int64_t offC) {
+  FusedStep f;
+  std::memset(&f, 0, sizeof(f));
+  f.rO = s.rO; f.nK = s.nK; f.gout = -1;
+  f.offA = (int32_t)offA; f.offB = (int32_t)offB; f.offC = (int32_t)offC;
+  for (int q = 0; q < s.rO; q++) { f.addA[q] = (uint16_t)s.addA[q]; f.addB[q] = (uint16_t)s.addB[q]; }
+  for (int j = 0; j < s.nK; j++) { f.kA[j] = (uint16_t)s.kA[j]; f.kB[j] = (uint16_t)s.kB[j]; }
+  if (s.nK <= 3)
+    for (int k = 0; k < (1 << s.nK); k++)
+      for (int j = 0; j < s.nK; j++) if ((k >> j) & 1) { f.kkA[k] += (uint16_t)s.kA[j]; f.kkB[k] += (uint16_t)s.kB[j]; }
+  return f;
 }
 
 // Can the plan run as one launch with every tensor of a leaf in shared memory?  (fused_tree.cu)
@@ -131,18 +156,8 @@ int prepare_fused(bbtn_handle *h, DevPlan *dp) {
   std::vector<FusedStep> fs;
   for (const Step &s : pl.steps) {
     if ((s.kind != STEP_ABSORB && s.kind != STEP_REDUCE) || s.rO > 13 || s.nK > 13 || s.n_slice) return BBTN_OK;
-    FusedStep f;
-    std::memset(&f, 0, sizeof(f));
-    f.rO = s.rO; f.nK = s.nK;
-    f.offA = (int32_t)((s.vA ? 0 : pl.arena_variant_elems) + s.offA);
-    f.offB = (int32_t)((s.vB ? 0 : pl.arena_variant_elems) + s.offB);
-    f.offC = (int32_t)((s.vC ? 0 : pl.arena_variant_elems) + s.offC);
-    for (int q = 0; q < s.rO; q++) { f.addA[q] = (uint16_t)s.addA[q]; f.addB[q] = (uint16_t)s.addB[q]; }
-    for (int j = 0; j < s.nK; j++) { f.kA[j] = (uint16_t)s.kA[j]; f.kB[j] = (uint16_t)s.kB[j]; }
-    if (s.nK <= 3)
-      for (int k = 0; k < (1 << s.nK); k++)
-        for (int j = 0; j < s.nK; j++) if ((k >> j) & 1) { f.kkA[k] += (uint16_t)s.kA[j]; f.kkB[k] += (uint16_t)s.kB[j]; }
-    fs.push_back(f);
+    fs.push_back(make_fused_step(s, (s.vA ? 0 : pl.arena_variant_elems) + s.offA, (s.vB ? 0 : pl.arena_variant_elems) + s.offB,
+                                 (s.vC ? 0 : pl.arena_variant_elems) + s.offC));
   }
   std::vector<int32_t> lb;
   for (size_t t = 0; t < pl.inputs.size(); t++) if (pl.inputs[t].rank > 0) lb.push_back((int32_t)t);
@@ -152,6 +167,126 @@ int prepare_fused(bbtn_handle *h, DevPlan *dp) {
   dp->n_build = (int)lb.size(); dp->fused_arena = (int)arena;
   dp->fused = 1;
   return BBTN_OK;
+}
+
+// first-fit allocator over shared-memory element offsets (blocks are multiples of 4 elements)
+struct SmallArena {
+  std::map<int, int> free_; int top = 0;
+  static int r4(int n) { return (n + 3) & ~3; }
+  int alloc(int n) {
+    n = r4(n);
+    for (auto it = free_.begin(); it != free_.end(); ++it)
+      if (it->second >= n) { const int off = it->first, rest = it->second - n; free_.erase(it); if (rest) free_[off + n] = rest; return off; }
+    if (!free_.empty()) {
+      auto last = std::prev(free_.end());
+      if (last->first + last->second == top) { const int off = last->first; top = off + n; free_.erase(last); return off; }
+    }
+    const int off = top; top += n; return off;
+  }
+  void release(int off, int n) {
+    n = r4(n);
+    auto it = free_.emplace(off, n).first;
+    auto nx = std::next(it);
+    if (nx != free_.end() && it->first + it->second == nx->first) { it->second += nx->second; free_.erase(nx); }
+    if (it != free_.begin()) { auto pv = std::prev(it); if (pv->first + pv->second == it->first) { pv->second += it->second; free_.erase(it); } }
+  }
+};
+
+// Larger plans: most tree nodes are tiny (a few hundred elements) and, launched one by one, cost a few microseconds of
+// latency each.  A node is SMALL if it is a streaming node and every tensor of its subtree has at most 2^R elements;
+// the maximal small subtrees run in shared memory as a prologue (fused_tree.cu, one CTA per leaf for those that end in
+// a leaf-dependent tensor, one CTA for the leaf-invariant ones) and write the tensor they end in to fresh storage
+// behind the planned arenas (their planned slots may still be occupied that early); the remaining nodes keep their
+// per-node launches with those operands re-pointed.  Host logic only; R is the largest of 12 .. 8 that fits.
+void prepare_hybrid(bbtn_handle *h, DevPlan *dp) {
+  if (dp->hybrid >= 0) return;
+  dp->hybrid = 0;
+  Plan &pl = dp->plan;
+  if ((h->P.flags & BBTN_NO_FUSED) || pl.steps.size() < 48) return;
+  if (pl.max_rank <= 13 && pl.arena_variant_elems + pl.arena_invariant_elems <= 60000) return;   // a candidate for the one-launch form
+  const int n_in = (int)pl.inputs.size(), n_st = (int)pl.steps.size();
+  std::map<std::pair<int, int64_t>, int> owner;              // (arena, offset) -> the tensor stored there right now
+  for (int t = 0; t < n_in; t++) if (pl.inputs[t].rank > 0) owner[{pl.inputs[t].variant, pl.inputs[t].offset}] = t;
+  std::vector<int> opA(n_st, -1), opB(n_st, -1), consumer(n_in + n_st, -1);
+  for (int s = 0; s < n_st; s++) {
+    const Step &st = pl.steps[s];
+    if (st.n_slice || st.xA || st.xB) return;
+    auto fa = owner.find({st.vA, st.offA});
+    if (fa == owner.end()) return;
+    opA[s] = fa->second; consumer[opA[s]] = s;
+    if (st.kind != STEP_PERMUTE) {
+      auto fb = owner.find({st.vB, st.offB});
+      if (fb == owner.end()) return;
+      opB[s] = fb->second; consumer[opB[s]] = s;
+    }
+    owner[{st.vC, st.offC}] = n_in + s;
+  }
+  const int64_t smem_cap = 227 * 1024 - 2048;
+  for (int R = 12; R >= 8; R--) {
+    std::vector<char> small(n_in + n_st, 0);
+    for (int t = 0; t < n_in; t++) small[t] = pl.inputs[t].rank > 0 && pl.inputs[t].rank <= R;
+    int n_small = 0; bool whole = false;
+    for (int s = 0; s < n_st; s++) {
+      const Step &st = pl.steps[s];
+      small[n_in + s] = (st.kind == STEP_ABSORB || st.kind == STEP_REDUCE) && st.rO <= R && st.nK <= 13 && st.rA <= R && st.rB <= R &&
+                        small[opA[s]] && opB[s] >= 0 && small[opB[s]];
+      if (small[n_in + s]) { n_small++; if (consumer[n_in + s] < 0) whole = true; }
+    }
+    if (whole) return;                                       // the whole tree is small: the one-launch form takes it
+    if (n_small < 24) return;
+    // group of every small step = leaf dependence of the tensor its subtree ends in
+    std::vector<int> grp(n_st, -1); std::vector<char> root(n_st, 0);
+    for (int s = n_st - 1; s >= 0; s--) {
+      if (!small[n_in + s]) continue;
+      const int c = consumer[n_in + s];
+      if (!small[n_in + c]) { root[s] = 1; grp[s] = pl.steps[s].vC ? 1 : 0; } else grp[s] = grp[c];
+    }
+    DevPlan::HybridGroup gnew[2];
+    std::vector<int64_t> newoff(n_st, -1);
+    int64_t ext[2] = {0, 0};
+    bool fits = true;
+    for (int g = 0; g < 2 && fits; g++) {
+      SmallArena sm; std::map<int, int> loc;
+      for (int s = 0; s < n_st; s++) {
+        if (grp[s] != g) continue;
+        for (int op : {opA[s], opB[s]})
+          if (op < n_in && !loc.count(op)) { loc[op] = sm.alloc(1 << pl.inputs[op].rank); gnew[g].build.push_back(op); gnew[g].build_off.push_back(loc[op]); }
+      }
+      for (int s = 0; s < n_st; s++) {
+        if (grp[s] != g) continue;
+        const Step &st = pl.steps[s];
+        const int offC = sm.alloc(1 << st.rO);
+        FusedStep f = make_fused_step(st, loc[opA[s]], loc[opB[s]], offC);
+        for (int op : {opA[s], opB[s]}) if (op >= n_in) sm.release(loc[op], 1 << pl.steps[op - n_in].rO);
+        loc[n_in + s] = offC;
+        if (root[s]) {
+          const int64_t base = g ? pl.arena_variant_elems : pl.arena_invariant_elems;
+          newoff[s] = base + ext[g];
+          ext[g] += (((int64_t)1 << st.rO) + 3) & ~(int64_t)3;
+          f.gout = (newoff[s] << 1) | g;
+          sm.release(offC, 1 << st.rO);
+        }
+        gnew[g].steps.push_back(f);
+        gnew[g].max_rank = std::max(gnew[g].max_rank, (int)st.rO);
+      }
+      gnew[g].arena = sm.top;
+      if ((int64_t)fused_tree_smem_bytes(sm.top, RING_U64) > smem_cap) fits = false;
+    }
+    if (!fits) continue;
+    for (int s = 0; s < n_st; s++) {
+      if (small[n_in + s]) continue;
+      Step st = pl.steps[s];
+      if (opA[s] >= n_in && newoff[opA[s] - n_in] >= 0) st.offA = newoff[opA[s] - n_in];
+      if (opB[s] >= n_in && newoff[opB[s] - n_in] >= 0) st.offB = newoff[opB[s] - n_in];
+      dp->hyb_big.push_back(st);
+    }
+    for (int g = 0; g < 2; g++) { dp->hyb[g].steps = std::move(gnew[g].steps); dp->hyb[g].build = std::move(gnew[g].build);
+                                  dp->hyb[g].build_off = std::move(gnew[g].build_off); dp->hyb[g].arena = gnew[g].arena; dp->hyb[g].max_rank = gnew[g].max_rank; }
+    pl.arena_invariant_elems += ext[0]; pl.arena_variant_elems += ext[1];
+    dp->hyb_rank = R;
+    dp->hybrid = 1;
+    return;
+  }
 }
 
 int ensure_batch(bbtn_handle *h, DevPlan *dp, int64_t B, bool host_io) {
@@ -192,7 +327,17 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
   while (energy_bits < 32 && ((int64_t)1 << energy_bits) <= h->P.energy_range) energy_bits++;
   auto pe = [&](int v, int64_t off) { return v ? ve + off * B : ie + off; };
   auto pc = [&](int v, int64_t off) { return (void *)(v ? vc + (size_t)off * B * csz : ic + (size_t)off * csz); };
-  for (const Step &s : pl.steps) {
+  if (dp->hybrid == 1)                                   // the small subtrees of every leaf, in shared memory (prepare_hybrid)
+    for (int g = 0; g < 2; g++) {
+      const DevPlan::HybridGroup &hg = dp->hyb[g];
+      if (hg.steps.empty()) continue;
+      FusedGlobal fg;
+      fg.build_off = (const int32_t *)hg.d_build_off.p; fg.ve = ve; fg.vc = vc; fg.ie = ie; fg.ic = ic; fg.finalize = 0;
+      launch_fused_tree(h->P.kind, (const InputRec *)dp->inputs.p, (const int32_t *)hg.d_build.p, (int)hg.build.size(), nullptr, 0,
+                        d_assign, (int)pl.fixed.size(), g ? B : 1, (const FusedStep *)hg.d_steps.p, (int)hg.steps.size(), hg.arena, 0, -1,
+                        nullptr, nullptr, nullptr, ring, hg.max_rank, st, fg);
+    }
+  for (const Step &s : dp->hybrid == 1 ? dp->hyb_big : pl.steps) {
     const int64_t nb = s.variant ? B : 1;
     switch (s.kind) {
       case STEP_ABSORB:
@@ -301,6 +446,8 @@ int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, int64
   for (const InputRec &r : pl.inputs) if (r.rank > 0) (r.variant ? n_var : n_inv)++;
   // K1: variant tensors, invariant tensors, offset[b]; K4: finalize
   info->n_kernel_launches = (int32_t)pl.steps.size() + (n_var > 0) + (n_inv > 0) + 2;
+  if (dp->hybrid == 1)                                   // small subtrees run as one or two shared-memory prologue launches
+    info->n_kernel_launches = (int32_t)dp->hyb_big.size() + !dp->hyb[0].steps.empty() + !dp->hyb[1].steps.empty() + (n_var > 0) + (n_inv > 0) + 2;
   return BBTN_OK;
 }
 
@@ -363,6 +510,10 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
   int n_rings = 1;
   if (!search && crt && d_mod) { if (stream_only) { rings[1] = RING_P12; n_rings = 2; } else n_rings = 3; }
   const bool use_graph = allow_graph && !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
+  for (int ring = 0; ring < n_rings; ring++) {             // shared-memory opt-in of the kernels that keep a leaf's tensors on chip
+    if (dp->fused == 1) configure_fused_tree(rings[ring], dp->plan.max_rank);
+    if (dp->hybrid == 1) for (auto &g : dp->hyb) if (!g.steps.empty()) configure_fused_tree(rings[ring], g.max_rank);
+  }
   if (dp->fused == 1) {
     const Plan &pl = dp->plan;
     for (int ring = 0; ring < n_rings; ring++)

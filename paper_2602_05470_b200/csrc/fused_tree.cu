@@ -25,7 +25,8 @@ __global__ void __launch_bounds__(1 << FTB, 1) fused_tree_kernel(int kind, const
                                                            const FusedStep *__restrict__ steps, int n_steps,
                                                            int arena_elems, int inv_base, int result_off,
                                                            int32_t *__restrict__ energy, uint64_t *__restrict__ count,
-                                                           uint32_t *__restrict__ count_mod, int ring) {
+                                                           uint32_t *__restrict__ count_mod, int ring, const FusedGlobal g,
+                                                           int64_t Bn) {
   using CT = typename R::T;
   constexpr int FT = 1 << FTB;
   extern __shared__ __align__(16) unsigned char smem[];
@@ -54,14 +55,14 @@ __global__ void __launch_bounds__(1 << FTB, 1) fused_tree_kernel(int kind, const
   for (int i = t; i < n_build; i += FT) {
     const InputRec r = inputs[list_build[i]];
     const int fu_val = r.fu >= 0 ? asg[r.fu] : 0, fv_val = r.fv >= 0 ? asg[r.fv] : 0;
-    const int base = (r.variant ? 0 : inv_base) + (int)r.offset;
+    const int base = g.build_off ? g.build_off[i] : (r.variant ? 0 : inv_base) + (int)r.offset;
     for (int x = 0; x < (1 << r.rank); x++) {
       int32_t e; CT c;
       input_element<R>(kind, r, fu_val, fv_val, r.bu >= 0 ? (x >> r.bu) & 1 : 0, r.bv >= 0 ? (x >> r.bv) & 1 : 0, e, c);
       te[base + x] = e; stc<R>(tc, base + x, c);
     }
   }
-  if (t == 0) {
+  if (t == 0 && g.finalize) {
     int32_t acc_e = 0; CT acc_c = R::from_small(1);
     for (int i = 0; i < n_scalar; i++) {
       const InputRec r = inputs[list_scalar[i]];
@@ -108,9 +109,16 @@ __global__ void __launch_bounds__(1 << FTB, 1) fused_tree_kernel(int kind, const
       }
       canonicalise<R>(acc_e, acc_c);
       te[d.offC + o] = acc_e; stc<R>(tc, d.offC + o, acc_c);
+      if (d.gout >= 0) {                                 // a tensor the rest of the tree reads from the global arena
+        const bool var = d.gout & 1;
+        const int64_t gi = var ? (d.gout >> 1) * Bn + (b << rO) + o : (d.gout >> 1) + o;
+        (var ? g.ve : g.ie)[gi] = acc_e;
+        stc<R>(reinterpret_cast<CT *>(var ? g.vc : g.ic), gi, acc_c);
+      }
     }
     __syncthreads();
   }
+  if (!g.finalize) return;
 
   // ---- K4: offset (.) root, canonical, reported units
   if (t == 0) {
@@ -140,22 +148,34 @@ size_t fused_tree_smem_bytes(int arena_elems, int ring) {
   return 2 * sizeof(FusedStep) + (((size_t)arena_elems * 4 + 15) & ~(size_t)15) + (size_t)arena_elems * csz + 16;
 }
 
+// Opt in to the device's maximum dynamic shared memory for the instantiation (ring, max_rank) will launch.  Call it
+// outside any stream capture, before launch_fused_tree.
+void configure_fused_tree(int ring, int max_rank) {
+  int dev = 0, max_smem = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  max_smem -= 1024;                                        // the kernel's static shared memory counts against the same limit
+  BBTN_RING_DISPATCH(ring, {
+    if (max_rank <= 8) cudaFuncSetAttribute(fused_tree_kernel<R, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    else cudaFuncSetAttribute(fused_tree_kernel<R, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+  });
+}
+
 void launch_fused_tree(int kind, const InputRec *d_inputs, const int32_t *d_list_build, int n_build,
                        const int32_t *d_list_scalar, int n_scalar, const uint8_t *d_assign, int n_fixed, int64_t B,
                        const FusedStep *d_steps, int n_steps, int arena_elems, int inv_base, int result_off,
-                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, int max_rank, cudaStream_t st) {
+                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, int max_rank, cudaStream_t st,
+                       const FusedGlobal &g) {
   const size_t smem = fused_tree_smem_bytes(arena_elems, ring);
   BBTN_RING_DISPATCH(ring, {
     if (max_rank <= 8) {
-      cudaFuncSetAttribute(fused_tree_kernel<R, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       fused_tree_kernel<R, 7><<<(unsigned)B, 128, smem, st>>>(kind, d_inputs, d_list_build, n_build, d_list_scalar, n_scalar, d_assign,
                                                               n_fixed, d_steps, n_steps, arena_elems, inv_base, result_off, energy,
-                                                              count, count_mod, ring);
+                                                              count, count_mod, ring, g, B);
     } else {
-      cudaFuncSetAttribute(fused_tree_kernel<R, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       fused_tree_kernel<R, 8><<<(unsigned)B, 256, smem, st>>>(kind, d_inputs, d_list_build, n_build, d_list_scalar, n_scalar, d_assign,
                                                               n_fixed, d_steps, n_steps, arena_elems, inv_base, result_off, energy,
-                                                              count, count_mod, ring);
+                                                              count, count_mod, ring, g, B);
     }
   });
 }

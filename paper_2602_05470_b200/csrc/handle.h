@@ -43,6 +43,17 @@ struct DevPlan {
   DevBuf fused_steps, list_build;
   int fused = -1;                               // -1 not decided yet, 0 no, 1 yes
   int n_build = 0, fused_arena = 0;
+  // larger networks: the SMALL SUBTREES of the plan (every tensor <= 2^hyb_rank elements) run as a shared-memory prologue,
+  // one CTA per leaf (group 1: subtrees that end in a leaf-dependent tensor) or one CTA (group 0: leaf-invariant ones),
+  // and only the rest of the tree as per-node launches (api.cu prepare_hybrid)
+  int hybrid = -1;                              // -1 not decided yet, 0 no, 1 yes
+  struct HybridGroup {
+    std::vector<FusedStep> steps; std::vector<int32_t> build, build_off;
+    int arena = 0, max_rank = 0;
+    DevBuf d_steps, d_build, d_build_off;
+  } hyb[2];
+  std::vector<Step> hyb_big;                    // the steps that stay per-node launches, operands re-pointed at the prologue's outputs
+  int hyb_rank = 0;
   bool tables_ready = false;
   int64_t B_cap = 0;
   std::vector<cudaGraphExec_t> graphs;          // per ring, for graph_B

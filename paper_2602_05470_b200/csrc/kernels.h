@@ -75,12 +75,24 @@ struct FusedStep {
   int32_t rO, nK, offA, offB, offC, pad;
   uint16_t addA[16], addB[16], kA[16], kB[16];   // unused entries are 0
   uint16_t kkA[8], kkB[8];                        // nK <= 3: the summed offsets of every k, ready to add
+  int64_t gout;                                   // -1, or (global element offset << 1) | variant: the output also goes to the arena
+};
+// The same kernel as a PROLOGUE of a larger plan (api.cu prepare_hybrid): it contracts the small subtrees of every
+// leaf in shared memory and writes the tensor each of them ends in to the global arena, where the per-node launches
+// of the rest of the tree pick it up.  build_off != nullptr: shared-memory offsets of the inputs to build (parallel
+// to list_build); steps with gout >= 0 store their output at ve + off * B + b * 2^rO (variant) or ie + off; finalize = 0.
+struct FusedGlobal {
+  const int32_t *build_off = nullptr;
+  int32_t *ve = nullptr; void *vc = nullptr; int32_t *ie = nullptr; void *ic = nullptr;
+  int finalize = 1;
 };
 size_t fused_tree_smem_bytes(int arena_elems, int ring);
+void configure_fused_tree(int ring, int max_rank);     // outside stream capture, before the first launch of that instantiation
 void launch_fused_tree(int kind, const InputRec *d_inputs, const int32_t *d_list_build, int n_build,
                        const int32_t *d_list_scalar, int n_scalar, const uint8_t *d_assign, int n_fixed, int64_t B,
                        const FusedStep *d_steps, int n_steps, int arena_elems, int inv_base, int result_off,
-                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, int max_rank, cudaStream_t st);
+                       int32_t *energy, uint64_t *count, uint32_t *count_mod, int ring, int max_rank, cudaStream_t st,
+                       const FusedGlobal &g = FusedGlobal());
 
 // K4: (E[b], c[b]) = offset[b] (.) root[b]; canonicalise; convert to reported units.
 //   root_e == nullptr: the network is all scalars.  root_stride 0: root is leaf-invariant.

@@ -605,6 +605,62 @@ def test_config4b_full_size_leaf_by_leaf(bb, oracle, f):
     assert bb.oplus_combine("ising", energy, count)[:2] == _expect("config4b ising 5x5x5 seed 1")
 
 
+@pytest.mark.parametrize("case", ["cube-crt", "ising24-crt", "king16-crt", "cube-search", "ising14-tiled"])
+def test_small_subtrees_run_as_shared_memory_prologue(bb, oracle, case):
+    # larger plans run their small subtrees (every tensor <= 2^12 elements) as one or two shared-memory launches and only
+    # the rest of the tree node by node (api.cu prepare_hybrid): far fewer launches than tree nodes, the same integers
+    # as the per-node form (BBTN_NO_FUSED) on every leaf, and the oracle's on sampled leaves -- all three count rings
+    if case.startswith("cube"):
+        inst = I.ising_lattice_3d(4, 4, 5, 2); f = 4
+        fixed = I.layer_fixed_set_3d(4, 4, 5, f)
+        tree = I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+    elif case.startswith("ising24"):
+        inst = I.ising_lattice_2d(24, 24, 5, field_h=1); f = 8
+        fixed = I.slit_fixed_set_2d(24, 24, f)
+        tree = I.elimination_tree(inst.input_index_sets(fixed), I.slit_angular_order_2d(24, 24, f))
+    elif case.startswith("king16"):
+        inst = I.kings_subgraph(16, 16, 0.8, 3, weights="rand"); f = 5
+        ids = _king_ids(inst, 16, 16)
+        fixed = np.array([ids[r][8] for r in range(16) if ids[r][8] >= 0][:f], np.int32)
+        tree = None
+    else:
+        inst = I.ising_lattice_2d(14, 14, 6); f = 3
+        ids = None
+        fixed = np.array([2 * 14 + 2, 2 * 14 + 11, 11 * 14 + 3], np.int32)
+        parts = I.lattice_block_parts(14, 14, [7], [7], None, exclude=fixed)
+        tree = I.grouped_elimination_tree(inst.input_index_sets(fixed), parts)
+    assign = I.all_assignments(len(fixed))
+    search = case.endswith("search")
+    base = bb.BBTN_SEARCH_ONLY if search else (bb.BBTN_COUNT_CRT if case.endswith("crt") else 0)
+    h = bb.Handle(inst, tree=tree, flags=base)
+    info = h.plan_query(fixed, len(assign))
+    assert info["n_kernel_launches"] < info["n_nodes"] // 2, info       # the prologue is active
+    got = h.contract_batch(fixed, assign)
+    got2 = h.contract_batch(fixed, assign[::-1].copy())                   # again (CUDA graph replay), other leaves
+    h.close()
+    h0 = bb.Handle(inst, tree=tree, flags=base | bb.BBTN_NO_FUSED)
+    info0 = h0.plan_query(fixed, len(assign))
+    assert info0["n_kernel_launches"] > info0["n_nodes"]
+    ref = h0.contract_batch(fixed, assign)
+    h0.close()
+    for x, y in zip(got, ref):
+        assert (x == y).all(), case
+    for x, y in zip(got2, ref):
+        assert (x == y[::-1]).all(), case
+    tl, tr = tree if tree is not None else (None, None)
+    for b in _sampled_leaves(len(assign), 6, 17):
+        if tree is not None:
+            we, wc = oracle.contract_tree(inst, tl, tr, fixed, assign[b])
+        else:
+            we, wc = oracle.frontier_dp(inst, None, fixed, assign[b])
+            we = NEG_INF if we is None else we
+        assert int(got[0][b]) == we, (case, b)
+        if not search:
+            assert int(got[1][b]) == wc & MASK64, (case, b)
+            if case.endswith("crt"):
+                assert (int(got[2][b, 0]), int(got[2][b, 1])) == (wc % bb.BBTN_P1, wc % bb.BBTN_P2), (case, b)
+
+
 def test_config3_full_size_24x24_all_leaves(bb):
     # the launch configuration time_to_solve.py times: slit of f spins, all 2^f leaves in one call
     from paper_2602_05470_b200 import time_to_solve as T
