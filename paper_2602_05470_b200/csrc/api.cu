@@ -505,7 +505,7 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
   // CRT mode: the two prime rings run as ONE pass (both residues in one 64-bit count) unless the plan holds a
   // permute or tiled-GEMM step, whose kernels exist for the single-prime rings only
   bool stream_only = true;
-  for (const Step &s : dp->plan.steps) if (s.kind == STEP_PERMUTE || s.kind == STEP_GEMM) stream_only = false;
+  for (const Step &s : dp->plan.steps) if (s.kind == STEP_GEMM) stream_only = false;      // (K2 moves the packed residues as 64-bit words)
   int rings[3] = {search ? (int)RING_NONE : (int)RING_U64, RING_P1, RING_P2};
   int n_rings = 1;
   if (!search && crt && d_mod) { if (stream_only) { rings[1] = RING_P12; n_rings = 2; } else n_rings = 3; }

@@ -285,6 +285,7 @@ struct Planner {
   std::vector<char> used;
   std::vector<int32_t> tl, tr;
   // local planning: operands that must outlive the step (they are read again by the next slice)
+  bool gather_friendly_b = false;                      // make_plan only: re-lay a mid-sized gathered operand (see do_step)
   struct Deferred { bool variant; int64_t off, ne; };
   std::vector<Deferred> deferred;                      // storage to give back when the sliced segment ends
 
@@ -434,17 +435,41 @@ struct Planner {
       O.idx.clear();
       for (int lab : A.idx) if (inO(lab)) O.idx.push_back(lab);
       for (int lab : nl) O.idx.push_back(lab);
+      // The gathered operand is read at fb(o): its layout decides how many sectors a warp's loads touch.  A mid-sized B
+      // (256+ elements) under a large output is first re-laid (K2) with its surviving indices in the ORDER OF THE OUTPUT
+      // (then consecutive outputs read the same or consecutive elements) and the summed ones on top; without this the L1
+      // data pipe, not HBM, bounds the write-heavy steps of balanced trees (7 sectors per load request on the cube).
+      std::vector<int> b_idx = B.idx;
+      int64_t b_off = B.off; bool b_tmp = false;
+      if (gather_friendly_b && rO >= 16 && rB >= 8 && rB + 2 <= rO && B.phys.empty() && !B.ext && B.slice.empty() && rB <= 31) {
+        std::vector<int> want;
+        for (int lab : O.idx) if (pos_of(B.idx, lab) >= 0) want.push_back(lab);
+        want.insert(want.end(), kl.begin(), kl.end());
+        const size_t head = std::min<size_t>(want.size(), 7);
+        if (!std::equal(want.begin(), want.begin() + head, B.idx.begin())) {
+          Step ps;
+          ps.kind = STEP_PERMUTE; ps.variant = B.variant; ps.rO = rB;
+          for (size_t j = 0; j < want.size(); j++) ps.perm[j] = pos_of(B.idx, want[j]);
+          b_off = (B.variant ? av : ai).alloc((int64_t)1 << rB);
+          ps.offA = B.off; ps.offC = b_off; ps.vA = ps.vC = B.variant; ps.rA = ps.rO;
+          ps.bytes = 24.0 * (double)((int64_t)1 << rB);
+          (B.variant ? out.bytes_variant : out.bytes_invariant) += ps.bytes;
+          out.steps.push_back(ps);
+          b_idx = want; b_tmp = true;
+        }
+      }
+      auto bit_b = [&](int pos) { return b_tmp ? (pos < 32 ? (1u << pos) : 0u) : bit_of(B, pos); };
       for (int p = 0; p < rO && p < 32; p++) {              // ranks above 32 occur only in dry runs (rho of an unsliced tree)
-        int pa = pos_of(A.idx, O.idx[p]), pb = pos_of(B.idx, O.idx[p]);
+        int pa = pos_of(A.idx, O.idx[p]), pb = pos_of(b_idx, O.idx[p]);
         st.addA[p] = pa >= 0 ? bit_of(A, pa) : 0u;
-        st.addB[p] = pb >= 0 ? bit_of(B, pb) : 0u;
+        st.addB[p] = pb >= 0 ? bit_b(pb) : 0u;
       }
       for (int j = 0; j < lk && j < 32; j++) {
         st.kA[j] = bit_of(A, pos_of(A.idx, kl[j]));
-        st.kB[j] = bit_of(B, pos_of(B.idx, kl[j]));
+        st.kB[j] = bit_b(pos_of(b_idx, kl[j]));
       }
       O.off = ao.alloc((int64_t)1 << rO);
-      st.offA = A.off; st.offB = B.off; st.offC = O.off;
+      st.offA = A.off; st.offB = b_off; st.offC = O.off;
       st.vA = A.variant; st.vB = B.variant; st.vC = var;
       st.rA = rA; st.rB = rB;
       st.n_slice = (int32_t)std::max(A.slice.size(), B.slice.size());
@@ -456,6 +481,7 @@ struct Planner {
       st.bytes = 12.0 * ((double)((int64_t)1 << rA) + (double)((int64_t)1 << rB) + (double)((int64_t)1 << rO));
       (var ? out.bytes_variant : out.bytes_invariant) += st.bytes;
       out.steps.push_back(st);
+      if (b_tmp) (B.variant ? av : ai).release(b_off, (int64_t)1 << rB);      // the re-laid copy is scratch of this step
       release(A); release(B);
     } else {
       // canonical GEMM order: A -> [g][k][m] (m fastest), B -> [g][k][n], C = [g][m][n]
@@ -524,6 +550,7 @@ int make_plan(const Problem &P, const std::vector<int32_t> &fixed, int force_mod
   out = Plan();
   out.fixed = fixed;
   Planner pl(P, force_mode, enforce_cap, single_arena, want_labels, out, err);
+  pl.gather_friendly_b = force_mode != 2;                 // (the all-tiled test mode keeps its node kinds)
   int rc;
   if ((rc = pl.set_fixed(fixed))) return rc;
   pl.count_occurrences();
