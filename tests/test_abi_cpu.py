@@ -215,6 +215,27 @@ def test_block_tree_plans_use_tiled_gemm_and_trace(lib):
     assert info["n_nodes"] == inst.n_edges + inst.n_vertices - 1
 
 
+def test_small_subtrees_become_a_prologue_and_mid_sized_operands_are_relaid_on_host(lib):
+    # host logic of the launch plan (no device): the small subtrees of the 5x5x5 cube's leaves collapse into one or two
+    # shared-memory launches (api.cu prepare_hybrid) and the planner re-lays the mid-sized gathered operands of its large
+    # nodes (K2 steps in a tree that has no tiled GEMM); BBTN_NO_FUSED keeps one launch per node.  The totals the planner
+    # reports for the tree itself (nodes, FMAs) do not depend on how it is launched.
+    inst = I.ising_lattice_3d(5, 5, 5, 1)
+    fixed = I.layer_fixed_set_3d(5, 5, 5, 8)
+    tree = I.elimination_tree(inst.input_index_sets(fixed), I.min_degree_order(inst, fixed))
+    hyb = bb.Handle(inst, tree=tree).plan_query(fixed, 256)
+    per_node = bb.Handle(inst, tree=tree, flags=bb.BBTN_NO_FUSED).plan_query(fixed, 256)
+    assert hyb["n_nodes"] == per_node["n_nodes"] == 407 and hyb["fma_variant"] == per_node["fma_variant"]
+    assert hyb["n_gemm_tiled"] == 0 and hyb["n_permute"] > 0
+    assert per_node["n_kernel_launches"] == per_node["n_nodes"] + per_node["n_permute"] + 4
+    assert hyb["n_kernel_launches"] < 80
+    # the prologue's outputs get fresh storage behind the planned arenas: a little more workspace, never less
+    assert per_node["workspace_bytes"] <= hyb["workspace_bytes"] <= 1.02 * per_node["workspace_bytes"]
+    # a small network (every tensor of a leaf fits shared memory) is left to the one-launch form
+    small = bb.Handle(I.kings_subgraph(12, 12, 0.8, 1)).plan_query()
+    assert small["n_kernel_launches"] > small["n_nodes"] and small["n_permute"] == 0
+
+
 def test_local_plan_query_and_sweep_order_hints_on_host(lib):
     # bbtn_local_plan_query / bbtn_add_sweep_order need no device: a King's subgraph whose sweep is wider than the threshold
     # gets sliced stretches with small local fixed sets; a hinted order is validated and can only make the plan cheaper
