@@ -599,7 +599,7 @@ def test_config4b_full_size_leaf_by_leaf(bb, oracle, f):
     h = bb.Handle(inst, tree=tree, max_elements_per_leaf=1 << 26)
     energy, count = h.contract_batch(fixed, assign)
     h.close()
-    for b in _sampled_leaves(1 << f, 8 if f == 6 else 16, 200 + f):
+    for b in _sampled_leaves(1 << f, 3 if f == 6 else 16, 200 + f):
         we, wc = oracle.contract_tree(inst, tree[0], tree[1], fixed, assign[b])
         assert (int(energy[b]), int(count[b])) == (we, wc & MASK64), (f, b)
     assert bb.oplus_combine("ising", energy, count)[:2] == _expect("config4b ising 5x5x5 seed 1")
