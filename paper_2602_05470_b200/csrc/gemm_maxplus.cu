@@ -256,7 +256,9 @@ void launch_gemm_maxplus(int64_t batch, int64_t G, int M, int N, int K, int a_km
   a.vecA = (ldA % 4 == 0) && (sA % 4 == 0) && (((int64_t)M * K) % 4 == 0 || G == 1) && al16(A);
   a.vecB = (N % 4 == 0) && (sB % 4 == 0) && (((int64_t)K * N) % 4 == 0 || G == 1) && al16(B);
   a.vecC = (N % 4 == 0) && (sC % 4 == 0) && (((int64_t)M * N) % 4 == 0 || G == 1) && al16(C);
-  const bool small = M <= 64 && N <= 64;                   // a 128-row tile would be >= 75 % padding
+  // the 64 x 64 tile: where a 128-row tile would be >= 75 % padding, and where there are fewer 128 x 128 tiles than SMs
+  const int64_t n_cta128 = (int64_t)((M + 127) / 128) * ((N + 127) / 128) * batch * G;
+  const bool small = (M <= 64 && N <= 64) || n_cta128 < 148;
   const bool p16 = energy_bits <= 11;
 #define BBTN_MP(KM, P, T) launch_mp<KM, P, T>(a, batch, st)
   if (a_kmajor) {

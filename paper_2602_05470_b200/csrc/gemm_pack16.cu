@@ -359,7 +359,10 @@ void launch_gemm_pack16(int64_t batch, int64_t G, int M, int N, int K, int a_kma
   a.vecA = (ldA % 4 == 0) && (sA % 4 == 0) && (((int64_t)M * K) % 4 == 0 || G == 1) && al16(Ae) && al16(Ac);
   a.vecB = (N % 4 == 0) && (sB % 4 == 0) && (((int64_t)K * N) % 4 == 0 || G == 1) && al16(Be) && al16(Bc);
   a.vecC = (N % 4 == 0) && (sC % 4 == 0) && (((int64_t)M * N) % 4 == 0 || G == 1) && al16(Ce) && al16(Cc);
-  const bool small = M <= 64 && N <= 64;                   // a 128-row tile would be >= 75 % padding
+  // the 64 x 64 tile: where a 128-row tile would be >= 75 % padding, and where 128 x 128 tiles would leave SMs idle
+  // (fewer tiles than SMs: four times as many small tiles fill the machine better than the big tile's efficiency costs)
+  const int64_t n_cta128 = (int64_t)((M + 127) / 128) * ((N + 127) / 128) * batch * G;
+  const bool small = (M <= 64 && N <= 64) || n_cta128 < 148;
   int lgK = 0;
   while (((int64_t)1 << lgK) < K) lgK++;
   const int cm = (count_bits <= 16 && 2 * count_bits + lgK <= 32) ? CM_ACC32 : (count_bits <= 13 ? CM_CARRY31 : CM_WIDE64);
