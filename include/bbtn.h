@@ -61,7 +61,7 @@ typedef enum {
 #define BBTN_ENERGY_LIMIT (1 << 28)
 
 /* flags of bbtn_problem_desc.flags */
-#define BBTN_COUNT_CRT 0x1u   /* also keep counts mod P1 and mod P2 (one or two more passes)       */
+#define BBTN_COUNT_CRT 0x1u   /* also keep counts mod P1 and mod P2 (one more pass over the tree)  */
 #define BBTN_IO_DEVICE 0x2u   /* batched calls take/return DEVICE pointers, asynchronous           */
 #define BBTN_NO_GRAPH  0x4u   /* launch kernels one by one instead of replaying a CUDA graph       */
 #define BBTN_FORCE_STREAMING 0x10u /* tuning/testing: never use the tiled GEMM + permute path          */

@@ -502,13 +502,10 @@ int bbtn::run_plan(bbtn_handle *h, DevPlan *dp, const uint8_t *assign, int64_t B
     }
   }
   const bool search = (h->P.flags & BBTN_SEARCH_ONLY) != 0;
-  // CRT mode: the two prime rings run as ONE pass (both residues in one 64-bit count) unless the plan holds a
-  // permute or tiled-GEMM step, whose kernels exist for the single-prime rings only
-  bool stream_only = true;
-  for (const Step &s : dp->plan.steps) if (s.kind == STEP_GEMM) stream_only = false;      // (K2 moves the packed residues as 64-bit words)
-  int rings[3] = {search ? (int)RING_NONE : (int)RING_U64, RING_P1, RING_P2};
-  int n_rings = 1;
-  if (!search && crt && d_mod) { if (stream_only) { rings[1] = RING_P12; n_rings = 2; } else n_rings = 3; }
+  // CRT mode: a second pass with both prime residues in one 64-bit count (every kernel of the path has that form; K2
+  // moves the pair as a 64-bit word)
+  const int rings[2] = {search ? (int)RING_NONE : (int)RING_U64, (int)RING_P12};
+  const int n_rings = (!search && crt && d_mod) ? 2 : 1;
   const bool use_graph = allow_graph && !(h->P.flags & BBTN_NO_GRAPH) && dp->plan.steps.size() >= 8;
   for (int ring = 0; ring < n_rings; ring++) {             // shared-memory opt-in of the kernels that keep a leaf's tensors on chip
     if (dp->fused == 1) configure_fused_tree(rings[ring], dp->plan.max_rank);

@@ -202,6 +202,13 @@ void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmaj
     else launch_v1<R, false, true>(grid, st, G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
     return;
   }
+  if (ring == RING_P12) {                                  // both prime residues packed in one 64-bit count (CRT mode's second pass)
+    using R = RingP12;
+    const uint64_t *ac = (const uint64_t *)Ac, *bc = (const uint64_t *)Bc; uint64_t *cc = (uint64_t *)Cc;
+    if (a_kmajor) launch_v1<R, true, false>(grid, st, G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
+    else launch_v1<R, false, false>(grid, st, G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
+    return;
+  }
   BBTN_RING_DISPATCH3(ring, {
     using CT = typename R::T;
     if (a_kmajor)
