@@ -96,7 +96,7 @@ def solve_king_bbtn(L, seed=1, log2_target=31, crt=True):
     dt = time.perf_counter() - t0
     h.close()
     cnt = bb.crt_combine(out["count"], *out["count_mod"]) if crt else out["count"]
-    rings = 2 if crt else 1         # mod 2^64, then both primes packed (streaming-only plans; else one pass per prime, counted as 2)
+    rings = 2 if crt else 1         # mod 2^64, then both primes packed in one 64-bit count
     return {"instance": f"king {L}x{L} p0.8 seed {seed}", "mode": f"BBTN branching on rho (Eq. 4), T_target = 2^{log2_target}"
             + (", counts mod 2^64 and mod (p1, p2), CRT-combined" if crt else ""),
             "n_vertices": k.n_vertices, "n_edges": k.n_edges, "seconds": dt, "energy": out["energy"],
