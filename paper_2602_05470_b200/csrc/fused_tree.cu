@@ -133,10 +133,8 @@ __global__ void __launch_bounds__(1 << FTB, 1) fused_tree_kernel(int kind, const
     } else if (ring == 0) {
       energy[b] = zero ? NEG_INF : (kind == 0 ? -e : e);
       count[b] = (uint64_t)c;
-    } else if (ring == RING_P12) {
-      if (count_mod) { count_mod[2 * b] = (uint32_t)c; count_mod[2 * b + 1] = (uint32_t)((uint64_t)c >> 32); }
-    } else if (count_mod) {
-      count_mod[2 * b + (ring - 1)] = (uint32_t)c;
+    } else if (count_mod) {                            // RING_P12: the residue mod P1 in the low word, mod P2 in the high word
+      count_mod[2 * b] = (uint32_t)c; count_mod[2 * b + 1] = (uint32_t)((uint64_t)c >> 32);
     }
   }
 }

@@ -209,13 +209,14 @@ void launch_gemm_tiled(int64_t batch, int64_t G, int M, int N, int K, int a_kmaj
     else launch_v1<R, false, false>(grid, st, G, M, N, K, Ae, ac, Be, bc, Ce, cc, sA, sB, sC);
     return;
   }
-  BBTN_RING_DISPATCH3(ring, {
+  {                                                        // RING_U64 with full-width counts on a small matrix
+    using R = RingU64;
     using CT = typename R::T;
     if (a_kmajor)
       launch_v1<R, true, false>(grid, st, G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
     else
       launch_v1<R, false, false>(grid, st, G, M, N, K, Ae, (const CT *)Ac, Be, (const CT *)Bc, Ce, (CT *)Cc, sA, sB, sC);
-  });
+  }
 }
 
 }  // namespace bbtn

@@ -176,10 +176,8 @@ __global__ void finalize_kernel(int kind, int64_t B, const int32_t *__restrict__
     } else if (ring == 0) {
       energy[b] = zero ? NEG_INF : (kind == 0 ? -e : e);
       count[b] = (uint64_t)c;
-    } else if (ring == RING_P12) {
-      if (count_mod) { count_mod[2 * b] = (uint32_t)c; count_mod[2 * b + 1] = (uint32_t)((uint64_t)c >> 32); }
-    } else if (count_mod) {
-      count_mod[2 * b + (ring - 1)] = (uint32_t)c;
+    } else if (count_mod) {                            // RING_P12: the residue mod P1 in the low word, mod P2 in the high word
+      count_mod[2 * b] = (uint32_t)c; count_mod[2 * b + 1] = (uint32_t)((uint64_t)c >> 32);
     }
   }
 }

@@ -7,9 +7,9 @@
 
 namespace bbtn {
 
-// counts mod 2^64 / mod 2^31-1 / mod 2^31-19 / no counts (search mode) / both primes packed in one 64-bit word
-enum RingId : int { RING_U64 = 0, RING_P1 = 1, RING_P2 = 2, RING_NONE = 3, RING_P12 = 4 };
-inline size_t ring_count_bytes(int ring) { return ring == RING_NONE ? 0 : ((ring == RING_U64 || ring == RING_P12) ? 8 : 4); }
+// counts mod 2^64 / no counts (search mode) / mod 2^31-1 and mod 2^31-19 packed in one 64-bit word (CRT mode's second pass)
+enum RingId : int { RING_U64 = 0, RING_NONE = 3, RING_P12 = 4 };
+inline size_t ring_count_bytes(int ring) { return ring == RING_NONE ? 0 : 8; }
 
 constexpr int32_t kNegInf = -(1 << 30);
 constexpr int32_t kZeroThreshold = -(1 << 29);   // e < threshold  <=>  zero element (reading A8)

@@ -97,14 +97,6 @@ template <> struct Vec4<uint64_t> {
   __device__ __forceinline__ void store(uint64_t *p) const { *reinterpret_cast<ulonglong2 *>(p) = a; *reinterpret_cast<ulonglong2 *>(p + 2) = b; }
   __device__ __forceinline__ void set(int u, uint64_t v) { if (u == 0) a.x = v; else if (u == 1) a.y = v; else if (u == 2) b.x = v; else b.y = v; }
 };
-template <> struct Vec4<uint32_t> {
-  uint4 a;
-  __device__ __forceinline__ void load(const uint32_t *p) { a = *reinterpret_cast<const uint4 *>(p); }
-  __device__ __forceinline__ void store(uint32_t *p) const { *reinterpret_cast<uint4 *>(p) = a; }
-  __device__ __forceinline__ void gload(const uint32_t *p) { load(p); }
-  __device__ __forceinline__ void gstore(uint32_t *p) const { store(p); }
-  __device__ __forceinline__ void set(int u, uint32_t v) { if (u == 0) a.x = v; else if (u == 1) a.y = v; else if (u == 2) a.z = v; else a.w = v; }
-};
 
 template <> struct Vec4<NoCount> {
   __device__ __forceinline__ void load(const NoCount *) {}
@@ -228,10 +220,8 @@ bool launch_permute_vec(int rank, const int32_t *perm, const int *inv, int64_t b
   const size_t smem = ((size_t)1 << nt) * (csz + 4);
   if (csz == 8)                                           // mod 2^64, or both prime residues packed: pure data movement
     permute_vec_kernel<uint64_t><<<grid, 256, smem, st>>>(p, src_e, (const uint64_t *)src_c, dst_e, (uint64_t *)dst_c);
-  else if (csz == 0)
-    permute_vec_kernel<NoCount><<<grid, 256, smem, st>>>(p, src_e, (const NoCount *)src_c, dst_e, (NoCount *)dst_c);
   else
-    permute_vec_kernel<uint32_t><<<grid, 256, smem, st>>>(p, src_e, (const uint32_t *)src_c, dst_e, (uint32_t *)dst_c);
+    permute_vec_kernel<NoCount><<<grid, 256, smem, st>>>(p, src_e, (const NoCount *)src_c, dst_e, (NoCount *)dst_c);
   return true;
 }
 }  // namespace
@@ -270,10 +260,8 @@ void launch_permute(int rank, const int32_t *perm, int64_t batch, const int32_t 
   const size_t smem = ((size_t)1 << nt) * (csz + 4);
   if (csz == 8)
     permute_kernel<uint64_t><<<grid, 256, smem, st>>>(p, src_e, (const uint64_t *)src_c, dst_e, (uint64_t *)dst_c);
-  else if (csz == 0)
-    permute_kernel<NoCount><<<grid, 256, smem, st>>>(p, src_e, (const NoCount *)src_c, dst_e, (NoCount *)dst_c);
   else
-    permute_kernel<uint32_t><<<grid, 256, smem, st>>>(p, src_e, (const uint32_t *)src_c, dst_e, (uint32_t *)dst_c);
+    permute_kernel<NoCount><<<grid, 256, smem, st>>>(p, src_e, (const NoCount *)src_c, dst_e, (NoCount *)dst_c);
 }
 
 }  // namespace bbtn

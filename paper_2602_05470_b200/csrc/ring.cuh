@@ -96,20 +96,11 @@ __device__ __forceinline__ void canonicalise(int32_t &e, typename R::T &c) {
 
 }  // namespace bbtn
 
-// dispatch over the three count rings only (kernels the search mode never launches: tiled GEMM, permute)
-#define BBTN_RING_DISPATCH3(ring, ...)                                  \
-  do {                                                                  \
-    if ((ring) == 0) { using R = ::bbtn::RingU64; __VA_ARGS__; }        \
-    else if ((ring) == 1) { using R = ::bbtn::RingP1; __VA_ARGS__; }    \
-    else { using R = ::bbtn::RingP2; __VA_ARGS__; }                     \
-  } while (0)
-
-// dispatch a templated launcher over the ring id
+// dispatch a templated launcher over the ring id.  The two primes only ever run packed (RingP12: CRT mode's second
+// pass), so the single-prime rings RingP1 / RingP2 are building blocks, not launch targets.
 #define BBTN_RING_DISPATCH(ring, ...)                                   \
   do {                                                                  \
     if ((ring) == 0) { using R = ::bbtn::RingU64; __VA_ARGS__; }        \
-    else if ((ring) == 1) { using R = ::bbtn::RingP1; __VA_ARGS__; }    \
-    else if ((ring) == 2) { using R = ::bbtn::RingP2; __VA_ARGS__; }    \
     else if ((ring) == 4) { using R = ::bbtn::RingP12; __VA_ARGS__; }   \
     else { using R = ::bbtn::RingNone; __VA_ARGS__; }                   \
   } while (0)
