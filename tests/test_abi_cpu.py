@@ -124,6 +124,19 @@ def test_no_cpu_fallback(lib):
     with pytest.raises(bb.BbtnError) as e:
         bb.int32_microbench(0, 10)
     assert e.value.status == bb.BBTN_ECUDA
+    # the no-allocation K5 entry point: its size limit is checked before anything touches a device, and without a
+    # device it fails like every other compute call
+    offs, verts = np.array([0, 4, 9], np.int32), np.arange(9, dtype=np.int32)
+    dummy = np.zeros(8, np.int32)
+    with pytest.raises(bb.BbtnError) as e:
+        h.region_bound_static(offs, verts, None, None, dummy, B=(1 << 19) + 1)
+    assert e.value.status == bb.BBTN_ESHAPE and "static scratch" in str(e.value)
+    with pytest.raises(bb.BbtnError) as e:
+        h.region_bound_static(offs, verts, None, None, dummy, B=4)
+    assert e.value.status == bb.BBTN_ECUDA
+    with pytest.raises(bb.BbtnError) as e:
+        h.region_bound_static(offs, verts, None, None, None, B=-1)
+    assert e.value.status == bb.BBTN_EINVAL
 
 
 def test_crt_combine_host():
