@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libbbtn.so")
-CU = ["kernels.cu", "permute.cu", "gemm.cu", "gemm_tiled.cu", "gemm_pack16.cu", "gemm_maxplus.cu", "absorb_vec.cu", "fused_tree.cu", "bound.cu", "microbench.cu", "api.cu", "bound_api.cu", "branching.cu", "local.cu"]
+CU = ["kernels.cu", "permute.cu", "gemm.cu", "gemm_tiled.cu", "gemm_pack16.cu", "gemm_maxplus.cu", "absorb_vec.cu", "absorb_stage.cu", "fused_tree.cu", "bound.cu", "microbench.cu", "api.cu", "bound_api.cu", "branching.cu", "local.cu"]
 CPP = ["plan.cpp"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets"]

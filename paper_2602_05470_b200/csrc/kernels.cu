@@ -230,6 +230,7 @@ void launch_construct(int kind, const InputRec *d_inputs, const int32_t *d_list_
 
 void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs) {
+  if (launch_absorb_stage(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st, xs)) return; // mid-sized B staged in shared memory (absorb_stage.cu)
   if (launch_absorb_vec(s, nb, Ae, Ac, Be, Bc, Ce, Cc, ring, st, xs)) return;   // 16-byte form (absorb_vec.cu)
   AbsorbArgs p;
   p.rO = s.rO; p.nK = s.nK;

@@ -33,6 +33,9 @@ void launch_permute(int rank, const int32_t *perm, int64_t batch, const int32_t 
 void launch_absorb(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);
 bool launch_absorb_vec(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
+                       int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);
+// the same with the tile's footprint of a mid-sized B staged in shared memory (absorb_stage.cu)
+bool launch_absorb_stage(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                        int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);   // false: shape not covered, use launch_absorb's scalar kernel
 void launch_reduce(const Step &s, int64_t nb, const int32_t *Ae, const void *Ac, const int32_t *Be, const void *Bc,
                    int32_t *Ce, void *Cc, int ring, cudaStream_t st, const uint8_t *xs = nullptr);
