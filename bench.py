@@ -523,7 +523,7 @@ def run_ours(args):
         {"kernel": "permute_vec_kernel (K2)", "bound": "hbm", "achieved": perm_bytes / perm_ms / 1e6, "peak": hbm_peak,
          "unit": "GB/s", "frac": perm_bytes / perm_ms / 1e6 / hbm_peak, "ms_per_launch": perm_ms,
          "algorithmic_bytes": perm_bytes, "what": f"2^{perm_rank} elements x 24 B (12 read + 12 written), seeded random bit permutation"},
-        {"kernel": "absorb_vec_kernel + K1/K4 (S1-S4 of the cube, one CUDA-graph replay)", "bound": "hbm",
+        {"kernel": "absorb_vec/absorb_stage kernels + shared-memory prologue + K1/K2/K4 (S1-S4 of the cube, one CUDA-graph replay)", "bound": "hbm",
          "achieved": info["bytes_per_call"] / cube_ms / 1e6, "peak": hbm_peak, "unit": "GB/s",
          "frac": info["bytes_per_call"] / cube_ms / 1e6 / hbm_peak, "ms_per_call": cube_ms,
          "algorithmic_bytes": info["bytes_per_call"], "what": "planner byte total: 12 B per element read or written by every tree node"}]
