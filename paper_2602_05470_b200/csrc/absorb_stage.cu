@@ -113,8 +113,6 @@ __global__ void __launch_bounds__(256) absorb_stage_kernel(StageArgs p, const in
         int32_t acc_e[4]; CT acc_c[4];
         const uint32_t sf = ts[j] + p.sfold[f];
 #pragma unroll
-        for (int u = 0; u < 4; u++) { acc_e[u] = NEG_INF; acc_c[u] = czero<R>(); }
-#pragma unroll
         for (int k = 0; k < 2; k++) {
           if (k < n_k) {
             const uint32_t sk = sf + (k ? p.sk : 0u);
@@ -143,9 +141,14 @@ __global__ void __launch_bounds__(256) absorb_stage_kernel(StageArgs p, const in
                 if (!p.b_unit) cb[u] = ldc<R>(sBc, is);
               }
             }
+            // the first term is taken as it is (a sum below -2^29 is canonicalised to the zero element at the end, exactly as
+            // (+) with the zero element would have left it), the second one is (+)-merged
 #pragma unroll
-            for (int u = 0; u < 4; u++)
-              oplus<R>(acc_e[u], acc_c[u], e4[k][u] + eb[u], p.b_unit ? c4[k].v[u] : R::mul(c4[k].v[u], cb[u]));
+            for (int u = 0; u < 4; u++) {
+              const int32_t e = e4[k][u] + eb[u];
+              const CT c = p.b_unit ? c4[k].v[u] : R::mul(c4[k].v[u], cb[u]);
+              if (k == 0) { acc_e[u] = e; acc_c[u] = c; } else oplus<R>(acc_e[u], acc_c[u], e, c);
+            }
           }
         }
         V4<CT> oc;
