@@ -134,7 +134,11 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
 #pragma unroll
                 for (int u = 0; u < 4; u++) {
                   const uint32_t ib = tbo[j] + kb + fbf + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-                  oplus<R>(acc_e[u], acc_c[u], e4[k][u] + be[ib], p.b_unit ? c4[k].v[u] : R::mul(c4[k].v[u], ldc<R>(bc, ib)));
+                  const int32_t e = e4[k][u] + be[ib];
+                  const CT c = p.b_unit ? c4[k].v[u] : R::mul(c4[k].v[u], ldc<R>(bc, ib));
+                  // the first term is taken as it is (a sum below -2^29 is canonicalised to the zero element below, exactly
+                  // as (+) with the zero element would have left it), the second one is (+)-merged
+                  if (k == 0) { acc_e[u] = e; acc_c[u] = c; } else oplus<R>(acc_e[u], acc_c[u], e, c);
                 }
               }
             }
