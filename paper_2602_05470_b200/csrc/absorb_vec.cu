@@ -175,13 +175,14 @@ __global__ void __launch_bounds__(256) absorb_vec_kernel(AbsorbVecArgs p, const 
           const uint32_t fbf = p.foldB[f];
 #pragma unroll
           for (int u = 0; u < 4; u++) {
-            acc_e[u] = NEG_INF; acc_c[u] = czero<R>();
 #pragma unroll
             for (int k = 0; k < 2; k++) {
               // element index inside the 8: K0: 2u + k;  K1: (u & 1) + 2k + 4(u >> 1)
               const int idx = LP == LP_K0 ? 2 * u + k : (u & 1) + 2 * k + 4 * (u >> 1);
               const uint32_t ib = tbo[j] + fbf + (k ? p.kB[0] : 0u) + ((u & 1) ? ub1 : 0u) + ((u & 2) ? ub2 : 0u);
-              oplus<R>(acc_e[u], acc_c[u], e8[idx] + be[ib], p.b_unit ? c8[idx >> 2].v[idx & 3] : R::mul(c8[idx >> 2].v[idx & 3], ldc<R>(bc, ib)));
+              const int32_t e = e8[idx] + be[ib];
+              const CT c = p.b_unit ? c8[idx >> 2].v[idx & 3] : R::mul(c8[idx >> 2].v[idx & 3], ldc<R>(bc, ib));
+              if (k == 0) { acc_e[u] = e; acc_c[u] = c; } else oplus<R>(acc_e[u], acc_c[u], e, c);      // (first term assigned, as above)
             }
           }
           V4<CT> oc;
