@@ -105,7 +105,7 @@ def solve_king_bbtn(L, seed=1, log2_target=31, crt=True):
             "algorithmic_gb_per_s": out["bytes"] * rings / dt / 1e9}
 
 
-def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None):
+def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None, search=False):
     """BBTN on sub-networks (bbtn_solve_local): local fixed sets per overflowing stretch of the tree, K5 region bounds
     against the caller's incumbent (if any) on every branch."""
     k = I.kings_subgraph(L, L, 0.8, seed)
@@ -116,7 +116,8 @@ def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None):
         for c0 in range(0, L, block):
             verts += [int(ids[r][c]) for r in range(r0, min(r0 + block, L)) for c in range(c0, min(c0 + block, L)) if ids[r][c] >= 0]
             offs.append(len(verts))
-    h = bb.Handle(k, flags=bb.BBTN_COUNT_CRT if crt else 0)
+    crt = crt and not search
+    h = bb.Handle(k, flags=bb.BBTN_SEARCH_ONLY if search else (bb.BBTN_COUNT_CRT if crt else 0))
     h.add_sweep_order(I.column_major_order(k))          # the library also tries sweeps along the columns
     t0 = time.perf_counter()
     plan = h.local_plan_query(log2_target)
@@ -129,7 +130,8 @@ def solve_king_local(L, seed=1, log2_target=32, crt=True, block=4, hint=None):
     cnt = bb.crt_combine(out["count"], *out["count_mod"]) if crt else out["count"]
     rings = 2 if crt else 1                             # mod 2^64, then both primes packed in one 64-bit count: 12 B/element each
     return {"instance": f"king {L}x{L} p0.8 seed {seed}", "mode": f"BBTN on sub-networks (bbtn_solve_local), T_target = 2^{log2_target}"
-            + (", counts mod 2^64, then (p1, p2) packed (2 passes) CRT-combined" if crt else ""),
+            + (", counts mod 2^64, then (p1, p2) packed (2 passes) CRT-combined" if crt else "")
+            + (", search mode (energy plane only, 4 B per element; the count reads 0)" if search else ""),
             "n_vertices": k.n_vertices, "n_edges": k.n_edges, "seconds": dt, "plan_only_seconds": t_plan, "energy": out["energy"],
             "count_mod_2_64": out["count"], "count": str(cnt), **{key: out[key] for key in bb.Handle._LOCAL_STATS},
             "fma": out["fma"] * rings, "bytes": out["bytes"] * rings,
@@ -156,7 +158,7 @@ def main():
     ap.add_argument("--configs", nargs="*", default=["1", "2", "3", "4b", "5"])
     ap.add_argument("--king-sizes", nargs="*", type=int, default=[16, 20, 24])
     ap.add_argument("--bbtn", nargs="*", default=[], help="L:seed:log2_target[:crt] runs of bbtn_solve_branching, e.g. 32:1:31:1")
-    ap.add_argument("--local", nargs="*", default=[], help="L:seed:log2_target[:crt] runs of bbtn_solve_local, e.g. 40:1:32:1")
+    ap.add_argument("--local", nargs="*", default=[], help="L:seed:log2_target[:mode] runs of bbtn_solve_local, mode 0 = mod 2^64, 1 = CRT, 2 = search; e.g. 40:1:32:1")
     ap.add_argument("--e1", nargs="*", type=int, default=[], help="lattice sizes L for the paper's +-J, h = 0.5 setting, unbranched")
     ap.add_argument("--repeat", type=int, default=5)
     a = ap.parse_args()
@@ -187,7 +189,7 @@ def main():
         emit(solve_e1(L))
     for spec in a.local:
         f = [int(x) for x in spec.split(":")]
-        emit(solve_king_local(f[0], f[1], f[2], crt=bool(f[3]) if len(f) > 3 else False))
+        emit(solve_king_local(f[0], f[1], f[2], crt=len(f) > 3 and f[3] == 1, search=len(f) > 3 and f[3] == 2))
     for spec in a.bbtn:
         f = [int(x) for x in spec.split(":")]
         emit(solve_king_bbtn(f[0], f[1], f[2], crt=bool(f[3]) if len(f) > 3 else False))
