@@ -203,7 +203,9 @@ void prepare_hybrid(bbtn_handle *h, DevPlan *dp) {
   dp->hybrid = 0;
   Plan &pl = dp->plan;
   if ((h->P.flags & BBTN_NO_FUSED) || pl.steps.size() < 48) return;
-  if (pl.max_rank <= 13 && pl.arena_variant_elems + pl.arena_invariant_elems <= 60000) return;   // a candidate for the one-launch form
+  if (pl.max_rank <= 13 && pl.arena_variant_elems + pl.arena_invariant_elems <= 60000 &&
+      (int64_t)fused_tree_smem_bytes((int)(pl.arena_variant_elems + pl.arena_invariant_elems), RING_U64) <= 227 * 1024 - 1024)
+    return;                                                // the one-launch form takes it (prepare_fused)
   const int n_in = (int)pl.inputs.size(), n_st = (int)pl.steps.size();
   std::map<std::pair<int, int64_t>, int> owner;              // (arena, offset) -> the tensor stored there right now
   for (int t = 0; t < n_in; t++) if (pl.inputs[t].rank > 0) owner[{pl.inputs[t].variant, pl.inputs[t].offset}] = t;
@@ -284,6 +286,11 @@ void prepare_hybrid(bbtn_handle *h, DevPlan *dp) {
                                   dp->hyb[g].build_off = std::move(gnew[g].build_off); dp->hyb[g].arena = gnew[g].arena; dp->hyb[g].max_rank = gnew[g].max_rank; }
     pl.arena_invariant_elems += ext[0]; pl.arena_variant_elems += ext[1];
     dp->hyb_rank = R;
+    // One CTA per leaf walks hundreds of nodes at ~0.5 us each, so the prologue's time grows with the number of waves of
+    // CTAs, while the per-node launches it replaces cost a few microseconds each whatever the batch: use it up to two waves
+    // (measured on the 24x24 lattice: 256 leaves 18.0 -> 17.1 ms, 1024 leaves 20.4 -> 21.2 ms, 4096 leaves 34 -> 46 ms)
+    const int64_t per_cta = (int64_t)fused_tree_smem_bytes(dp->hyb[1].arena, RING_U64) + 1024;
+    dp->hyb_max_B = dp->hyb[1].steps.empty() ? INT64_MAX : 2 * 148 * std::max<int64_t>(1, (227 * 1024) / per_cta);
     dp->hybrid = 1;
     return;
   }
@@ -327,7 +334,8 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
   while (energy_bits < 32 && ((int64_t)1 << energy_bits) <= h->P.energy_range) energy_bits++;
   auto pe = [&](int v, int64_t off) { return v ? ve + off * B : ie + off; };
   auto pc = [&](int v, int64_t off) { return (void *)(v ? vc + (size_t)off * B * csz : ic + (size_t)off * csz); };
-  if (dp->hybrid == 1)                                   // the small subtrees of every leaf, in shared memory (prepare_hybrid)
+  const bool hyb = dp->hybrid == 1 && B <= dp->hyb_max_B;
+  if (hyb)                                               // the small subtrees of every leaf, in shared memory (prepare_hybrid)
     for (int g = 0; g < 2; g++) {
       const DevPlan::HybridGroup &hg = dp->hyb[g];
       if (hg.steps.empty()) continue;
@@ -337,7 +345,7 @@ void enqueue_ring(const bbtn_handle *h, DevPlan *dp, int64_t B, const uint8_t *d
                         d_assign, (int)pl.fixed.size(), g ? B : 1, (const FusedStep *)hg.d_steps.p, (int)hg.steps.size(), hg.arena, 0, -1,
                         nullptr, nullptr, nullptr, ring, hg.max_rank, st, fg);
     }
-  for (const Step &s : dp->hybrid == 1 ? dp->hyb_big : pl.steps) {
+  for (const Step &s : hyb ? dp->hyb_big : pl.steps) {
     const int64_t nb = s.variant ? B : 1;
     switch (s.kind) {
       case STEP_ABSORB:
@@ -446,7 +454,7 @@ int bbtn_plan_query(bbtn_handle *h, const int32_t *fixed, int32_t n_fixed, int64
   for (const InputRec &r : pl.inputs) if (r.rank > 0) (r.variant ? n_var : n_inv)++;
   // K1: variant tensors, invariant tensors, offset[b]; K4: finalize
   info->n_kernel_launches = (int32_t)pl.steps.size() + (n_var > 0) + (n_inv > 0) + 2;
-  if (dp->hybrid == 1)                                   // small subtrees run as one or two shared-memory prologue launches
+  if (dp->hybrid == 1 && B <= dp->hyb_max_B)             // small subtrees run as one or two shared-memory prologue launches
     info->n_kernel_launches = (int32_t)dp->hyb_big.size() + !dp->hyb[0].steps.empty() + !dp->hyb[1].steps.empty() + (n_var > 0) + (n_inv > 0) + 2;
   return BBTN_OK;
 }

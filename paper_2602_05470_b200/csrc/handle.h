@@ -54,6 +54,7 @@ struct DevPlan {
   } hyb[2];
   std::vector<Step> hyb_big;                    // the steps that stay per-node launches, operands re-pointed at the prologue's outputs
   int hyb_rank = 0;
+  int64_t hyb_max_B = 0;                        // the prologue pays while its CTAs fit about two waves; beyond, node-by-node launches batch better
   bool tables_ready = false;
   int64_t B_cap = 0;
   std::vector<cudaGraphExec_t> graphs;          // per ring, for graph_B
