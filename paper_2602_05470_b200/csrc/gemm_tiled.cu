@@ -365,7 +365,10 @@ void launch_gemm_tiled_u64(int64_t batch, int64_t G, int M, int N, int K, int a_
   if (mode != WIDE && energy_bits <= 11) {
     launch_gemm_pack16(batch, G, M, N, K, a_kmajor, Ae, Ac, Be, Bc, Ce, Cc, sA, sB, sC, count_bits, st);
   } else if (mode == ACC32) {
-    if (a_kmajor) launch_one<ACC32, true, 2>(a, batch, st); else launch_one<ACC32, false, 2>(a, batch, st);
+    // fewer 128 x 128 tiles than SMs: the 128 x 64 tile doubles the CTAs
+    const int64_t n_cta128 = (int64_t)((M + 127) / 128) * ((N + 127) / 128) * batch * G;
+    if (n_cta128 < 148) { if (a_kmajor) launch_one<ACC32, true, 1>(a, batch, st); else launch_one<ACC32, false, 1>(a, batch, st); }
+    else if (a_kmajor) launch_one<ACC32, true, 2>(a, batch, st); else launch_one<ACC32, false, 2>(a, batch, st);
   } else if (mode == NARROW64) {
     if (a_kmajor) launch_one<NARROW64, true, 1>(a, batch, st); else launch_one<NARROW64, false, 1>(a, batch, st);
   } else if (mode == ACC64N) {
